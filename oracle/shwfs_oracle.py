@@ -1,0 +1,219 @@
+"""ctypes front end of the float64 CPU oracle (oracle/shwfs_oracle.c).
+
+TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs may import this module.  It
+imports nothing from paper_1408_0698_b200 and shares no code with the CUDA path.
+
+Every function is a thin marshalling layer over one C function whose header
+comment cites the passage it follows (PAPER.md:91 and the O1..O9 steps of
+SURVEY.md 8(c)); there is no arithmetic of the method in this file.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "shwfs_oracle.c"
+_LIB = _HERE / "libshwfs_oracle.so"
+_lib = None
+
+
+def build(force: bool = False) -> Path:
+    """Compile shwfs_oracle.c -> libshwfs_oracle.so with gcc -O2 -fopenmp (the oracle as it stands)."""
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = _LIB.with_suffix(f".tmp{os.getpid()}.so")
+        cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
+               "-o", str(tmp), str(_SRC), "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_f32p = np.ctypeslib.ndpointer(dtype=np.float32, flags="C_CONTIGUOUS")
+_f64p = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
+_i32p = np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(str(_LIB))
+        L.shwfs_oracle_field.argtypes = [_f32p, _f32p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
+                                         C.c_double, _f64p]
+        L.shwfs_oracle_field.restype = None
+        L.shwfs_oracle_dft1.argtypes = [_f64p, _f64p, C.c_int, C.c_int]
+        L.shwfs_oracle_dft1.restype = None
+        L.shwfs_oracle_dft2.argtypes = [_f64p, _f64p, C.c_int, C.c_int]
+        L.shwfs_oracle_dft2.restype = C.c_int
+        L.shwfs_oracle_dft2_brute.argtypes = [_f64p, _f64p, C.c_int, C.c_int]
+        L.shwfs_oracle_dft2_brute.restype = None
+        L.shwfs_oracle_intensity.argtypes = [_f64p, C.c_int, _f64p]
+        L.shwfs_oracle_intensity.restype = None
+        L.shwfs_oracle_convolve_direct.argtypes = [_f64p, _f32p, C.c_int, _f64p]
+        L.shwfs_oracle_convolve_direct.restype = None
+        L.shwfs_oracle_convolve_fft.argtypes = [_f64p, _f32p, C.c_int, _f64p]
+        L.shwfs_oracle_convolve_fft.restype = C.c_int
+        L.shwfs_oracle_centre.argtypes = [_f64p, C.c_int, _f64p]
+        L.shwfs_oracle_centre.restype = None
+        L.shwfs_oracle_bin.argtypes = [_f64p, C.c_int, C.c_int, _f64p]
+        L.shwfs_oracle_bin.restype = None
+        L.shwfs_oracle_threshold_cog.argtypes = [_f64p, C.c_int, C.c_double, C.c_int, _f64p]
+        L.shwfs_oracle_threshold_cog.restype = None
+        L.shwfs_oracle_valid_list.argtypes = [_f32p, C.c_int, C.c_int, C.c_double, C.c_void_p]
+        L.shwfs_oracle_valid_list.restype = C.c_int
+        L.shwfs_oracle_measure.argtypes = [_f32p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _f32p, _i32p,
+                                           C.c_int, C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_int,
+                                           _f64p, C.c_int, C.c_void_p, C.c_int]
+        L.shwfs_oracle_measure.restype = C.c_int
+        L.shwfs_oracle_max_threads.argtypes = []
+        L.shwfs_oracle_max_threads.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _c(a, dt):
+    return np.ascontiguousarray(a, dtype=dt)
+
+
+def _cplx_in(z, P):
+    z = np.ascontiguousarray(z, dtype=np.complex128).reshape(P, P)
+    return z.view(np.float64).reshape(P, 2 * P)
+
+
+def field(phase_frame, amplitude, n, P, sy, sx, c_phi=1.0):
+    """O1+O2: complex P x P field of subaperture (sy,sx) (patch in the corner, zero padded)."""
+    ph = _c(phase_frame, np.float32)
+    am = _c(amplitude, np.float32)
+    N = ph.shape[-1]
+    out = np.zeros((P, 2 * P), dtype=np.float64)
+    lib().shwfs_oracle_field(ph, am, N, n, P, sy, sx, float(c_phi), out)
+    return out.view(np.complex128).reshape(P, P)
+
+
+def dft1(x, sign=-1):
+    x = np.ascontiguousarray(x, dtype=np.complex128)
+    L = x.shape[0]
+    out = np.zeros(2 * L, dtype=np.float64)
+    lib().shwfs_oracle_dft1(x.view(np.float64), out, L, sign)
+    return out.view(np.complex128)
+
+
+def dft2(x, sign=-1):
+    """O3: unnormalised 2-D DFT with exp(sign*2*pi*i*...) (naive for P<=16, radix-2 above)."""
+    P = x.shape[0]
+    out = np.zeros((P, 2 * P), dtype=np.float64)
+    rc = lib().shwfs_oracle_dft2(_cplx_in(x, P), out, P, sign)
+    if rc:
+        raise MemoryError("oracle dft2")
+    return out.view(np.complex128).reshape(P, P)
+
+
+def dft2_brute(x, sign=-1):
+    P = x.shape[0]
+    out = np.zeros((P, 2 * P), dtype=np.float64)
+    lib().shwfs_oracle_dft2_brute(_cplx_in(x, P), out, P, sign)
+    return out.view(np.complex128).reshape(P, P)
+
+
+def intensity(E):
+    """O4: |E|^2 / P^2."""
+    P = E.shape[0]
+    out = np.zeros((P, P), dtype=np.float64)
+    lib().shwfs_oracle_intensity(_cplx_in(E, P), P, out)
+    return out
+
+
+def convolve(I, K, direct=False):
+    """O5: circular convolution, kernel centre at (P/2, P/2)."""
+    I = _c(I, np.float64)
+    K = _c(K, np.float32)
+    P = I.shape[0]
+    out = np.zeros((P, P), dtype=np.float64)
+    if direct:
+        lib().shwfs_oracle_convolve_direct(I, K, P, out)
+    elif lib().shwfs_oracle_convolve_fft(I, K, P, out):
+        raise MemoryError("oracle convolve")
+    return out
+
+
+def centre(Cimg):
+    """O6: roll by P/2 on both axes."""
+    Cimg = _c(Cimg, np.float64)
+    P = Cimg.shape[0]
+    out = np.zeros((P, P), dtype=np.float64)
+    lib().shwfs_oracle_centre(Cimg, P, out)
+    return out
+
+
+def bin_image(Sh, b):
+    """O7: b x b block sums."""
+    Sh = _c(Sh, np.float64)
+    P = Sh.shape[0]
+    D = P // b
+    out = np.zeros((D, D), dtype=np.float64)
+    lib().shwfs_oracle_bin(Sh, P, b, out)
+    return out
+
+
+def threshold_cog(B, tau=0.0, mode=0):
+    """O8+O9: thresholded centre of gravity, returns (s_x, s_y) in detector pixels."""
+    B = _c(B, np.float64)
+    D = B.shape[0]
+    out = np.zeros(2, dtype=np.float64)
+    lib().shwfs_oracle_threshold_cog(B, D, float(tau), int(mode), out)
+    return out
+
+
+def valid_list(amplitude, n, min_illum=0.5):
+    """H0 / reading A2: (sy,sx) of subapertures with mean amplitude >= min_illum, row-major."""
+    am = _c(amplitude, np.float32)
+    N = am.shape[0]
+    S = N // n
+    yx = np.zeros((S * S, 2), dtype=np.int32)
+    cnt = lib().shwfs_oracle_valid_list(am, N, n, float(min_illum), yx.ctypes.data_as(C.c_void_p))
+    return yx[:cnt].copy()
+
+
+def max_threads() -> int:
+    return int(lib().shwfs_oracle_max_threads())
+
+
+def measure(phase, amplitude, valid_yx, n, P, b, *, c_phi=1.0, tau=0.0, mode=0, kernels=None,
+            conv_direct=False, stage=-1, nthreads=0):
+    """O1..O9 for every frame and valid subaperture.
+
+    phase [T,N,N] fp32, amplitude [N,N] fp32, valid_yx [nsub,2] int32, kernels [nsub,P,P] fp32 or None.
+    Returns slopes [T,nsub,2] float64, or (slopes, images) if stage in {0,1,2}:
+    0 = centred intensity [T,nsub,P,P], 1 = centred convolved image, 2 = binned image [T,nsub,D,D].
+    """
+    ph = _c(phase, np.float32)
+    if ph.ndim == 2:
+        ph = ph[None]
+    T, N, _ = ph.shape
+    am = _c(amplitude, np.float32)
+    yx = _c(valid_yx, np.int32)
+    nsub = yx.shape[0]
+    slopes = np.zeros((T, nsub, 2), dtype=np.float64)
+    kptr = None
+    if kernels is not None:
+        kernels = _c(kernels, np.float32)
+        assert kernels.shape == (nsub, P, P), kernels.shape
+        kptr = kernels.ctypes.data_as(C.c_void_p)
+    images = None
+    iptr = None
+    if stage >= 0:
+        D = P // b
+        shp = (T, nsub, D, D) if stage == 2 else (T, nsub, P, P)
+        images = np.zeros(shp, dtype=np.float64)
+        iptr = images.ctypes.data_as(C.c_void_p)
+    rc = lib().shwfs_oracle_measure(ph, T, N, n, P, b, am, yx, nsub, float(c_phi), float(tau), int(mode),
+                                    kptr, int(bool(conv_direct)), slopes, int(stage), iptr, int(nthreads))
+    if rc:
+        raise RuntimeError(f"shwfs_oracle_measure failed with code {rc}")
+    return (slopes, images) if stage >= 0 else slopes

@@ -1,0 +1,177 @@
+"""Seeded synthetic inputs for the Shack-Hartmann WFS hot path (numpy only).
+
+This module serves BOTH the CUDA library and the CPU oracle with identical arrays and therefore holds
+none of the method's arithmetic: it only makes *inputs* -- pupil amplitude masks, von Karman phase screens
+and LGS elongation kernels -- with the shapes, sizes and statistics of the paper's MAORY workloads
+("800x800 ... 4.875e-2 m"; "FFT from the Kolmogorov or Von Karman models of the
+phase Power Spectrum"; "80x80 subapertures") and of BASELINE.json:configs.  The paper's own
+.fits wavefront histories are not available; these stand in for them.
+
+It imports neither the oracle nor the CUDA binding.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass
+
+import numpy as np
+
+ARCSEC = math.pi / (180.0 * 3600.0)
+LAMBDA_M = 0.589e-6          # sensing wavelength, sodium line (BASELINE.json:configs[0])
+R0_M = 0.15                  # Fried parameter at 0.5 um   (BASELINE.json:configs[0])
+L0_M = 25.0                  # outer scale                 (BASELINE.json:configs[0])
+SEED0 = 14080698
+
+
+@dataclass(frozen=True)
+class WfsConfig:
+    """One row of the config table in SURVEY.md section 8 (BASELINE.json:configs[k-1])."""
+    cfg: int            # 1..5
+    name: str
+    N: int              # pupil grid side
+    dx: float           # metres per pupil pixel
+    S: int              # subapertures per side
+    n: int              # phase px per subaperture side
+    P: int              # zero-padded FFT side
+    b: int              # binning
+    W: int              # number of WFS
+    T: int              # frames per WFS
+    batch: int          # frames per shwfs_measure call
+    r_out: float        # pupil outer radius [m]
+    r_in: float         # central obstruction radius [m]
+    tau: float          # CoG threshold fraction
+    elong_max_arcsec: float   # long-axis FWHM at the farthest subaperture; 0 = no elongation
+    screen_M: int       # side of the FFT grid the screens are filtered on
+    min_illum: float = 0.5
+    fwhm_short_arcsec: float = 1.0
+
+    @property
+    def D(self) -> int:
+        return self.P // self.b
+
+    @property
+    def pixel_scale_arcsec(self) -> float:
+        """Unbinned focal-plane pixel, lambda / (P dx)."""
+        return LAMBDA_M / (self.P * self.dx) / ARCSEC
+
+
+CONFIGS = {
+    1: WfsConfig(1, "tiny", 80, 0.10, 10, 8, 16, 1, 1, 4, 4, 4.0, 0.0, 0.0, 0.0, 256),
+    2: WfsConfig(2, "8m", 640, 0.0125, 40, 16, 32, 2, 1, 100, 100, 4.0, 0.8, 0.10, 0.0, 1024),
+    3: WfsConfig(3, "lgs1", 800, 0.04875, 80, 10, 32, 2, 1, 100, 100, 19.5, 5.5, 0.10, 4.0, 1024),
+    4: WfsConfig(4, "lgs6", 800, 0.04875, 80, 10, 32, 2, 6, 1000, 100, 19.5, 5.5, 0.10, 4.0, 1024),
+    5: WfsConfig(5, "stress", 1280, 0.030468750, 80, 16, 64, 4, 6, 1000, 100, 19.5, 5.5, 0.10, 6.0, 2048),
+}
+
+
+def seed_for(cfg: int, wfs: int, frame: int) -> int:
+    """seed = 14080698 + 100000*cfg + 1000*wfs + frame."""
+    return SEED0 + 100000 * cfg + 1000 * wfs + frame
+
+
+def pupil_mask(c: WfsConfig) -> np.ndarray:
+    """Reading A1: a[y,x] = 1 where r_in <= r <= r_out at the pixel centre, else 0 (fp32 [N,N])."""
+    ax = (np.arange(c.N, dtype=np.float64) + 0.5 - c.N / 2.0) * c.dx
+    r = np.hypot(ax[None, :], ax[:, None])
+    return ((r >= c.r_in) & (r <= c.r_out)).astype(np.float32)
+
+
+def _psd_filter(M: int, dx: float) -> np.ndarray:
+    f = np.fft.fftfreq(M, dx)
+    f2 = f[None, :] ** 2 + f[:, None] ** 2
+    psd = 0.022896 * R0_M ** (-5.0 / 3.0) * (f2 + L0_M ** -2.0) ** (-11.0 / 6.0)
+    psd[0, 0] = 0.0
+    return np.sqrt(psd) / dx
+
+
+_FILTERS: dict = {}
+
+
+def phase_screen(c: WfsConfig, wfs: int, frame: int) -> np.ndarray:
+    """One von Karman screen in radians at 0.589 um, fp32 [N,N] (recipe of SURVEY.md 8(d))."""
+    key = (c.screen_M, c.dx)
+    if key not in _FILTERS:
+        _FILTERS[key] = _psd_filter(c.screen_M, c.dx)
+    w = np.random.default_rng(seed_for(c.cfg, wfs, frame)).standard_normal((c.screen_M, c.screen_M))
+    scr = np.real(np.fft.ifft2(np.fft.fft2(w) * _FILTERS[key]))
+    scr *= 0.5 / 0.589
+    return np.ascontiguousarray(scr[: c.N, : c.N], dtype=np.float32)
+
+
+def phase_frames(c: WfsConfig, wfs: int, frames) -> np.ndarray:
+    """Stack of screens [len(frames), N, N] fp32."""
+    return np.stack([phase_screen(c, wfs, int(t)) for t in frames], axis=0)
+
+
+def launch_point(c: WfsConfig, wfs: int):
+    """Reading A13: launch telescope of WFS w at the pupil edge, 60 deg apart."""
+    ang = math.radians(60.0 * wfs)
+    return c.r_out * math.cos(ang), c.r_out * math.sin(ang)
+
+
+def elongation_params(c: WfsConfig, wfs: int, valid_yx: np.ndarray):
+    """Readings A11-A13: per-subaperture (sigma_long, sigma_short, theta) in unbinned pixels / radians."""
+    yx = np.asarray(valid_yx, dtype=np.float64)
+    yc = ((yx[:, 0] + 0.5) * c.n - c.N / 2.0) * c.dx
+    xc = ((yx[:, 1] + 0.5) * c.n - c.N / 2.0) * c.dx
+    lx, ly = launch_point(c, wfs)
+    d = np.hypot(xc - lx, yc - ly)
+    e_max = math.sqrt(c.elong_max_arcsec ** 2 - c.fwhm_short_arcsec ** 2)
+    fwhm_l = np.sqrt(c.fwhm_short_arcsec ** 2 + (e_max * d / d.max()) ** 2)
+    to_sigma = 1.0 / (2.0 * math.sqrt(2.0 * math.log(2.0))) / c.pixel_scale_arcsec
+    theta = np.arctan2(yc - ly, xc - lx)
+    return fwhm_l * to_sigma, np.full_like(d, c.fwhm_short_arcsec * to_sigma), theta
+
+
+def elongation_kernels(c: WfsConfig, wfs: int, valid_yx: np.ndarray, subset=None, device=None,
+                       chunk: int = 64):
+    """Wrapped (periodically summed) rotated Gaussians, normalised to sum 1 in float64, cast to fp32.
+
+    K_i[r,c] = sum_{m,l=-M..M} g(c-P/2+l*P, r-P/2+m*P),
+    g(x,y) = exp(-((x cos t + y sin t)^2 / sL^2 + (-x sin t + y cos t)^2 / sS^2) / 2),  M = ceil(6 sL / P) + 1
+    (readings A11-A13; the quadratic form is expanded to A x^2 + 2 B x y + C y^2 before the
+    exponential, nothing else).  The per-subaperture parameters always come from the FULL valid list;
+    `subset` (indices into it) restricts which kernels are evaluated.  Returns fp32 [len(subset),P,P]: a
+    numpy array, or -- when `device` is a torch device -- a torch tensor on it (same formula in torch
+    float64, for speed at the full sizes).  Returns None when the config has no elongation.
+    """
+    if c.elong_max_arcsec <= 0.0:
+        return None
+    s_l, s_s, th = elongation_params(c, wfs, valid_yx)
+    P = c.P
+    wraps = int(math.ceil(6.0 * float(s_l.max()) / P)) + 1
+    if subset is not None:
+        subset = np.asarray(subset, dtype=np.int64)
+        s_l, s_s, th = s_l[subset], s_s[subset], th[subset]
+    qa = 0.5 * (np.cos(th) ** 2 / s_l ** 2 + np.sin(th) ** 2 / s_s ** 2)       # exponent = -(qa x^2
+    qc = 0.5 * (np.sin(th) ** 2 / s_l ** 2 + np.cos(th) ** 2 / s_s ** 2)       #   + qb x y + qc y^2)
+    qb = np.cos(th) * np.sin(th) * (1.0 / s_l ** 2 - 1.0 / s_s ** 2)
+    nw = 2 * wraps + 1
+    ax_np = ((np.arange(P, dtype=np.float64) - P / 2.0)[None, :]
+             + (np.arange(-wraps, wraps + 1, dtype=np.float64) * P)[:, None]).reshape(-1)
+    if device is None:
+        xp, ax = np, ax_np
+        as_x = lambda a: np.asarray(a, dtype=np.float64)
+        out = np.empty((len(s_l), P, P), dtype=np.float32)
+    else:
+        import torch
+        xp = torch
+        as_x = lambda a: torch.as_tensor(np.asarray(a, dtype=np.float64), device=device)
+        ax = as_x(ax_np)
+        out = torch.empty((len(s_l), P, P), dtype=torch.float32, device=device)
+    xy = ax[None, :, None] * ax[None, None, :]                  # y (rows) times x (columns)
+    x2 = (ax * ax)[None, None, :]
+    y2 = (ax * ax)[None, :, None]
+    for i0 in range(0, len(s_l), chunk):
+        a_, b_, c_ = (as_x(q[i0:i0 + chunk])[:, None, None] for q in (qa, qb, qc))
+        g = xy * b_
+        g += x2 * a_
+        g += y2 * c_
+        g = xp.exp(-g)
+        g = g.reshape(-1, nw, P, nw, P).sum(axis=3).sum(axis=1)   # periodic sum over image cells
+        g = g / g.sum(axis=(1, 2)).reshape(-1, 1, 1)
+        if xp is np:
+            out[i0:i0 + chunk] = g.astype(np.float32)
+        else:
+            out[i0:i0 + chunk] = g.to(out.dtype)
+    return out
