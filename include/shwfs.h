@@ -1,0 +1,131 @@
+/*
+ * shwfs.h -- C ABI of the B200-native Shack-Hartmann wavefront-sensor hot path.
+ *
+ * The operation is the LGS/NGS Shack-Hartmann sensor module of PAPER.md:91 (section 4):
+ *   "The WF is split into sub-apertures and the spot computed by FFT for each sensor sub-aperture.
+ *    [...] We consider the physical extension of the projection of the laser on the sodium layer
+ *    through a convolution for a gaussian of the desired properties. [...] the centroid computed on
+ *    the final [...] image to retrieve the slopes."
+ * and its output is the "X- and Y- slopes" vector of PAPER.md:76.  The call set follows
+ * BASELINE.json:north_star: shwfs_create(geometry, lambda, pad, binning, elongation kernels),
+ * shwfs_measure(phase[T,N,N] fp32 device ptr -> slopes[T,nsub,2], stream), shwfs_destroy.
+ * The paper gives no formula; the conventions (steps H1..H8, readings A1..A15) are those of
+ * SURVEY.md section 8 and DESIGN.md sections 2-4.
+ *
+ * Per (frame t, valid subaperture i):
+ *   H1 gather   p[j,k] = phase[t, sy*n+j, sx*n+k],  a[j,k] = amplitude[sy*n+j, sx*n+k]
+ *   H2 field    e[j,k] = a * exp(i*(phase_to_rad*p - pi*(j+k)/P)), zero padded to P x P
+ *   H3 DFT      E[v,u] = sum e[j,k] exp(-2*pi*i*(v*j+u*k)/P)
+ *   H4          I = |E|^2 / P^2
+ *   H5          C = I (*) K_i, circular on P x P, kernel centre at (P/2,P/2)   (only if kernels given)
+ *   H6 centre   Sh[r,c] = C[(r-P/2) mod P, (c-P/2) mod P];  bin  B[R,C] = sum of b x b blocks
+ *   H7          m = max B;  Wt = max(B - tau*m, 0)  (mode 0)  |  B*[B >= tau*m]  (mode 1)
+ *   H8          slope_x = sum Wt*(C-(D-1)/2) / sum Wt,  slope_y with R;  sum Wt == 0 -> (0,0)
+ * All arithmetic is fp32 on the device.  How the library reaches that result (lag-domain form,
+ * pruned transforms) is an implementation matter: DESIGN.md section 6.
+ *
+ * Conventions
+ *   - Every function returns 0 (SHWFS_OK) or a negative error code; nothing throws, aborts or exits;
+ *     output arguments are untouched on failure.
+ *   - "HOST" pointers are ordinary host memory, "DEVICE" pointers are CUDA device memory of the
+ *     device that was current at shwfs_create.  shwfs_create copies every HOST array it is given.
+ *   - shwfs_measure / shwfs_debug_spots only enqueue work on `cuda_stream` (a cudaStream_t passed
+ *     as void*, NULL = default stream): no allocation, no synchronisation, no host<->device copy.
+ *     Results are valid once the caller has synchronised that stream.
+ *   - A handle is not thread-safe; distinct handles are independent (one handle = one WFS).
+ */
+#ifndef SHWFS_H_
+#define SHWFS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SHWFS_OK            0
+#define SHWFS_EINVAL       (-1)  /* null pointer, inconsistent sizes, T < 0, no valid subaperture      */
+#define SHWFS_EUNSUPPORTED (-2)  /* sizes are consistent but no kernel instance covers them            */
+#define SHWFS_ENOMEM       (-3)  /* host or device allocation failed                                   */
+#define SHWFS_ECUDA        (-4)  /* a CUDA call failed; shwfs_last_cuda_error gives the CUDA text      */
+
+/* Algorithms.  Both give the H1..H8 result to fp32 rounding. */
+#define SHWFS_ALGO_AUTO     0    /* the fastest instance for the handle's sizes (default)              */
+#define SHWFS_ALGO_LITERAL  1    /* P x P shared-memory FFT chain, exactly the H3..H6 order             */
+#define SHWFS_ALGO_WK       2    /* Wiener-Khinchin lag-domain form: autocorrelation of the field, x   */
+                                 /* precomputed (kernel MTF x bin x centre) table, D x D real transform */
+#define SHWFS_ALGO_WK_GENERIC 3  /* same form, size-generic unspecialised kernel                       */
+
+typedef struct shwfs_handle shwfs_handle;              /* opaque */
+
+typedef struct {
+  int32_t n_pupil;          /* N  : phase frames are N x N, row-major, x (columns) fastest             */
+  int32_t n_sub_side;       /* S  : S x S lenslet grid, S * n_pix == N                                 */
+  int32_t n_pix;            /* n  : phase pixels per subaperture side                                  */
+  float   pixel_size_m;     /* dx : metres per pupil pixel (> 0; only used by shwfs_pixel_scale)       */
+  const float   *amplitude; /* HOST [N*N] pupil amplitude mask (any finite values, normally 0..1)      */
+  float   min_illum;        /* subaperture valid if mean(amplitude over its patch) >= min_illum        */
+  const int32_t *valid_yx;  /* optional HOST [n_valid*2] explicit (sy,sx) list; overrides the rule     */
+  int32_t n_valid;          /* length of valid_yx (ignored when valid_yx is NULL)                      */
+  float   threshold_frac;   /* tau in [0,1): fraction of the per-spot peak; 0 = plain CoG              */
+  int32_t threshold_mode;   /* 0 = subtract-and-clip (default), 1 = hard mask                          */
+  float   phase_to_rad;     /* c_phi: multiplies the input to give radians at lambda (1 if already)    */
+} shwfs_geometry;
+
+/* Build one WFS.  lambda_m > 0; pad = P (power of two, n <= P <= 64); bin = b (b | P, (P/2) % b == 0).
+ * elong_kernels: HOST [nsub*P*P] fp32 spatial kernels at unbinned resolution, centre at (P/2,P/2),
+ * index order of the valid list, used as given (no renormalisation) -- or NULL for no elongation (H5
+ * skipped).  The valid list is row-major over (sy,sx) (sy outer).  On success *out receives the handle.
+ * Errors: EINVAL (null g/out/amplitude, N != S*n, bad P/b/lambda/dx/tau/mode, valid_yx entry out of range
+ * or n_valid <= 0, no valid subaperture), EUNSUPPORTED (n > 32 or P/b > 32), ENOMEM, ECUDA.             */
+int shwfs_create(const shwfs_geometry *g, float lambda_m, int32_t pad, int32_t bin,
+                 const float *elong_kernels, shwfs_handle **out);
+
+/* phase_dev: DEVICE [T*N*N] fp32 (16-byte aligned); slopes_dev: DEVICE [T*nsub*2] fp32,
+ * slopes[t][i][0] = x-slope, [1] = y-slope, in binned detector pixels about the detector centre;
+ * i indexes the valid list.  Positive x-slope <=> phase increasing with x (the column index).
+ * T == 0 is a successful no-op.  Non-finite phase values are not checked: they reach only that spot's
+ * slopes.  Errors: EINVAL (null h, null pointers with T > 0, T < 0), ECUDA (launch failure).           */
+int shwfs_measure(shwfs_handle *h, const float *phase_dev, int32_t T, float *slopes_dev,
+                  void *cuda_stream);
+
+/* Same measurement from HOST buffers: phase_host [T*N*N] -> slopes_host [T*nsub*2].  The library copies
+ * in frame chunks through its own pinned staging buffers and device scratch (allocated on first use,
+ * owned by the handle), overlaps copies with compute on two internal streams, and returns after the
+ * slopes have landed in slopes_host.  This is the end-to-end entry point timed as "e2e" by bench.py.   */
+int shwfs_measure_host(shwfs_handle *h, const float *phase_host, int32_t T, float *slopes_host);
+
+/* Frees everything the handle owns.  shwfs_destroy(NULL) returns 0. */
+int shwfs_destroy(shwfs_handle *h);
+
+/* ---- queries ---------------------------------------------------------------------------------- */
+int shwfs_num_subaps(const shwfs_handle *h, int32_t *nsub);
+int shwfs_valid_list(const shwfs_handle *h, int32_t *yx_host /* HOST [nsub*2] */);
+/* radians of wavefront tilt angle per binned detector pixel: b * lambda / (P * dx) */
+int shwfs_pixel_scale(const shwfs_handle *h, double *rad_per_detector_px);
+
+/* Select the algorithm used by shwfs_measure (SHWFS_ALGO_*).  EUNSUPPORTED if that algorithm has no
+ * instance for the handle's sizes.  shwfs_get_algorithm reports the resolved (never AUTO) choice.    */
+int shwfs_set_algorithm(shwfs_handle *h, int32_t algo);
+int shwfs_get_algorithm(const shwfs_handle *h, int32_t *algo);
+
+/* Number of kernels this handle has launched since shwfs_create (bench.py's gpu_launches). */
+int shwfs_launch_count(const shwfs_handle *h, int64_t *count);
+
+/* ---- debug (parity on images; not on the timed path) ------------------------------------------- */
+/* stage 0: centred intensity  roll(I)  DEVICE out [T*nsub*P*P]
+ * stage 1: centred image after elongation  Sh  [T*nsub*P*P]  (== stage 0 without kernels)
+ * stage 2: binned image B  [T*nsub*D*D], D = P/b -- produced by the handle's CURRENT algorithm, so it
+ *          is the image the timed path thresholds; stages 0 and 1 exist only in the literal chain.   */
+int shwfs_debug_spots(shwfs_handle *h, const float *phase_dev, int32_t T, int32_t stage,
+                      float *out_dev, void *cuda_stream);
+
+const char *shwfs_strerror(int code);
+/* Text of the last CUDA error seen by this process's calls into the library ("" if none). */
+const char *shwfs_last_cuda_error(void);
+int shwfs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SHWFS_H_ */

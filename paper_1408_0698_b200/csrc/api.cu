@@ -1,0 +1,384 @@
+/*
+ * api.cu -- the C ABI of include/shwfs.h: handle life cycle, argument checking, algorithm choice and
+ * the host-buffer pipeline.  No arithmetic of the method lives here; see wk.cu and literal.cu.
+ */
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "internal.h"
+
+namespace {
+
+thread_local char g_cuda_err[256] = "";
+
+#define CU_TRY(call, where)                                \
+    do {                                                   \
+        cudaError_t e_ = (call);                           \
+        if (e_ != cudaSuccess) {                           \
+            shwfs_note_cuda_error(e_, where);              \
+            rc = (e_ == cudaErrorMemoryAllocation) ? SHWFS_ENOMEM : SHWFS_ECUDA; \
+            goto fail;                                     \
+        }                                                  \
+    } while (0)
+
+bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+
+void free_handle(shwfs_handle *h)
+{
+    if (!h) return;
+    int prev = -1;
+    cudaGetDevice(&prev);
+    if (prev != h->device) cudaSetDevice(h->device);
+    cudaFree(h->d_amp);
+    cudaFree(h->d_valid);
+    cudaFree(h->d_kernels);
+    cudaFree(h->d_wk_table);
+    cudaFree(h->d_khat);
+    for (int k = 0; k < 2; ++k) {
+        if (h->h_pin[k]) cudaFreeHost(h->h_pin[k]);
+        cudaFree(h->d_phase[k]);
+        if (h->ev_h2d[k]) cudaEventDestroy(h->ev_h2d[k]);
+        if (h->ev_done[k]) cudaEventDestroy(h->ev_done[k]);
+    }
+    cudaFree(h->d_slopes);
+    if (h->h_slopes_pin) cudaFreeHost(h->h_slopes_pin);
+    if (h->st_copy) cudaStreamDestroy(h->st_copy);
+    if (h->st_comp) cudaStreamDestroy(h->st_comp);
+    free(h->h_valid);
+    if (prev >= 0 && prev != h->device) cudaSetDevice(prev);
+    delete h;
+    cudaGetLastError();
+}
+
+int pick_auto(const shwfs_handle *h)
+{
+    /* without kernels one P x P FFT is cheaper than the autocorrelation once
+     * n >= 16; with kernels the lag-domain form always wins.  Fall back along the chain. */
+    const bool wk = shwfs_wk_supported(h, 0), lit = shwfs_literal_supported(h);
+    if (!h->has_kernels && lit && (h->n >= 16 || !wk)) return SHWFS_ALGO_LITERAL;
+    if (wk) return SHWFS_ALGO_WK;
+    if (shwfs_wk_supported(h, 1)) return SHWFS_ALGO_WK_GENERIC;
+    if (lit) return SHWFS_ALGO_LITERAL;
+    return -1;
+}
+
+int ensure_khat(shwfs_handle *h)
+{
+    if (!h->has_kernels || h->d_khat) return SHWFS_OK;
+    cudaError_t e = cudaMalloc(&h->d_khat, sizeof(float2) * (size_t)h->nsub * h->P * h->P);
+    if (e != cudaSuccess) { h->d_khat = nullptr; shwfs_note_cuda_error(e, "cudaMalloc(khat)"); return SHWFS_ENOMEM; }
+    e = shwfs_literal_build_khat(h, 0);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(0);
+    if (e != cudaSuccess) {
+        shwfs_note_cuda_error(e, "literal_build_khat");
+        cudaFree(h->d_khat); h->d_khat = nullptr;
+        return SHWFS_ECUDA;
+    }
+    return SHWFS_OK;
+}
+
+}  // namespace
+
+void shwfs_note_cuda_error(cudaError_t e, const char *where)
+{
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    cudaGetLastError();   /* clear the sticky-free error state */
+}
+
+extern "C" {
+
+int shwfs_version(void) { return 100; }
+
+const char *shwfs_strerror(int code)
+{
+    switch (code) {
+    case SHWFS_OK: return "ok";
+    case SHWFS_EINVAL: return "invalid argument";
+    case SHWFS_EUNSUPPORTED: return "sizes not supported by any kernel instance";
+    case SHWFS_ENOMEM: return "out of memory";
+    case SHWFS_ECUDA: return "CUDA error (see shwfs_last_cuda_error)";
+    default: return "unknown error code";
+    }
+}
+
+const char *shwfs_last_cuda_error(void) { return g_cuda_err; }
+
+int shwfs_create(const shwfs_geometry *g, float lambda_m, int32_t pad, int32_t bin,
+                 const float *elong_kernels, shwfs_handle **out)
+{
+    if (!g || !out || !g->amplitude) return SHWFS_EINVAL;
+    const int N = g->n_pupil, S = g->n_sub_side, n = g->n_pix, P = pad, b = bin;
+    if (N <= 0 || S <= 0 || n <= 0 || (long long)S * n != N) return SHWFS_EINVAL;
+    if (!is_pow2(P) || P < n || P > 64 || b <= 0 || P % b || (P / 2) % b) return SHWFS_EINVAL;
+    if (!(lambda_m > 0.f) || !(g->pixel_size_m > 0.f)) return SHWFS_EINVAL;
+    if (!(g->threshold_frac >= 0.f && g->threshold_frac < 1.f)) return SHWFS_EINVAL;
+    if (g->threshold_mode != 0 && g->threshold_mode != 1) return SHWFS_EINVAL;
+    if (!isfinite(g->phase_to_rad) || !isfinite(g->min_illum)) return SHWFS_EINVAL;
+    if (g->valid_yx && g->n_valid <= 0) return SHWFS_EINVAL;
+
+    /* H0: valid-subaperture list (reading A2), row-major over (sy,sx) */
+    int32_t *valid = (int32_t *)malloc(sizeof(int32_t) * 2 * (size_t)S * S);
+    if (!valid) return SHWFS_ENOMEM;
+    int nsub = 0;
+    if (g->valid_yx) {
+        if (g->n_valid > S * S) { free(valid); return SHWFS_EINVAL; }
+        for (int i = 0; i < g->n_valid; ++i) {
+            const int sy = g->valid_yx[2 * i], sx = g->valid_yx[2 * i + 1];
+            if (sy < 0 || sy >= S || sx < 0 || sx >= S) { free(valid); return SHWFS_EINVAL; }
+            valid[2 * i] = sy; valid[2 * i + 1] = sx;
+        }
+        nsub = g->n_valid;
+    } else {
+        for (int sy = 0; sy < S; ++sy)
+            for (int sx = 0; sx < S; ++sx) {
+                double s = 0.0;
+                for (int j = 0; j < n; ++j)
+                    for (int k = 0; k < n; ++k) s += (double)g->amplitude[(size_t)(sy * n + j) * N + sx * n + k];
+                if (s / ((double)n * n) >= (double)g->min_illum) { valid[2 * nsub] = sy; valid[2 * nsub + 1] = sx; ++nsub; }
+            }
+    }
+    if (nsub == 0) { free(valid); return SHWFS_EINVAL; }
+
+    shwfs_handle *h = new (std::nothrow) shwfs_handle();
+    if (!h) { free(valid); return SHWFS_ENOMEM; }
+    memset(h, 0, sizeof(*h));
+    h->N = N; h->S = S; h->n = n; h->P = P; h->b = b; h->D = P / b; h->nsub = nsub;
+    h->dx = g->pixel_size_m; h->lambda_m = lambda_m; h->tau = g->threshold_frac; h->c_phi = g->phase_to_rad;
+    h->mode = g->threshold_mode; h->has_kernels = elong_kernels != nullptr;
+    h->h_valid = valid;
+    h->chunk_frames = 0;
+
+    int rc = SHWFS_OK;
+    CU_TRY(cudaGetDevice(&h->device), "cudaGetDevice");
+    if (!shwfs_wk_supported(h, 0) && !shwfs_wk_supported(h, 1) && !shwfs_literal_supported(h)) { rc = SHWFS_EUNSUPPORTED; goto fail; }
+    h->algo = pick_auto(h);
+    if (h->algo < 0) { rc = SHWFS_EUNSUPPORTED; goto fail; }
+
+    CU_TRY(cudaMalloc(&h->d_amp, sizeof(float) * (size_t)N * N), "cudaMalloc(amplitude)");
+    CU_TRY(cudaMemcpy(h->d_amp, g->amplitude, sizeof(float) * (size_t)N * N, cudaMemcpyHostToDevice), "cudaMemcpy(amplitude)");
+    CU_TRY(cudaMalloc(&h->d_valid, sizeof(int2) * (size_t)nsub), "cudaMalloc(valid)");
+    CU_TRY(cudaMemcpy(h->d_valid, valid, sizeof(int2) * (size_t)nsub, cudaMemcpyHostToDevice), "cudaMemcpy(valid)");
+    if (h->has_kernels) {
+        const size_t kb = sizeof(float) * (size_t)nsub * P * P;
+        CU_TRY(cudaMalloc(&h->d_kernels, kb), "cudaMalloc(kernels)");
+        CU_TRY(cudaMemcpy(h->d_kernels, elong_kernels, kb, cudaMemcpyHostToDevice), "cudaMemcpy(kernels)");
+    }
+    if (shwfs_wk_supported(h, 1) || shwfs_wk_supported(h, 0)) {
+        const int per = n * (2 * n - 1);
+        h->wk_table_stride = h->has_kernels ? per : 0;
+        CU_TRY(cudaMalloc(&h->d_wk_table, sizeof(float2) * (size_t)per * (h->has_kernels ? nsub : 1)), "cudaMalloc(wk table)");
+        CU_TRY(shwfs_wk_build_table(h, 0), "wk_build_table");
+    }
+    CU_TRY(cudaStreamSynchronize(0), "create sync");
+    if (h->algo == SHWFS_ALGO_LITERAL) { rc = ensure_khat(h); if (rc) goto fail; }
+    *out = h;
+    return SHWFS_OK;
+fail:
+    free_handle(h);
+    return rc;
+}
+
+int shwfs_destroy(shwfs_handle *h)
+{
+    if (!h) return SHWFS_OK;
+    if (h->st_comp) cudaStreamSynchronize(h->st_comp);
+    if (h->st_copy) cudaStreamSynchronize(h->st_copy);
+    free_handle(h);
+    return SHWFS_OK;
+}
+
+int shwfs_num_subaps(const shwfs_handle *h, int32_t *nsub)
+{
+    if (!h || !nsub) return SHWFS_EINVAL;
+    *nsub = h->nsub;
+    return SHWFS_OK;
+}
+
+int shwfs_valid_list(const shwfs_handle *h, int32_t *yx_host)
+{
+    if (!h || !yx_host) return SHWFS_EINVAL;
+    memcpy(yx_host, h->h_valid, sizeof(int32_t) * 2 * (size_t)h->nsub);
+    return SHWFS_OK;
+}
+
+int shwfs_pixel_scale(const shwfs_handle *h, double *rad_per_detector_px)
+{
+    if (!h || !rad_per_detector_px) return SHWFS_EINVAL;
+    *rad_per_detector_px = (double)h->b * (double)h->lambda_m / ((double)h->P * (double)h->dx);
+    return SHWFS_OK;
+}
+
+int shwfs_set_algorithm(shwfs_handle *h, int32_t algo)
+{
+    if (!h) return SHWFS_EINVAL;
+    int a = algo;
+    if (a == SHWFS_ALGO_AUTO) a = pick_auto(h);
+    switch (a) {
+    case SHWFS_ALGO_LITERAL:
+        if (!shwfs_literal_supported(h)) return SHWFS_EUNSUPPORTED;
+        { int rc = ensure_khat(h); if (rc) return rc; }
+        break;
+    case SHWFS_ALGO_WK: if (!shwfs_wk_supported(h, 0)) return SHWFS_EUNSUPPORTED; break;
+    case SHWFS_ALGO_WK_GENERIC: if (!shwfs_wk_supported(h, 1)) return SHWFS_EUNSUPPORTED; break;
+    default: return SHWFS_EINVAL;
+    }
+    h->algo = a;
+    return SHWFS_OK;
+}
+
+int shwfs_get_algorithm(const shwfs_handle *h, int32_t *algo)
+{
+    if (!h || !algo) return SHWFS_EINVAL;
+    *algo = h->algo;
+    return SHWFS_OK;
+}
+
+int shwfs_launch_count(const shwfs_handle *h, int64_t *count)
+{
+    if (!h || !count) return SHWFS_EINVAL;
+    *count = h->launches;
+    return SHWFS_OK;
+}
+
+static int run_path(shwfs_handle *h, const float *phase_dev, int T, float *slopes_dev, int stage, float *img,
+                    cudaStream_t st)
+{
+    if ((long long)T * h->nsub > 0x7fffffffLL / 2) return SHWFS_EINVAL;
+    cudaError_t e;
+    if (stage == 0 || stage == 1) {
+        int rc = ensure_khat(h);
+        if (rc) return rc;
+        if (!shwfs_literal_supported(h)) return SHWFS_EUNSUPPORTED;
+        e = shwfs_literal_launch(h, phase_dev, T, slopes_dev, stage, img, st);
+    } else if (h->algo == SHWFS_ALGO_LITERAL) {
+        e = shwfs_literal_launch(h, phase_dev, T, slopes_dev, stage, img, st);
+    } else {
+        e = shwfs_wk_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr,
+                            h->algo == SHWFS_ALGO_WK_GENERIC, st);
+    }
+    if (e != cudaSuccess) { shwfs_note_cuda_error(e, "kernel launch"); return SHWFS_ECUDA; }
+    return SHWFS_OK;
+}
+
+int shwfs_measure(shwfs_handle *h, const float *phase_dev, int32_t T, float *slopes_dev, void *cuda_stream)
+{
+    if (!h || T < 0) return SHWFS_EINVAL;
+    if (T == 0) return SHWFS_OK;
+    if (!phase_dev || !slopes_dev) return SHWFS_EINVAL;
+    return run_path(h, phase_dev, T, slopes_dev, -1, nullptr, (cudaStream_t)cuda_stream);
+}
+
+int shwfs_debug_spots(shwfs_handle *h, const float *phase_dev, int32_t T, int32_t stage, float *out_dev,
+                      void *cuda_stream)
+{
+    if (!h || T < 0 || stage < 0 || stage > 2) return SHWFS_EINVAL;
+    if (T == 0) return SHWFS_OK;
+    if (!phase_dev || !out_dev) return SHWFS_EINVAL;
+    /* the debug path needs somewhere to put the slopes it also computes */
+    const size_t need = 2 * (size_t)T * h->nsub;
+    if (h->d_slopes_cap < need) {
+        cudaStreamSynchronize((cudaStream_t)cuda_stream);
+        cudaFree(h->d_slopes); h->d_slopes = nullptr; h->d_slopes_cap = 0;
+        cudaError_t e = cudaMalloc(&h->d_slopes, sizeof(float) * need);
+        if (e != cudaSuccess) { shwfs_note_cuda_error(e, "cudaMalloc(debug slopes)"); return SHWFS_ENOMEM; }
+        h->d_slopes_cap = need;
+    }
+    return run_path(h, phase_dev, T, h->d_slopes, stage, out_dev, (cudaStream_t)cuda_stream);
+}
+
+}  // extern "C"
+
+/* ------------------------------------------------------------------------------------------------
+ * Host-buffer entry point: frames are cut into chunks of ~64 MiB, copied on st_copy into one of two
+ * device buffers and measured on st_comp, so the H2D copy of chunk c+1 overlaps the kernels of
+ * chunk c.  A pinned (cudaHostAlloc / cudaHostRegister) caller buffer is copied from directly; a
+ * pageable one goes through the handle's own two pinned staging buffers.
+ * ---------------------------------------------------------------------------------------------- */
+namespace {
+
+int host_init(shwfs_handle *h)
+{
+    if (h->host_ready) return SHWFS_OK;
+    int rc = SHWFS_OK;
+    const size_t frame_bytes = sizeof(float) * (size_t)h->N * h->N;
+    size_t chunk = ((size_t)64 << 20) / frame_bytes;
+    if (chunk < 1) chunk = 1;
+    if (chunk > 256) chunk = 256;
+    h->chunk_frames = (int)chunk;
+    CU_TRY(cudaStreamCreateWithFlags(&h->st_copy, cudaStreamNonBlocking), "cudaStreamCreate");
+    CU_TRY(cudaStreamCreateWithFlags(&h->st_comp, cudaStreamNonBlocking), "cudaStreamCreate");
+    for (int k = 0; k < 2; ++k) {
+        CU_TRY(cudaEventCreateWithFlags(&h->ev_h2d[k], cudaEventDisableTiming), "cudaEventCreate");
+        CU_TRY(cudaEventCreateWithFlags(&h->ev_done[k], cudaEventDisableTiming), "cudaEventCreate");
+        CU_TRY(cudaMalloc(&h->d_phase[k], frame_bytes * chunk), "cudaMalloc(frame chunk)");
+    }
+    h->host_ready = 1;
+    return SHWFS_OK;
+fail:
+    return rc;   /* partial allocations are released by shwfs_destroy */
+}
+
+bool is_pinned(const void *p)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeHost;
+}
+
+}  // namespace
+
+extern "C" int shwfs_measure_host(shwfs_handle *h, const float *phase_host, int32_t T, float *slopes_host)
+{
+    if (!h || T < 0) return SHWFS_EINVAL;
+    if (T == 0) return SHWFS_OK;
+    if (!phase_host || !slopes_host) return SHWFS_EINVAL;
+    if ((long long)T * h->nsub > 0x7fffffffLL / 2) return SHWFS_EINVAL;
+    int rc = SHWFS_OK;
+    int prev = -1;
+    cudaGetDevice(&prev);
+    if (prev != h->device) cudaSetDevice(h->device);
+    {
+        rc = host_init(h);
+        if (rc) goto fail;
+        const size_t frame_elems = (size_t)h->N * h->N, frame_bytes = sizeof(float) * frame_elems;
+        const size_t n_slopes = 2 * (size_t)T * h->nsub;
+        if (h->d_slopes_cap < n_slopes) {
+            cudaStreamSynchronize(h->st_comp);
+            cudaFree(h->d_slopes); h->d_slopes = nullptr; h->d_slopes_cap = 0;
+            CU_TRY(cudaMalloc(&h->d_slopes, sizeof(float) * n_slopes), "cudaMalloc(slopes)");
+            h->d_slopes_cap = n_slopes;
+        }
+        const bool pinned_in = is_pinned(phase_host);
+        if (!pinned_in)
+            for (int k = 0; k < 2; ++k)
+                if (!h->h_pin[k]) CU_TRY(cudaHostAlloc(&h->h_pin[k], frame_bytes * h->chunk_frames, cudaHostAllocDefault), "cudaHostAlloc");
+        int c = 0;
+        for (int t0 = 0; t0 < T; t0 += h->chunk_frames, ++c) {
+            const int k = c & 1;
+            const int tc = (T - t0 < h->chunk_frames) ? T - t0 : h->chunk_frames;
+            const float *src = phase_host + (size_t)t0 * frame_elems;
+            if (!pinned_in) {
+                CU_TRY(cudaEventSynchronize(h->ev_h2d[k]), "cudaEventSynchronize");   /* staging buffer free again */
+                memcpy(h->h_pin[k], src, frame_bytes * tc);
+                src = h->h_pin[k];
+            }
+            CU_TRY(cudaStreamWaitEvent(h->st_copy, h->ev_done[k], 0), "cudaStreamWaitEvent");
+            CU_TRY(cudaMemcpyAsync(h->d_phase[k], src, frame_bytes * tc, cudaMemcpyHostToDevice, h->st_copy), "cudaMemcpyAsync(H2D)");
+            CU_TRY(cudaEventRecord(h->ev_h2d[k], h->st_copy), "cudaEventRecord");
+            CU_TRY(cudaStreamWaitEvent(h->st_comp, h->ev_h2d[k], 0), "cudaStreamWaitEvent");
+            rc = run_path(h, h->d_phase[k], tc, h->d_slopes + 2 * (size_t)t0 * h->nsub, -1, nullptr, h->st_comp);
+            if (rc) goto fail;
+            CU_TRY(cudaEventRecord(h->ev_done[k], h->st_comp), "cudaEventRecord");
+        }
+        CU_TRY(cudaMemcpyAsync(slopes_host, h->d_slopes, sizeof(float) * n_slopes, cudaMemcpyDeviceToHost, h->st_comp), "cudaMemcpyAsync(D2H)");
+        CU_TRY(cudaStreamSynchronize(h->st_comp), "cudaStreamSynchronize");
+    }
+fail:
+    if (rc && h->st_comp) { cudaStreamSynchronize(h->st_comp); cudaStreamSynchronize(h->st_copy); }
+    if (prev >= 0 && prev != h->device) cudaSetDevice(prev);
+    return rc;
+}

@@ -1,0 +1,69 @@
+/*
+ * internal.h -- private declarations shared by the translation units of libshwfs.so.
+ * Not part of the ABI (include/shwfs.h is) and never included by anything under oracle/.
+ *
+ * Notation follows SURVEY.md section 8 / DESIGN.md: N pupil side, S subapertures per side, n phase
+ * pixels per subaperture side, P padded FFT side, b binning, D = P/b detector side, nsub valid
+ * subapertures, T frames.
+ */
+#ifndef SHWFS_INTERNAL_H_
+#define SHWFS_INTERNAL_H_
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/shwfs.h"
+
+struct shwfs_handle {
+    /* geometry */
+    int N, S, n, P, b, D, nsub;
+    float dx, lambda_m, tau, c_phi;
+    int mode;              /* threshold mode */
+    int device;
+    int has_kernels;
+    int algo;              /* resolved SHWFS_ALGO_* used by shwfs_measure */
+    int64_t launches;
+
+    /* device tables (owned) */
+    float  *d_amp;         /* [N*N] amplitude mask                                             */
+    int2   *d_valid;       /* [nsub] (x = sy, y = sx)                                          */
+    float  *d_kernels;     /* [nsub*P*P] spatial elongation kernels (kept for lazy tables)     */
+    float2 *d_wk_table;    /* lag-domain table M: [nsub][n][2n-1] (or [1][n][2n-1] w/o kernels) */
+    int     wk_table_stride; /* elements between subapertures: n*(2n-1), or 0 when shared      */
+    float2 *d_khat;        /* literal chain: DFT of the re-centred kernel, [nsub][P][P]; lazy  */
+
+    /* host copies for queries */
+    int32_t *h_valid;      /* [nsub*2] (sy,sx) */
+
+    /* shwfs_measure_host staging (lazy) */
+    float *h_pin[2];       /* pinned staging for pageable callers */
+    float *d_phase[2];     /* device frame chunks */
+    float *d_slopes;       /* device slopes for the whole call, grown on demand */
+    float *h_slopes_pin;   /* pinned landing buffer for slopes of a pageable caller */
+    size_t d_slopes_cap;   /* floats */
+    int    chunk_frames;
+    cudaStream_t st_copy, st_comp;
+    cudaEvent_t ev_h2d[2], ev_done[2];
+    int host_ready;
+};
+
+/* ---- launchers: each enqueues on `st` and returns the CUDA status of the launch ---------------- */
+
+/* Lag-domain table M, built once at create in float64 on the device. */
+cudaError_t shwfs_wk_build_table(shwfs_handle *h, cudaStream_t st);
+
+/* Wiener-Khinchin path: slopes (and optionally the binned image B, [T*nsub*D*D]) */
+cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *slopes,
+                            float *binned_or_null, int generic, cudaStream_t st);
+int shwfs_wk_supported(const shwfs_handle *h, int generic);
+
+/* Literal chain: P x P FFT(s) in shared memory/registers.  stage < 0: slopes only.
+ * stage 0/1/2 also writes that image to `img`.                                              */
+cudaError_t shwfs_literal_launch(shwfs_handle *h, const float *phase, int T, float *slopes,
+                                 int stage, float *img, cudaStream_t st);
+cudaError_t shwfs_literal_build_khat(shwfs_handle *h, cudaStream_t st);
+int shwfs_literal_supported(const shwfs_handle *h);
+
+void shwfs_note_cuda_error(cudaError_t e, const char *where);
+
+#endif /* SHWFS_INTERNAL_H_ */

@@ -1,0 +1,494 @@
+/*
+ * wk.cu -- Wiener-Khinchin (lag-domain) form of the Shack-Hartmann hot path, sm_100a.
+ *
+ * What it computes is H1..H8 of include/shwfs.h ("The WF is split into sub-apertures and
+ * the spot computed by FFT for each sensor sub-aperture ... a convolution for a gaussian ... the
+ * centroid computed on the final image to retrieve the slopes").  How: the binned, centred, convolved
+ * image B is linear in the intensity I = |DFT(e)|^2 / P^2, and the DFT of I is the (aperiodic)
+ * autocorrelation of the n x n field e (invariant I13 of SURVEY.md 8(c)).  Writing w = exp(2*pi*i/P),
+ * w_D = exp(2*pi*i/D), D = P/b:
+ *
+ *     G[ly,lx]  = sum_{j,k} e[j,k] * conj(e[j+ly, k+lx])              |ly|,|lx| < n          (H3+H4)
+ *     B[R,C]    = sum_{ly,lx} G[ly,lx] * M_i[ly,lx] * w_D^(R*ly + C*lx)                      (H5+H6)
+ *     M_i[l]    = Z_i[l] * beta(ly) * beta(lx) / P^2,   beta(l) = sum_{alpha<b} w^(alpha*l),
+ *     Z_i[l]    = sum_q K_i[q] w^(-q.l)  with kernels,  (-1)^(ly+lx) without
+ *
+ * G[-l] = conj(G[l]) and M[-l] = conj(M[l]) (K real), so only ly >= 0 is computed and the factor 2
+ * for ly >= 1 is folded into M.  The result equals the literal P x P FFT chain up to fp32 rounding
+ * for ANY P >= n (the identity is one of trigonometric polynomials), costs n^2(n+1)/2 * n complex
+ * MACs instead of three P x P transforms, and needs a D x D rather than P x P final transform.
+ * DESIGN.md section 6 has the derivation, the thread mapping and the flop counts.
+ */
+#include "internal.h"
+#include "fft_regs.cuh"
+
+namespace {
+
+using namespace shwfs;
+
+/* ------------------------------------------------------------------------------------------------
+ * Table M (float64 on the device, stored as float2).  One CTA per subaperture (or one CTA in all
+ * when there are no kernels).  Layout M[i][ly][a], a = lx + n - 1.
+ * ---------------------------------------------------------------------------------------------- */
+__global__ void wk_table_kernel(const float *__restrict__ K, int has_k, int n, int P, int b,
+                                float2 *__restrict__ M)
+{
+    extern __shared__ double2 tmp[];           /* [P][2n-1]: row-wise partial transform of K */
+    const int LX = 2 * n - 1;
+    const int i = blockIdx.x;
+    if (has_k) {
+        const float *Ki = K + (size_t)i * P * P;
+        for (int idx = threadIdx.x; idx < P * LX; idx += blockDim.x) {
+            const int qy = idx / LX, lx = idx % LX - (n - 1);
+            double sr = 0.0, si = 0.0;
+            for (int qx = 0; qx < P; ++qx) {
+                const int m = ((qx * lx) % P + P) % P;        /* w^(-qx*lx) */
+                double s, c;
+                sincospi(-2.0 * (double)m / (double)P, &s, &c);
+                const double kv = (double)Ki[qy * P + qx];
+                sr += kv * c;
+                si += kv * s;
+            }
+            tmp[idx] = make_double2(sr, si);
+        }
+        __syncthreads();
+    }
+    const double inv_pp = 1.0 / ((double)P * (double)P);
+    for (int idx = threadIdx.x; idx < n * LX; idx += blockDim.x) {
+        const int ly = idx / LX, a = idx % LX, lx = a - (n - 1);
+        double zr, zi;
+        if (has_k) {
+            zr = 0.0; zi = 0.0;
+            for (int qy = 0; qy < P; ++qy) {
+                const int m = (qy * ly) % P;                   /* w^(-qy*ly) */
+                double s, c;
+                sincospi(-2.0 * (double)m / (double)P, &s, &c);
+                const double2 t = tmp[qy * LX + a];
+                zr += t.x * c - t.y * s;
+                zi += t.x * s + t.y * c;
+            }
+        } else {
+            zr = ((ly + lx) & 1) ? -1.0 : 1.0;
+            zi = 0.0;
+        }
+        double byr = 0.0, byi = 0.0, bxr = 0.0, bxi = 0.0;     /* beta(ly), beta(lx) */
+        for (int al = 0; al < b; ++al) {
+            double s, c;
+            sincospi(2.0 * (double)((al * ly) % P) / (double)P, &s, &c);
+            byr += c; byi += s;
+            sincospi(2.0 * (double)(((al * lx) % P + P) % P) / (double)P, &s, &c);
+            bxr += c; bxi += s;
+        }
+        const double br = byr * bxr - byi * bxi, bi = byr * bxi + byi * bxr;
+        const double scale = inv_pp * (ly >= 1 ? 2.0 : 1.0);
+        M[(size_t)i * n * LX + idx] = make_float2((float)((zr * br - zi * bi) * scale),
+                                                  (float)((zr * bi + zi * br) * scale));
+    }
+}
+
+/* H2: field value of one pupil pixel.  turns = phase_to_rad / (2*pi); ramp = (j+k) / (2P) in turns
+ * (reading A5).  The argument is reduced to [-1/2, 1/2] turns before the fast sincos so that the
+ * +-60 rad open-loop phases of the MAORY pupil keep ~1e-6 absolute accuracy.                    */
+__device__ __forceinline__ float2 field_value(float ph, float amp, float turns, float ramp)
+{
+    float u = fmaf(ph, turns, -ramp);
+    u -= rintf(u);
+    float s, c;
+    __sincosf(u * 6.283185307179586f, &s, &c);
+    return make_float2(amp * c, amp * s);
+}
+
+/* H7 + H8 on a half-warp: lane C (0..15) holds column C of B as bcol[R].  Returns slopes in lane 0
+ * of the half-warp.  Shuffles use xor offsets < 16, so the two halves of a warp stay separate.    */
+__device__ __forceinline__ float2 cog16(const float (&bcol)[16], int C, float tau, int mode)
+{
+    float mx = bcol[0];
+#pragma unroll
+    for (int R = 1; R < 16; ++R) mx = fmaxf(mx, bcol[R]);
+#pragma unroll
+    for (int o = 8; o >= 1; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    const float thr = tau * mx;
+    float sw = 0.f, sy = 0.f;
+#pragma unroll
+    for (int R = 0; R < 16; ++R) {
+        const float v = bcol[R];
+        const float w = mode == 0 ? fmaxf(v - thr, 0.f) : (v >= thr ? v : 0.f);
+        sw += w;
+        sy = fmaf(w, (float)R - 7.5f, sy);
+    }
+    float sx = sw * ((float)C - 7.5f);
+#pragma unroll
+    for (int o = 8; o >= 1; o >>= 1) {
+        sw += __shfl_xor_sync(0xffffffffu, sw, o);
+        sx += __shfl_xor_sync(0xffffffffu, sx, o);
+        sy += __shfl_xor_sync(0xffffffffu, sy, o);
+    }
+    if (sw == 0.f) return make_float2(0.f, 0.f);
+    return make_float2(sx / sw, sy / sw);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * Specialised kernel: n in {8,10,16}, D = 16.  One CTA = 32 consecutive spots g = i*T + t (frame
+ * fastest, so the 32 lanes of a warp mostly share one subaperture's table M_i), n/2 warps.
+ *
+ *   phase 0  all threads: gather the 32 patches, H2 sincos, field e -> shared memory.
+ *   phase 1  lane = spot, warp c = lag-row class {c, n-c} (class 0 = {0, n/2}): the thread
+ *            accumulates G[ly, -(n-1)..n-1] for its lag rows in registers, one row pair (j, j+ly)
+ *            at a time (2n-1 independent complex accumulators, 4 n^2 FFMA per 2*2n/4 LDS.128), then
+ *            multiplies by M_i[ly,:], aliases lx mod 16 and does the 16-point x-transform in
+ *            registers: H[ly][C] -> shared memory.
+ *   phase 2  half-warp = spot, lane = detector column C: 16-point y-transform (real part) of
+ *            H[0..n-1][C], then H7/H8 with half-warp shuffles; lane 0 writes the two slopes.
+ * ---------------------------------------------------------------------------------------------- */
+template <int n>
+struct WkCfg {
+    static constexpr int LX = 2 * n - 1;
+    static constexpr int NW = n / 2;
+    static constexpr int THREADS = 32 * NW;
+    static constexpr int SPOTS = 32;
+    static constexpr int ES = (((2 * n * n) / 4) | 1) * 4;  /* floats per spot; /4 odd => LDS.128 conflict-free */
+    static constexpr int HS = (((n * 32) / 4) | 1) * 4;
+    static constexpr size_t SMEM = sizeof(float) * (size_t)(SPOTS * ES + SPOTS * HS) + sizeof(int) * 3 * SPOTS;
+    static_assert(n % 2 == 0 && n <= 16, "n must be even and <= 16");
+};
+
+struct WkArgs {
+    const float *phase;
+    const float *amp;
+    const int2 *valid;
+    const float2 *M;
+    float *slopes;
+    float *binned;
+    long long frame_stride;
+    int T, N, nsub, mstride, total, mode;
+    float tau, turns, ramp_unit;
+};
+
+template <int n>
+__device__ __forceinline__ void rowpair_acc(const float *__restrict__ p1, const float *__restrict__ p2,
+                                            float (&acc)[2 * (2 * n - 1)])
+{
+    float r1[2 * n], r2[2 * n];
+#pragma unroll
+    for (int q = 0; q < (2 * n) / 4; ++q) {
+        const float4 v = reinterpret_cast<const float4 *>(p1)[q];
+        r1[4 * q] = v.x; r1[4 * q + 1] = v.y; r1[4 * q + 2] = v.z; r1[4 * q + 3] = v.w;
+        const float4 u = reinterpret_cast<const float4 *>(p2)[q];
+        r2[4 * q] = u.x; r2[4 * q + 1] = u.y; r2[4 * q + 2] = u.z; r2[4 * q + 3] = u.w;
+    }
+    /* G[lx] += e[j,k] * conj(e[j+ly,k2]),  lx = k2 - k */
+#pragma unroll
+    for (int k = 0; k < n; ++k) {
+#pragma unroll
+        for (int k2 = 0; k2 < n; ++k2) {
+            const int a = k2 - k + n - 1;
+            acc[2 * a] = fmaf(r1[2 * k], r2[2 * k2], acc[2 * a]);
+            acc[2 * a] = fmaf(r1[2 * k + 1], r2[2 * k2 + 1], acc[2 * a]);
+            acc[2 * a + 1] = fmaf(r1[2 * k + 1], r2[2 * k2], acc[2 * a + 1]);
+            acc[2 * a + 1] = fmaf(-r1[2 * k], r2[2 * k2 + 1], acc[2 * a + 1]);
+        }
+    }
+}
+
+template <int n>
+__device__ __forceinline__ void lag_row(const float *__restrict__ eb, int ly, int rows,
+                                        const float2 *__restrict__ Mrow, float *__restrict__ hrow)
+{
+    constexpr int LX = 2 * n - 1;
+    float acc[2 * LX];
+#pragma unroll
+    for (int a = 0; a < 2 * LX; ++a) acc[a] = 0.f;
+#pragma unroll 1
+    for (int j = 0; j < rows; ++j)
+        rowpair_acc<n>(eb + j * 2 * n, eb + (j + ly) * 2 * n, acc);
+
+    /* S = G * M, aliased onto lx mod 16 */
+    float sr[16], si[16];
+#pragma unroll
+    for (int m = 0; m < 16; ++m) {
+        bool first = true;
+        sr[m] = 0.f; si[m] = 0.f;
+#pragma unroll
+        for (int pass = 0; pass < 2; ++pass) {
+            const int lx = pass == 0 ? m : m - 16;
+            if (lx > n - 1 || lx < -(n - 1)) continue;
+            const int a = lx + n - 1;
+            const float2 mv = __ldg(Mrow + a);
+            const float gr = acc[2 * a], gi = acc[2 * a + 1];
+            if (first) {
+                sr[m] = fmaf(gr, mv.x, -gi * mv.y);
+                si[m] = fmaf(gr, mv.y, gi * mv.x);
+                first = false;
+            } else {
+                sr[m] = fmaf(gr, mv.x, fmaf(-gi, mv.y, sr[m]));
+                si[m] = fmaf(gr, mv.y, fmaf(gi, mv.x, si[m]));
+            }
+        }
+    }
+    fft_dif<16, +1>(sr, si);                     /* H[C] = sum_m s'[m] w_16^(C m) */
+#pragma unroll
+    for (int C = 0; C < 16; C += 2) {
+        constexpr int dummy = 0; (void)dummy;
+        const int p0 = fft_out_index<16>(C), p1 = fft_out_index<16>(C + 1);
+        reinterpret_cast<float4 *>(hrow)[C / 2] = make_float4(sr[p0], si[p0], sr[p1], si[p1]);
+    }
+}
+
+template <int n>
+__global__ void __launch_bounds__(WkCfg<n>::THREADS) wk_measure_kernel(const WkArgs A)
+{
+    using Cfg = WkCfg<n>;
+    extern __shared__ __align__(16) float smem[];
+    float *ebuf = smem;
+    float *hbuf = smem + Cfg::SPOTS * Cfg::ES;
+    int *s_off = reinterpret_cast<int *>(hbuf + Cfg::SPOTS * Cfg::HS);
+    int *s_t = s_off + Cfg::SPOTS;
+    int *s_i = s_t + Cfg::SPOTS;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g0 = blockIdx.x * Cfg::SPOTS;
+
+    if (tid < Cfg::SPOTS) {
+        const int g = g0 + tid;
+        int i = -1, t = 0, off = 0;
+        if (g < A.total) {
+            i = g / A.T;
+            t = g - i * A.T;
+            const int2 yx = A.valid[i];
+            off = yx.x * n * A.N + yx.y * n;
+        }
+        s_off[tid] = off; s_t[tid] = t; s_i[tid] = i;
+    }
+    __syncthreads();
+
+    /* ---- phase 0: H1 gather + H2 field ---- */
+    for (int p = tid; p < Cfg::SPOTS * n * n; p += Cfg::THREADS) {
+        const int s = p / (n * n), q = p - s * (n * n), j = q / n, k = q - j * n;
+        float2 e = make_float2(0.f, 0.f);
+        if (s_i[s] >= 0) {
+            const int o = s_off[s] + j * A.N + k;
+            const float ph = __ldg(A.phase + (size_t)s_t[s] * A.frame_stride + o);
+            const float am = __ldg(A.amp + o);
+            e = field_value(ph, am, A.turns, (float)(j + k) * A.ramp_unit);
+        }
+        reinterpret_cast<float2 *>(ebuf + s * Cfg::ES)[q] = e;
+    }
+    __syncthreads();
+
+    /* ---- phase 1: autocorrelation rows, table product, x-transform ---- */
+    {
+        const float *eb = ebuf + lane * Cfg::ES;
+        float *hb = hbuf + lane * Cfg::HS;
+        const int i = max(s_i[lane], 0);
+        const float2 *Mi = A.M + (size_t)i * A.mstride;
+        const int lyA = warp == 0 ? 0 : warp;
+        const int lyB = warp == 0 ? n / 2 : n - warp;
+        lag_row<n>(eb, lyA, n - lyA, Mi + lyA * Cfg::LX, hb + lyA * 32);
+        lag_row<n>(eb, lyB, n - lyB, Mi + lyB * Cfg::LX, hb + lyB * 32);
+    }
+    __syncthreads();
+
+    /* ---- phase 2: y-transform (real part), threshold, centre of gravity ---- */
+    {
+        const int half = lane >> 4, C = lane & 15;
+        for (int s = warp * 2 + half; s < Cfg::SPOTS; s += 2 * Cfg::NW) {
+            const float *hb = hbuf + s * Cfg::HS + 2 * C;
+            float yr[16], yi[16];
+#pragma unroll
+            for (int m = 0; m < 16; ++m) {
+                if (m < n) {
+                    const float2 v = *reinterpret_cast<const float2 *>(hb + m * 32);
+                    yr[m] = v.x; yi[m] = v.y;
+                } else { yr[m] = 0.f; yi[m] = 0.f; }
+            }
+            fft_dif<16, +1, n>(yr, yi);          /* B[R,C] = Re sum_m H[m][C] w_16^(R m) */
+            float bcol[16];
+#pragma unroll
+            for (int R = 0; R < 16; ++R) bcol[R] = yr[fft_out_index<16>(R)];
+            const float2 sl = cog16(bcol, C, A.tau, A.mode);
+            const int i = s_i[s];
+            if (i >= 0) {
+                const size_t o = (size_t)s_t[s] * A.nsub + i;
+                if (C == 0) reinterpret_cast<float2 *>(A.slopes)[o] = sl;
+                if (A.binned) {
+#pragma unroll
+                    for (int R = 0; R < 16; ++R) A.binned[(o * 16 + R) * 16 + C] = bcol[R];
+                }
+            }
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * Size-generic kernel (any even or odd n <= 32, any D <= 32): one CTA of 128 threads per spot, the
+ * same three steps written as plain loops.  Slow; it exists so that every size the ABI accepts has
+ * a kernel, and as an independently written cross-check of the specialised instances.
+ * ---------------------------------------------------------------------------------------------- */
+constexpr int GEN_THREADS = 128;
+
+__global__ void __launch_bounds__(GEN_THREADS) wk_generic_kernel(const WkArgs A, int n, int D)
+{
+    extern __shared__ __align__(16) float smem[];
+    const int LX = 2 * n - 1;
+    float2 *e = reinterpret_cast<float2 *>(smem);           /* [n*n]   */
+    float2 *S = e + n * n;                                  /* [n*LX]  */
+    float2 *tw = S + n * LX;                                /* [D]     */
+    float *B = reinterpret_cast<float *>(tw + D);           /* [D*D]   */
+    float *red = B + D * D;                                 /* [3*GEN_THREADS] */
+
+    const int tid = threadIdx.x;
+    const int g = blockIdx.x;
+    const int i = g / A.T, t = g - i * A.T;
+    const int2 yx = A.valid[i];
+    const int off = yx.x * n * A.N + yx.y * n;
+
+    for (int q = tid; q < n * n; q += GEN_THREADS) {
+        const int j = q / n, k = q - j * n, o = off + j * A.N + k;
+        e[q] = field_value(A.phase[(size_t)t * A.frame_stride + o], A.amp[o], A.turns,
+                           (float)(j + k) * A.ramp_unit);
+    }
+    for (int m = tid; m < D; m += GEN_THREADS) {
+        float s, c;
+        sincospif(2.f * (float)m / (float)D, &s, &c);
+        tw[m] = make_float2(c, s);
+    }
+    __syncthreads();
+
+    const float2 *Mi = A.M + (size_t)i * A.mstride;
+    for (int idx = tid; idx < n * LX; idx += GEN_THREADS) {
+        const int ly = idx / LX, lx = idx - ly * LX - (n - 1);
+        const int k_lo = lx < 0 ? -lx : 0, k_hi = lx < 0 ? n : n - lx;
+        float gr = 0.f, gi = 0.f;
+        for (int j = 0; j + ly < n; ++j)
+            for (int k = k_lo; k < k_hi; ++k) {
+                const float2 u = e[j * n + k], v = e[(j + ly) * n + k + lx];
+                gr = fmaf(u.x, v.x, fmaf(u.y, v.y, gr));     /* u * conj(v) */
+                gi = fmaf(u.y, v.x, fmaf(-u.x, v.y, gi));
+            }
+        const float2 mv = Mi[idx];
+        S[idx] = make_float2(gr * mv.x - gi * mv.y, gr * mv.y + gi * mv.x);
+    }
+    __syncthreads();
+
+    for (int px = tid; px < D * D; px += GEN_THREADS) {
+        const int R = px / D, C = px - R * D;
+        float acc = 0.f;
+        for (int ly = 0; ly < n; ++ly)
+            for (int a = 0; a < LX; ++a) {
+                int m = (R * ly + C * (a - (n - 1))) % D;
+                if (m < 0) m += D;
+                const float2 w = tw[m], s = S[ly * LX + a];
+                acc += s.x * w.x - s.y * w.y;
+            }
+        B[px] = acc;
+    }
+    __syncthreads();
+
+    /* H7: peak */
+    float mx = -INFINITY;
+    for (int px = tid; px < D * D; px += GEN_THREADS) mx = fmaxf(mx, B[px]);
+    red[tid] = mx;
+    __syncthreads();
+    for (int o = GEN_THREADS / 2; o >= 1; o >>= 1) {
+        if (tid < o) red[tid] = fmaxf(red[tid], red[tid + o]);
+        __syncthreads();
+    }
+    const float thr = A.tau * red[0];
+    __syncthreads();
+    /* H8: centre of gravity */
+    const float ref = 0.5f * (float)(D - 1);
+    float sw = 0.f, sx = 0.f, sy = 0.f;
+    for (int px = tid; px < D * D; px += GEN_THREADS) {
+        const int R = px / D, C = px - R * D;
+        const float v = B[px];
+        const float w = A.mode == 0 ? fmaxf(v - thr, 0.f) : (v >= thr ? v : 0.f);
+        sw += w;
+        sx = fmaf(w, (float)C - ref, sx);
+        sy = fmaf(w, (float)R - ref, sy);
+    }
+    red[tid] = sw; red[GEN_THREADS + tid] = sx; red[2 * GEN_THREADS + tid] = sy;
+    __syncthreads();
+    for (int o = GEN_THREADS / 2; o >= 1; o >>= 1) {
+        if (tid < o) {
+            red[tid] += red[tid + o];
+            red[GEN_THREADS + tid] += red[GEN_THREADS + tid + o];
+            red[2 * GEN_THREADS + tid] += red[2 * GEN_THREADS + tid + o];
+        }
+        __syncthreads();
+    }
+    const size_t o = (size_t)t * A.nsub + i;
+    if (tid == 0) {
+        const float w = red[0];
+        A.slopes[2 * o] = w == 0.f ? 0.f : red[GEN_THREADS] / w;
+        A.slopes[2 * o + 1] = w == 0.f ? 0.f : red[2 * GEN_THREADS] / w;
+    }
+    if (A.binned)
+        for (int px = tid; px < D * D; px += GEN_THREADS) A.binned[o * D * D + px] = B[px];
+}
+
+template <int n>
+cudaError_t launch_special(const WkArgs &A, cudaStream_t st)
+{
+    using Cfg = WkCfg<n>;
+    static bool attr_set[64] = {false};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev >= 0 && dev < 64 && !attr_set[dev]) {
+        cudaError_t e = cudaFuncSetAttribute(wk_measure_kernel<n>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)Cfg::SMEM);
+        if (e != cudaSuccess) return e;
+        attr_set[dev] = true;
+    }
+    const int grid = (A.total + Cfg::SPOTS - 1) / Cfg::SPOTS;
+    wk_measure_kernel<n><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(A);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+int shwfs_wk_supported(const shwfs_handle *h, int generic)
+{
+    if (generic) return h->n <= 32 && h->D <= 32;
+    return h->D == 16 && (h->n == 8 || h->n == 10 || h->n == 16);
+}
+
+cudaError_t shwfs_wk_build_table(shwfs_handle *h, cudaStream_t st)
+{
+    const int LX = 2 * h->n - 1;
+    const int blocks = h->has_kernels ? h->nsub : 1;
+    const size_t smem = h->has_kernels ? sizeof(double2) * (size_t)h->P * LX : 0;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(wk_table_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    wk_table_kernel<<<blocks, 128, smem, st>>>(h->d_kernels, h->has_kernels, h->n, h->P, h->b, h->d_wk_table);
+    return cudaGetLastError();
+}
+
+cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *slopes, float *binned,
+                            int generic, cudaStream_t st)
+{
+    WkArgs A;
+    A.phase = phase; A.amp = h->d_amp; A.valid = h->d_valid; A.M = h->d_wk_table;
+    A.slopes = slopes; A.binned = binned;
+    A.frame_stride = (long long)h->N * h->N;
+    A.T = T; A.N = h->N; A.nsub = h->nsub; A.mstride = h->wk_table_stride;
+    A.total = T * h->nsub; A.mode = h->mode;
+    A.tau = h->tau;
+    A.turns = (float)((double)h->c_phi / 6.283185307179586476925286766559);
+    A.ramp_unit = 0.5f / (float)h->P;
+    if (A.total == 0) return cudaSuccess;
+    h->launches += 1;
+    if (!generic) {
+        switch (h->n) {
+        case 8: return launch_special<8>(A, st);
+        case 10: return launch_special<10>(A, st);
+        case 16: return launch_special<16>(A, st);
+        default: return cudaErrorInvalidValue;
+        }
+    }
+    const int n = h->n, D = h->D, LX = 2 * n - 1;
+    const size_t smem = sizeof(float2) * (size_t)(n * n + n * LX + D) + sizeof(float) * (size_t)(D * D + 3 * GEN_THREADS);
+    wk_generic_kernel<<<A.total, GEN_THREADS, smem, st>>>(A, n, D);
+    return cudaGetLastError();
+}
