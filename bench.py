@@ -1,0 +1,300 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Shack-Hartmann WFS hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+
+One "step" = one pass of the whole hot path (H1..H8, include/shwfs.h) over one batch of synthetic
+input of the headline workload, config 4 of BASELINE.json: 6 LGS WFS x 4632 valid subapertures
+(80x80 grid, 10x10 px, pad 32, elongation, 2x2 binning, tau = 0.1) x 100 frames = 2 779 200 spots.
+`value` is subaperture-spots/s with inputs resident in HBM; `e2e` is the same through
+shwfs_measure_host from pinned host buffers (H2D of every frame and D2H of the slopes inside the timed
+region).  Prints ONE JSON line on rank 0.  DESIGN.md section 8 explains every field.
+
+`--impl reference` times the float64 CPU oracle (oracle/, as it stands) on a bounded sample of the
+same workload -- the only other place this file runs anything under oracle/ is the `cpu_baseline` leg.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+import numpy as np
+
+# ---- constants of the roofline ----------------------------------------------
+# algorithmic flops per spot: F_alg (pruned first FFT + frame-paired convolution FFTs)
+# and F_nom (1 or 3 full complex P x P FFTs at 5 L log2 L per length-L line)
+F_ALG = {1: 7680, 2: 38400, 3: 84800, 4: 84800, 5: 399360}
+F_NOM = {1: 10240, 2: 51200, 3: 153600, 4: 153600, 5: 737280}
+# FP32 CUDA-core peak derived from unit counts and clocks (B200_PROFILING.md: 148 SMs, 1965 MHz; 128 FP32
+# lanes per SM, FMA = 2 flop): 148 * 128 * 2 * 1.965e9.  Measured FFMA chain on this pool: 72.4 TFLOP/s
+# (profiles/r01_fp32_peak.md).
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def _dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+class ClockSampler:
+    """Polls SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.01):
+        self.samples, self.reasons, self.period, self._stop = [], set(), period_s, threading.Event()
+        self.max_mhz, self.ok = None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # NVML missing: report that instead of inventing clocks
+            self.err = repr(e)
+        self.th = threading.Thread(target=self._run, daemon=True)
+
+    _NAMES = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+              0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+              0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)) if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons") \
+                    else int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in self._NAMES.items():
+                    if r & bit and name != "gpu_idle":
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def start(self):
+        if self.ok:
+            self.th.start()
+
+    def stop(self):
+        self._stop.set()
+        if self.ok:
+            self.th.join(timeout=2)
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "note": "no NVML samples"}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def workload_name(c):
+    el = f", elongation <= {c.elong_max_arcsec:g} arcsec" if c.elong_max_arcsec > 0 else ""
+    return (f"config{c.cfg} ({c.name}): {c.W} WFS x {c.S}x{c.S} subapertures of {c.n}x{c.n} px on a {c.N}x{c.N} pupil, "
+            f"pad {c.P}, {c.b}x{c.b} binning, tau={c.tau:g}{el}, {c.batch}-frame batches")
+
+
+# ---------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """The oracle as it stands on the host cores, K steps of a bounded sample (rank 0 only)."""
+    rank, _, world = _dist_env()
+    if rank != 0:
+        return
+    from oracle import shwfs_oracle as O
+    from paper_1408_0698_b200 import workloads as W
+    c = W.CONFIGS[args.config]
+    amp = W.pupil_mask(c)
+    yx = O.valid_list(amp, c.n, c.min_illum)
+    K = W.elongation_kernels(c, 0, yx)
+    frames = args.ref_frames
+    ph = W.phase_frames(c, 0, range(frames))
+    cores = O.max_threads()
+    for _ in range(max(args.warmup, 1)):
+        O.measure(ph[:1], amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        O.measure(ph, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K)
+    dt = time.perf_counter() - t0
+    spots = frames * len(yx)
+    v = spots * args.steps / dt
+    sample = f"WFS 0, {frames} frame(s) x {len(yx)} valid subapertures = {spots} spots per step"
+    print(json.dumps({
+        "impl": "reference", "metric": "subaperture_spots_per_s", "value": v, "unit": "spots/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(c), "sample": sample},
+        "cpu_baseline": {"value": v, "unit": "spots/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "spots/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ---------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1408_0698_b200 import binding as B, workloads as W
+    from paper_1408_0698_b200.distributed import job_throughput, max_over_ranks, rank_frames
+
+    rank, local_rank, world = _dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    c = W.CONFIGS[args.config]
+    frames = c.batch
+    # one handle per WFS (elongation kernels differ by launch point, reading A13), synthetic frames in HBM
+    sensors = [B.from_config(c, w) for w in range(c.W)]
+    nsub = sensors[0].nsub
+    my_frames = rank_frames(c.T, frames, rank, world)          # each rank owns its own batch of the stream
+    phase = [W.phase_frames_device(c, w, my_frames, dev) for w in range(c.W)]
+    slopes = [torch.empty((frames, nsub, 2), dtype=torch.float32, device=dev) for _ in range(c.W)]
+    spots_per_step = c.W * frames * nsub
+    in_bytes = sum(p.numel() * 4 for p in phase)
+    out_bytes = sum(s.numel() * 4 for s in slopes)
+    stream = torch.cuda.Stream(dev)
+
+    def step(events=None):
+        for w, s in enumerate(sensors):
+            if events is not None:
+                e0 = torch.cuda.Event(enable_timing=True); e0.record(stream)
+            s.measure(phase[w], out=slopes[w], stream=stream)
+            if events is not None:
+                e1 = torch.cuda.Event(enable_timing=True); e1.record(stream)
+                events.append((e0, e1))
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident throughput
+    with torch.cuda.stream(stream):
+        for _ in range(max(args.warmup, 3)):
+            step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    l0 = sum(s.launch_count for s in sensors)
+    ev = []
+    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    with torch.cuda.stream(stream):
+        t_beg.record(stream)
+        for _ in range(args.steps):
+            step(ev)
+        t_end.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    launches = sum(s.launch_count for s in sensors) - l0
+    ms_total = t_beg.elapsed_time(t_end)
+    kern_ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    ms_total = max_over_ranks(ms_total, dev)
+    value = job_throughput(spots_per_step, args.steps, ms_total, world)
+
+    # ---- end to end from pinned host memory through shwfs_measure_host
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    h_phase = [torch.empty((frames, c.N, c.N), dtype=torch.float32, pin_memory=True) for _ in range(c.W)]
+    for w in range(c.W):
+        h_phase[w].copy_(phase[w])
+    h_slopes = [torch.empty((frames, nsub, 2), dtype=torch.float32, pin_memory=True) for _ in range(c.W)]
+    for w, s in enumerate(sensors):                       # warm-up: allocates the staging buffers
+        s.measure_host(h_phase[w], out=h_slopes[w])
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        for w, s in enumerate(sensors):
+            s.measure_host(h_phase[w], out=h_slopes[w])
+    torch.cuda.synchronize(dev)
+    e2e_s = time.perf_counter() - t0
+    e2e_value = job_throughput(spots_per_step, e2e_steps, 1e3 * max_over_ranks(e2e_s, dev), world)
+    e2e_check = float((h_slopes[0].to(dev) - slopes[0]).abs().max().item())
+
+    if rank == 0:
+        spots_per_launch = frames * nsub
+        ach = F_ALG[c.cfg] * spots_per_launch / (kern_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                    "frac": ach / FP32_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+                    "kernel": f"wk_measure_kernel<{c.n}>" if sensors[0].algorithm == B.ALGO_WK else f"algo{sensors[0].algorithm}",
+                    "kernel_ms": kern_ms, "spots_per_launch": spots_per_launch,
+                    "flops_per_spot": F_ALG[c.cfg], "flops_basis": "F_alg (SURVEY.md 8(d))",
+                    "frac_nominal_fft_flops": F_NOM[c.cfg] * spots_per_launch / (kern_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
+                    "peak_basis": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (measured FFMA chain 72.4)",
+                    "hbm_frac": (in_bytes + out_bytes) / c.W / (kern_ms * 1e-3) / 1e9 / _hbm_peak()}
+        cpu = None if args.no_cpu_baseline else cpu_baseline(c, args, phase)
+        out = {
+            "metric": "subaperture_spots_per_s", "value": value, "unit": "spots/s", "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(c), "spots_per_step_per_gpu": spots_per_step,
+                       "l2": f"inputs larger than L2 ({in_bytes / 1e6:.0f} MB read per step), no flush"},
+            "wfs_frames_per_s": value / nsub, "system_frames_per_s": value / nsub / c.W,
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": "spots/s", "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes,
+                    "steps": e2e_steps, "api": "shwfs_measure_host", "max_abs_diff_vs_device_path": e2e_check},
+            "gpu_launches": int(launches),
+            "roofline": roofline,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(out))
+    for s in sensors:
+        s.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def _hbm_peak():
+    try:
+        return float(json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["hbm_gbs"])
+    except Exception:
+        return 6650.0   # B200_PROFILING.md fallback
+
+
+def cpu_baseline(c, args, phase_dev):
+    """The oracle as it stands on this box's host cores over a bounded sample of the same batch."""
+    from oracle import shwfs_oracle as O
+    from paper_1408_0698_b200 import workloads as W
+    amp = W.pupil_mask(c)
+    yx = O.valid_list(amp, c.n, c.min_illum)
+    K = W.elongation_kernels(c, 0, yx)
+    ph = phase_dev[0][: args.cpu_frames].cpu().numpy()
+    O.measure(ph[:1], amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K)           # page in / build
+    t0 = time.perf_counter()
+    O.measure(ph, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K)
+    dt = time.perf_counter() - t0
+    spots = ph.shape[0] * len(yx)
+    return {"value": spots / dt, "unit": "spots/s", "cores": O.max_threads(), "kind": "oracle",
+            "sample": f"WFS 0, first {ph.shape[0]} frames of the timed batch = {spots} spots, {dt:.1f} s"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--cpu-frames", type=int, default=100)
+    ap.add_argument("--ref-frames", type=int, default=4)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -175,3 +175,25 @@ def elongation_kernels(c: WfsConfig, wfs: int, valid_yx: np.ndarray, subset=None
         else:
             out[i0:i0 + chunk] = g.to(out.dtype)
     return out
+
+
+def phase_frames_device(c: WfsConfig, wfs: int, frames, device, out=None):
+    """Same von Karman recipe as phase_screen, evaluated with torch on `device` (float64 FFT, cast to fp32).
+
+    The noise comes from torch's generator seeded with seed_for(cfg, wfs, frame), so the values differ from
+    the numpy screens while the spectrum, variance and range are the same.  Used for the full-size timing
+    runs only (throughput does not depend on the values); parity inputs come from
+    phase_screen.  Returns a float32 tensor [len(frames), N, N] on `device` (written into `out` if given).
+    """
+    import torch
+    frames = list(frames)
+    filt = torch.as_tensor(_psd_filter(c.screen_M, c.dx), device=device)
+    if out is None:
+        out = torch.empty((len(frames), c.N, c.N), dtype=torch.float32, device=device)
+    gen = torch.Generator(device=device)
+    for q, t in enumerate(frames):
+        gen.manual_seed(seed_for(c.cfg, wfs, int(t)))
+        w = torch.randn((c.screen_M, c.screen_M), dtype=torch.float64, device=device, generator=gen)
+        scr = torch.fft.ifft2(torch.fft.fft2(w) * filt).real * (0.5 / 0.589)
+        out[q] = scr[: c.N, : c.N].to(torch.float32)
+    return out
