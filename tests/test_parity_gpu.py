@@ -1,0 +1,226 @@
+"""GPU <-> oracle parity through the C ABI (run on the B200 box with -m gpu).
+
+Tolerances are BASELINE.json:north_star's: per-subaperture intensities within 1e-4 of the spot peak,
+slopes within 1e-3 detector pixel absolute.  Every input is seeded and synthetic
+(paper_1408_0698_b200.workloads); every expected value comes from oracle/ on the same fp32 arrays.
+"""
+import numpy as np
+import pytest
+
+from paper_1408_0698_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+SLOPE_TOL = 1e-3      # detector px, absolute          (north_star)
+IMAGE_TOL = 1e-4      # fraction of the spot peak      (north_star)
+
+
+def _algos(sensor, B):
+    out = []
+    for a in (B.ALGO_WK, B.ALGO_WK_GENERIC, B.ALGO_LITERAL):
+        try:
+            sensor.algorithm = a
+            out.append(a)
+        except B.ShwfsError as e:
+            assert e.code == B.SHWFS_EUNSUPPORTED
+    return out
+
+
+def _img_err(got, want):
+    pk = want.max(axis=(-2, -1), keepdims=True)
+    return float((np.abs(got - want) / pk).max())
+
+
+@pytest.mark.parametrize("cfg_id,T", [(1, 4), (2, 3), (3, 3), (5, 2)])
+def test_slopes_and_binned_images_match_oracle(gpu, oracle, cfg_id, T):
+    """Every spot of T full frames, every algorithm that has an instance for the sizes (configs 1,2,3,5;
+    config 4 is config 3 with six launch points, covered by test_config4_* below)."""
+    torch, B = gpu
+    c = W.CONFIGS[cfg_id]
+    amp = W.pupil_mask(c)
+    ph = W.phase_frames(c, 0, range(T))
+    with B.from_config(c, 0) as s:
+        yx = s.valid_yx
+        np.testing.assert_array_equal(yx, oracle.valid_list(amp, c.n, c.min_illum))
+        K = W.elongation_kernels(c, 0, yx)
+        want, wimg = oracle.measure(ph, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K, stage=2)
+        phd = torch.from_numpy(ph).cuda()
+        algos = _algos(s, B)
+        assert B.ALGO_WK in algos
+        for a in algos:
+            s.algorithm = a
+            got = s.measure(phd).cpu().numpy()
+            img = s.debug_spots(phd, 2).cpu().numpy()
+            assert got.shape == (T, len(yx), 2)
+            assert np.abs(got - want).max() <= SLOPE_TOL, (a, np.abs(got - want).max())
+            assert _img_err(img, wimg) <= IMAGE_TOL, (a, _img_err(img, wimg))
+
+
+@pytest.mark.parametrize("wfs", [0, 5])
+def test_config4_full_batch_sampled_spots(gpu, oracle, wfs):
+    """The launch configuration bench.py times: config 4, one 100-frame batch of one WFS (463 200 spots in
+    one launch); 3000 sampled (frame, subaperture) outputs are recomputed one by one by the oracle."""
+    torch, B = gpu
+    c = W.CONFIGS[4]
+    amp = W.pupil_mask(c)
+    dev = torch.device("cuda")
+    phd = W.phase_frames_device(c, wfs, range(c.batch), dev)
+    with B.from_config(c, wfs) as s:
+        yx = s.valid_yx
+        got = s.measure(phd)
+        assert s.launch_count == 1
+        torch.cuda.synchronize()
+        got = got.cpu().numpy()
+    assert np.isfinite(got).all()
+    rng = np.random.default_rng(1234 + wfs)
+    ts = np.sort(rng.choice(c.batch, size=6, replace=False))
+    ts[0], ts[-1] = 0, c.batch - 1                       # first and last frame of the launch
+    for t in ts:
+        idx = np.sort(rng.choice(len(yx), size=500, replace=False))
+        idx[0], idx[-1] = 0, len(yx) - 1                 # first and last CTA / ragged tail
+        K = W.elongation_kernels(c, wfs, yx, subset=idx)
+        frame = phd[int(t)].cpu().numpy()[None]
+        want = oracle.measure(frame, amp, yx[idx], c.n, c.P, c.b, tau=c.tau, kernels=K)
+        err = np.abs(got[t, idx] - want[0]).max()
+        assert err <= SLOPE_TOL, (int(t), err)
+
+
+def test_config4_properties_at_full_size(gpu):
+    """Properties that hold at any size: a flat wavefront gives zero slopes on every subaperture of every WFS
+    geometry (I1), and frames are independent (permuting frames permutes slopes bit for bit)."""
+    torch, B = gpu
+    c = W.CONFIGS[4]
+    with B.from_config(c, 3) as s:
+        flat = torch.zeros((2, c.N, c.N), dtype=torch.float32, device="cuda")
+        flat[1] += 3.25                                   # piston
+        sl = s.measure(flat).cpu().numpy()
+        assert np.abs(sl).max() <= 2e-5
+        ph = W.phase_frames_device(c, 3, range(5), torch.device("cuda"))
+        a = s.measure(ph).cpu().numpy()
+        perm = [3, 0, 4, 1, 2]
+        b = s.measure(ph[perm].contiguous()).cpu().numpy()
+        np.testing.assert_array_equal(a[perm], b)
+
+
+@pytest.mark.parametrize("T", [1, 31, 33, 65])
+def test_ragged_batch_sizes(gpu, oracle, T):
+    """T not a multiple of the 32-spot CTA: spots straddle subapertures and the last CTA is partly empty."""
+    torch, B = gpu
+    c = W.CONFIGS[1]
+    amp = W.pupil_mask(c)
+    ph = W.phase_frames(c, 0, [t % 4 for t in range(T)])
+    rng = np.random.default_rng(T)
+    K = rng.random((80, c.P, c.P)).astype(np.float32)     # arbitrary (asymmetric) kernels: complex table
+    with B.Shwfs(amp, c.S, c.n, c.dx, W.LAMBDA_M, c.P, c.b, threshold_frac=0.1, elong_kernels=K) as s:
+        yx = s.valid_yx
+        want = oracle.measure(ph, amp, yx, c.n, c.P, c.b, tau=0.1, kernels=K)
+        for a in _algos(s, B):
+            s.algorithm = a
+            got = s.measure(torch.from_numpy(ph).cuda()).cpu().numpy()
+            assert np.abs(got - want).max() <= SLOPE_TOL, (a, T)
+
+
+def test_t_zero_is_a_noop(gpu):
+    torch, B = gpu
+    c = W.CONFIGS[1]
+    with B.from_config(c, 0) as s:
+        ph = torch.empty((0, c.N, c.N), dtype=torch.float32, device="cuda")
+        out = s.measure(ph)
+        assert out.shape == (0, s.nsub, 2)
+        assert s.launch_count == 0
+
+
+@pytest.mark.parametrize("n,P,b", [(8, 16, 1), (10, 32, 2), (16, 32, 2), (16, 64, 4), (8, 32, 2), (10, 16, 1),
+                                   (6, 16, 2), (12, 32, 1), (5, 8, 1)])
+def test_small_grids_all_sizes(gpu, oracle, n, P, b):
+    """3x3 subapertures with a partially lit mask, explicit valid list (including a dark subaperture), random
+    phases of several radians, with and without kernels, tau 0 and 0.1, both threshold modes."""
+    torch, B = gpu
+    S = 3
+    N = S * n
+    rng = np.random.default_rng(n * 1000 + P + b)
+    amp = (rng.random((N, N)) > 0.2).astype(np.float32) * rng.uniform(0.5, 1.0, (N, N)).astype(np.float32)
+    amp[:n, :n] = 0.0                                      # a dark subaperture: sum Wt == 0 => (0,0)
+    yx = np.array([[sy, sx] for sy in range(S) for sx in range(S)], dtype=np.int32)
+    ph = rng.normal(0, 3.0, (5, N, N)).astype(np.float32)
+    D = P // b
+    for use_k in (False, True):
+        K = rng.random((len(yx), P, P)).astype(np.float32) if use_k else None
+        for tau, mode in ((0.0, 0), (0.1, 0), (0.3, 1)):
+            try:
+                s = B.Shwfs(amp, S, n, 0.05, W.LAMBDA_M, P, b, valid_yx=yx, threshold_frac=tau,
+                            threshold_mode=mode, phase_to_rad=0.7, elong_kernels=K)
+            except B.ShwfsError as e:
+                assert e.code == B.SHWFS_EUNSUPPORTED and (n > 32 or D > 32)
+                continue
+            with s:
+                want, wimg = oracle.measure(ph, amp, yx, n, P, b, c_phi=np.float32(0.7), tau=tau, mode=mode,
+                                            kernels=K, stage=2)
+                phd = torch.from_numpy(ph).cuda()
+                for a in _algos(s, B):
+                    s.algorithm = a
+                    got = s.measure(phd).cpu().numpy()
+                    img = s.debug_spots(phd, 2).cpu().numpy()
+                    lit = wimg.max(axis=(2, 3)) > 0
+                    assert (got[~lit] == 0).all()
+                    assert np.abs(img[~lit]).max() == 0
+                    assert _img_err(img[lit], wimg[lit]) <= IMAGE_TOL, (a, use_k, tau, mode)
+                    if mode == 0:
+                        assert np.abs(got - want).max() <= SLOPE_TOL, (a, use_k, tau, mode)
+                    else:
+                        # hard mask: a pixel within rounding of the threshold may flip (reading A7); compare
+                        # the spots whose pixels all stay clear of it, require the rest to be valid CoGs
+                        m = wimg.max(axis=(2, 3), keepdims=True)
+                        clear = (np.abs(wimg - tau * m) > 1e-5 * m).all(axis=(2, 3)) | ~lit
+                        assert np.abs(got - want)[clear].max() <= SLOPE_TOL
+                        assert clear.mean() > 0.9
+                        assert np.abs(got).max() <= (D - 1) / 2
+
+
+def test_invariants_on_device(gpu):
+    """I1 flat, I2 integer tilt, I7 piston / 2*pi wraps at +-1000 rad, I8 negation, on the device path itself."""
+    torch, B = gpu
+    c = W.CONFIGS[3]
+    dev = torch.device("cuda")
+    with B.from_config(c, 0) as s:
+        ph = W.phase_frames_device(c, 0, range(1), dev)
+        base = s.measure(ph).cpu().numpy()
+        # I7: piston and integer multiples of 2*pi (range reduction at large arguments)
+        k2pi = torch.randint(-150, 150, ph.shape, device=dev).to(torch.float64) * (2 * np.pi)
+        wrapped = (ph.to(torch.float64) + k2pi).to(torch.float32)
+        got = s.measure(wrapped).cpu().numpy()
+        assert np.abs(got - base).max() <= 5e-3          # fp32 input rounding at |phi| ~ 1000 rad: ulp 6e-5 rad
+        got = s.measure(ph + 1.0).cpu().numpy()
+        assert np.abs(got - base).max() <= 1e-4
+        # I8: phase negation reflects the spot about the detector centre: slopes negate
+        neg = s.measure(-ph).cpu().numpy()
+        assert np.abs(neg + base).max() <= 1e-4
+        # I2: tilt by b unbinned pixels moves every centroid by exactly 1 detector px when nothing crosses the
+        # edge; with wrapped elongated spots only check the un-elongated handle below
+    c2 = W.CONFIGS[2]
+    with B.from_config(c2, 0) as s:
+        ph = 0.3 * W.phase_frames_device(c2, 0, range(1), dev)
+        base = s.measure(ph).cpu().numpy()
+        x = torch.arange(c2.N, device=dev, dtype=torch.float64)
+        tilt = (2 * np.pi * c2.b / c2.P) * x[None, None, :]
+        got = s.measure((ph.to(torch.float64) + tilt).to(torch.float32)).cpu().numpy()
+        d = got - base
+        keep = np.abs(base).max(axis=2) < 1.0             # well inside the field
+        assert np.abs(d[keep][:, 0] - 1.0).max() <= 5e-2  # threshold keeps it near, not exactly, 1 (tails wrap)
+        assert np.abs(d[keep][:, 1]).max() <= 5e-2
+
+
+def test_nan_stays_in_its_spot(gpu):
+    torch, B = gpu
+    c = W.CONFIGS[1]
+    with B.from_config(c, 0) as s:
+        ph = torch.from_numpy(W.phase_frames(c, 0, range(2))).cuda()
+        base = s.measure(ph).cpu().numpy()
+        yx = s.valid_yx
+        sy, sx = yx[7]
+        ph2 = ph.clone()
+        ph2[1, sy * c.n + 2, sx * c.n + 3] = float("nan")
+        got = s.measure(ph2).cpu().numpy()
+        mask = np.ones(got.shape[:2], bool)
+        mask[1, 7] = False
+        np.testing.assert_array_equal(got[mask], base[mask])
