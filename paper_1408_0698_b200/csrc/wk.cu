@@ -21,6 +21,7 @@
  */
 #include "internal.h"
 #include "fft_regs.cuh"
+#include "field.cuh"
 
 namespace {
 
@@ -84,18 +85,6 @@ __global__ void wk_table_kernel(const float *__restrict__ K, int has_k, int n, i
         M[(size_t)i * n * LX + idx] = make_float2((float)((zr * br - zi * bi) * scale),
                                                   (float)((zr * bi + zi * br) * scale));
     }
-}
-
-/* H2: field value of one pupil pixel.  turns = phase_to_rad / (2*pi); ramp = (j+k) / (2P) in turns
- * (reading A5).  The argument is reduced to [-1/2, 1/2] turns before the fast sincos so that the
- * +-60 rad open-loop phases of the MAORY pupil keep ~1e-6 absolute accuracy.                    */
-__device__ __forceinline__ float2 field_value(float ph, float amp, float turns, float ramp)
-{
-    float u = fmaf(ph, turns, -ramp);
-    u -= rintf(u);
-    float s, c;
-    __sincosf(u * 6.283185307179586f, &s, &c);
-    return make_float2(amp * c, amp * s);
 }
 
 /* H7 + H8 on a half-warp: lane C (0..15) holds column C of B as bcol[R].  Returns slopes in lane 0

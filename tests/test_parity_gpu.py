@@ -56,6 +56,35 @@ def test_slopes_and_binned_images_match_oracle(gpu, oracle, cfg_id, T):
             assert _img_err(img, wimg) <= IMAGE_TOL, (a, _img_err(img, wimg))
 
 
+@pytest.mark.parametrize("cfg_id,T", [(1, 4), (2, 1), (3, 1), (5, 1)])
+def test_unbinned_intensities_match_oracle(gpu, oracle, cfg_id, T):
+    """north_star: "per-subaperture intensities within 1e-4 of the spot peak" -- the centred P x P intensity
+    |DFT(e)|^2/P^2 (stage 0) and the centred image after the elongation convolution (stage 1) of every spot,
+    produced by the literal FFT chain, against the oracle's O4/O6 and O5/O6 images."""
+    torch, B = gpu
+    c = W.CONFIGS[cfg_id]
+    amp = W.pupil_mask(c)
+    ph = W.phase_frames(c, 0, range(T))
+    with B.from_config(c, 0) as s:
+        yx = s.valid_yx
+        if cfg_id == 5:                                   # 64x64 float64 images: keep a spread subset
+            yx = yx[:: 4]
+        K = W.elongation_kernels(c, 0, s.valid_yx)
+    if K is not None and cfg_id == 5:
+        K = K[:: 4]
+    with B.Shwfs(amp, c.S, c.n, c.dx, W.LAMBDA_M, c.P, c.b, valid_yx=yx, threshold_frac=c.tau,
+                 elong_kernels=K) as s:
+        phd = torch.from_numpy(ph).cuda()
+        for stage in (0, 1):
+            want_sl, wimg = oracle.measure(ph, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K, stage=stage)
+            img = s.debug_spots(phd, stage).cpu().numpy()
+            assert img.shape == (T, len(yx), c.P, c.P)
+            assert _img_err(img, wimg) <= IMAGE_TOL, (stage, _img_err(img, wimg))
+        s.algorithm = B.ALGO_LITERAL
+        got = s.measure(phd).cpu().numpy()
+        assert np.abs(got - want_sl).max() <= SLOPE_TOL
+
+
 @pytest.mark.parametrize("wfs", [0, 5])
 def test_config4_full_batch_sampled_spots(gpu, oracle, wfs):
     """The launch configuration bench.py times: config 4, one 100-frame batch of one WFS (463 200 spots in
