@@ -89,7 +89,8 @@ __global__ void wk_table_kernel(const float *__restrict__ K, int has_k, int n, i
 
 /* H7 + H8 on a half-warp: lane C (0..15) holds column C of B as bcol[R].  Returns slopes in lane 0
  * of the half-warp.  Shuffles use xor offsets < 16, so the two halves of a warp stay separate.    */
-__device__ __forceinline__ float2 cog16(const float (&bcol)[16], int C, float tau, int mode)
+template <int MODE>
+__device__ __forceinline__ float2 cog16(const float (&bcol)[16], int C, float tau)
 {
     float mx = bcol[0];
 #pragma unroll
@@ -101,7 +102,7 @@ __device__ __forceinline__ float2 cog16(const float (&bcol)[16], int C, float ta
 #pragma unroll
     for (int R = 0; R < 16; ++R) {
         const float v = bcol[R];
-        const float w = mode == 0 ? fmaxf(v - thr, 0.f) : (v >= thr ? v : 0.f);
+        const float w = MODE == 0 ? fmaxf(v - thr, 0.f) : (v >= thr ? v : 0.f);
         sw += w;
         sy = fmaf(w, (float)R - 7.5f, sy);
     }
@@ -113,19 +114,22 @@ __device__ __forceinline__ float2 cog16(const float (&bcol)[16], int C, float ta
         sy += __shfl_xor_sync(0xffffffffu, sy, o);
     }
     if (sw == 0.f) return make_float2(0.f, 0.f);
-    return make_float2(sx / sw, sy / sw);
+    const float inv = 1.0f / sw;
+    return make_float2(sx * inv, sy * inv);
 }
 
 /* ------------------------------------------------------------------------------------------------
  * Specialised kernel: n in {8,10,16}, D = 16.  One CTA = 32 consecutive spots g = i*T + t (frame
  * fastest, so the 32 lanes of a warp mostly share one subaperture's table M_i), n/2 warps.
  *
- *   phase 0  all threads: gather the 32 patches, H2 sincos, field e -> shared memory.
+ *   phase 0  thread = (pixel pair, spot group): H1 gather as 8-byte loads (all of a thread's loads in
+ *            flight at once), H2 sincos, field e -> shared memory.
  *   phase 1  lane = spot, warp c = lag-row class {c, n-c} (class 0 = {0, n/2}): the thread
  *            accumulates G[ly, -(n-1)..n-1] for its lag rows in registers, one row pair (j, j+ly)
  *            at a time (2n-1 independent complex accumulators, 4 n^2 FFMA per 2*2n/4 LDS.128), then
  *            multiplies by M_i[ly,:], aliases lx mod 16 and does the 16-point x-transform in
- *            registers: H[ly][C] -> shared memory.
+ *            registers: H[ly][C] -> shared memory.  Lag row 0 is Hermitian in lx (G[0,-lx] =
+ *            conj G[0,lx]), so only lx >= 0 is accumulated there: every class costs 4 n^3 FFMA.
  *   phase 2  half-warp = spot, lane = detector column C: 16-point y-transform (real part) of
  *            H[0..n-1][C], then H7/H8 with half-warp shuffles; lane 0 writes the two slopes.
  * ---------------------------------------------------------------------------------------------- */
@@ -135,9 +139,13 @@ struct WkCfg {
     static constexpr int NW = n / 2;
     static constexpr int THREADS = 32 * NW;
     static constexpr int SPOTS = 32;
+    static constexpr int NP = n * n / 2;                    /* pixel pairs (float4 of e) per spot        */
+    static constexpr int SG = THREADS / NP;                 /* spot groups in phase 0: 4 / 3 / 2         */
+    static constexpr int ITEMS = (SPOTS + SG - 1) / SG;     /* spots per phase-0 thread: 8 / 11 / 16     */
     static constexpr int ES = (((2 * n * n) / 4) | 1) * 4;  /* floats per spot; /4 odd => LDS.128 conflict-free */
     static constexpr int HS = (((n * 32) / 4) | 1) * 4;
-    static constexpr size_t SMEM = sizeof(float) * (size_t)(SPOTS * ES + SPOTS * HS) + sizeof(int) * 3 * SPOTS;
+    static constexpr size_t SMEM = sizeof(float) * (size_t)(SPOTS * ES + SPOTS * HS) + sizeof(int4) * SPOTS;
+    static constexpr int MIN_CTAS = (int)((227 * 1024) / (SMEM + 1024)) < 1 ? 1 : (int)((227 * 1024) / (SMEM + 1024));
     static_assert(n % 2 == 0 && n <= 16, "n must be even and <= 16");
 };
 
@@ -154,18 +162,23 @@ struct WkArgs {
 };
 
 template <int n>
+__device__ __forceinline__ void load_row(const float *__restrict__ p, float (&r)[2 * n])
+{
+#pragma unroll
+    for (int q = 0; q < (2 * n) / 4; ++q) {
+        const float4 v = reinterpret_cast<const float4 *>(p)[q];
+        r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w;
+    }
+}
+
+/* G[lx] += e1[k] * conj(e2[k2]),  lx = k2 - k, all n^2 products of one row pair */
+template <int n>
 __device__ __forceinline__ void rowpair_acc(const float *__restrict__ p1, const float *__restrict__ p2,
                                             float (&acc)[2 * (2 * n - 1)])
 {
     float r1[2 * n], r2[2 * n];
-#pragma unroll
-    for (int q = 0; q < (2 * n) / 4; ++q) {
-        const float4 v = reinterpret_cast<const float4 *>(p1)[q];
-        r1[4 * q] = v.x; r1[4 * q + 1] = v.y; r1[4 * q + 2] = v.z; r1[4 * q + 3] = v.w;
-        const float4 u = reinterpret_cast<const float4 *>(p2)[q];
-        r2[4 * q] = u.x; r2[4 * q + 1] = u.y; r2[4 * q + 2] = u.z; r2[4 * q + 3] = u.w;
-    }
-    /* G[lx] += e[j,k] * conj(e[j+ly,k2]),  lx = k2 - k */
+    load_row<n>(p1, r1);
+    load_row<n>(p2, r2);
 #pragma unroll
     for (int k = 0; k < n; ++k) {
 #pragma unroll
@@ -179,19 +192,32 @@ __device__ __forceinline__ void rowpair_acc(const float *__restrict__ p1, const 
     }
 }
 
+/* lag row 0: the row against itself, lx >= 0 only */
 template <int n>
-__device__ __forceinline__ void lag_row(const float *__restrict__ eb, int ly, int rows,
-                                        const float2 *__restrict__ Mrow, float *__restrict__ hrow)
+__device__ __forceinline__ void rowself_acc(const float *__restrict__ p, float (&acc)[2 * (2 * n - 1)])
 {
-    constexpr int LX = 2 * n - 1;
-    float acc[2 * LX];
+    float r[2 * n];
+    load_row<n>(p, r);
 #pragma unroll
-    for (int a = 0; a < 2 * LX; ++a) acc[a] = 0.f;
-#pragma unroll 1
-    for (int j = 0; j < rows; ++j)
-        rowpair_acc<n>(eb + j * 2 * n, eb + (j + ly) * 2 * n, acc);
+    for (int k = 0; k < n; ++k) {
+        acc[2 * (n - 1)] = fmaf(r[2 * k], r[2 * k], acc[2 * (n - 1)]);
+        acc[2 * (n - 1)] = fmaf(r[2 * k + 1], r[2 * k + 1], acc[2 * (n - 1)]);
+#pragma unroll
+        for (int k2 = k + 1; k2 < n; ++k2) {
+            const int a = k2 - k + n - 1;
+            acc[2 * a] = fmaf(r[2 * k], r[2 * k2], acc[2 * a]);
+            acc[2 * a] = fmaf(r[2 * k + 1], r[2 * k2 + 1], acc[2 * a]);
+            acc[2 * a + 1] = fmaf(r[2 * k + 1], r[2 * k2], acc[2 * a + 1]);
+            acc[2 * a + 1] = fmaf(-r[2 * k], r[2 * k2 + 1], acc[2 * a + 1]);
+        }
+    }
+}
 
-    /* S = G * M, aliased onto lx mod 16 */
+/* S = G * M aliased onto lx mod 16, 16-point x-transform, H[ly][0..15] -> shared memory */
+template <int n>
+__device__ __forceinline__ void finish_row(const float (&acc)[2 * (2 * n - 1)], const float2 *__restrict__ Mrow,
+                                           float *__restrict__ hrow)
+{
     float sr[16], si[16];
 #pragma unroll
     for (int m = 0; m < 16; ++m) {
@@ -217,22 +243,19 @@ __device__ __forceinline__ void lag_row(const float *__restrict__ eb, int ly, in
     fft_dif<16, +1>(sr, si);                     /* H[C] = sum_m s'[m] w_16^(C m) */
 #pragma unroll
     for (int C = 0; C < 16; C += 2) {
-        constexpr int dummy = 0; (void)dummy;
         const int p0 = fft_out_index<16>(C), p1 = fft_out_index<16>(C + 1);
         reinterpret_cast<float4 *>(hrow)[C / 2] = make_float4(sr[p0], si[p0], sr[p1], si[p1]);
     }
 }
 
-template <int n>
-__global__ void __launch_bounds__(WkCfg<n>::THREADS) wk_measure_kernel(const WkArgs A)
+template <int n, int MODE>
+__global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_measure_kernel(const WkArgs A)
 {
     using Cfg = WkCfg<n>;
     extern __shared__ __align__(16) float smem[];
     float *ebuf = smem;
     float *hbuf = smem + Cfg::SPOTS * Cfg::ES;
-    int *s_off = reinterpret_cast<int *>(hbuf + Cfg::SPOTS * Cfg::HS);
-    int *s_t = s_off + Cfg::SPOTS;
-    int *s_i = s_t + Cfg::SPOTS;
+    int4 *s_info = reinterpret_cast<int4 *>(hbuf + Cfg::SPOTS * Cfg::HS);   /* {patch offset, t, i, -} */
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g0 = blockIdx.x * Cfg::SPOTS;
@@ -246,21 +269,52 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS) wk_measure_kernel(const WkA
             const int2 yx = A.valid[i];
             off = yx.x * n * A.N + yx.y * n;
         }
-        s_off[tid] = off; s_t[tid] = t; s_i[tid] = i;
+        s_info[tid] = make_int4(off, t, i, 0);
     }
     __syncthreads();
 
-    /* ---- phase 0: H1 gather + H2 field ---- */
-    for (int p = tid; p < Cfg::SPOTS * n * n; p += Cfg::THREADS) {
-        const int s = p / (n * n), q = p - s * (n * n), j = q / n, k = q - j * n;
-        float2 e = make_float2(0.f, 0.f);
-        if (s_i[s] >= 0) {
-            const int o = s_off[s] + j * A.N + k;
-            const float ph = __ldg(A.phase + (size_t)s_t[s] * A.frame_stride + o);
-            const float am = __ldg(A.amp + o);
-            e = field_value(ph, am, A.turns, (float)(j + k) * A.ramp_unit);
+    /* ---- phase 0: H1 gather + H2 field.  Thread = pixel pair q2 of the spots sg, sg+SG, ... ---- */
+    {
+        const int sg = tid / Cfg::NP, q2 = tid - sg * Cfg::NP;
+        if (sg < Cfg::SG) {
+            const int j = q2 / (n / 2), kk = q2 - j * (n / 2);
+            const int poff = j * A.N + 2 * kk;
+            const float ramp0 = (float)(j + 2 * kk) * A.ramp_unit, ramp1 = ramp0 + A.ramp_unit;
+            float2 ph[Cfg::ITEMS];
+            int aoff[Cfg::ITEMS];
+#pragma unroll
+            for (int r = 0; r < Cfg::ITEMS; ++r) {
+                const int s = sg + r * Cfg::SG;
+                aoff[r] = -1;
+                ph[r] = make_float2(0.f, 0.f);
+                if (s < Cfg::SPOTS) {
+                    const int4 inf = s_info[s];
+                    if (inf.z >= 0) {
+                        aoff[r] = inf.x + poff;
+                        ph[r] = __ldg(reinterpret_cast<const float2 *>(A.phase + (size_t)inf.y * A.frame_stride + aoff[r]));
+                    }
+                }
+            }
+            float2 am = make_float2(0.f, 0.f);
+            int acur = -1;
+#pragma unroll
+            for (int r = 0; r < Cfg::ITEMS; ++r) {
+                const int s = sg + r * Cfg::SG;
+                if (s < Cfg::SPOTS) {
+                    float4 e = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (aoff[r] >= 0) {
+                        if (aoff[r] != acur) {          /* amplitude patch changes only with the subaperture */
+                            acur = aoff[r];
+                            am = __ldg(reinterpret_cast<const float2 *>(A.amp + acur));
+                        }
+                        const float2 e0 = field_value(ph[r].x, am.x, A.turns, ramp0);
+                        const float2 e1 = field_value(ph[r].y, am.y, A.turns, ramp1);
+                        e = make_float4(e0.x, e0.y, e1.x, e1.y);
+                    }
+                    reinterpret_cast<float4 *>(ebuf + s * Cfg::ES)[q2] = e;
+                }
+            }
         }
-        reinterpret_cast<float2 *>(ebuf + s * Cfg::ES)[q] = e;
     }
     __syncthreads();
 
@@ -268,12 +322,28 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS) wk_measure_kernel(const WkA
     {
         const float *eb = ebuf + lane * Cfg::ES;
         float *hb = hbuf + lane * Cfg::HS;
-        const int i = max(s_i[lane], 0);
+        const int i = max(s_info[lane].z, 0);
         const float2 *Mi = A.M + (size_t)i * A.mstride;
-        const int lyA = warp == 0 ? 0 : warp;
-        const int lyB = warp == 0 ? n / 2 : n - warp;
-        lag_row<n>(eb, lyA, n - lyA, Mi + lyA * Cfg::LX, hb + lyA * 32);
-        lag_row<n>(eb, lyB, n - lyB, Mi + lyB * Cfg::LX, hb + lyB * 32);
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            const int ly = pass == 0 ? warp : (warp == 0 ? n / 2 : n - warp);
+            float acc[2 * Cfg::LX];
+#pragma unroll
+            for (int a = 0; a < 2 * Cfg::LX; ++a) acc[a] = 0.f;
+            if (ly == 0) {
+#pragma unroll 1
+                for (int j = 0; j < n; ++j) rowself_acc<n>(eb + j * 2 * n, acc);
+#pragma unroll
+                for (int lx = 1; lx < n; ++lx) {
+                    acc[2 * (n - 1 - lx)] = acc[2 * (n - 1 + lx)];
+                    acc[2 * (n - 1 - lx) + 1] = -acc[2 * (n - 1 + lx) + 1];
+                }
+            } else {
+#pragma unroll 1
+                for (int j = 0; j < n - ly; ++j) rowpair_acc<n>(eb + j * 2 * n, eb + (j + ly) * 2 * n, acc);
+            }
+            finish_row<n>(acc, Mi + ly * Cfg::LX, hb + ly * 32);
+        }
     }
     __syncthreads();
 
@@ -294,10 +364,10 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS) wk_measure_kernel(const WkA
             float bcol[16];
 #pragma unroll
             for (int R = 0; R < 16; ++R) bcol[R] = yr[fft_out_index<16>(R)];
-            const float2 sl = cog16(bcol, C, A.tau, A.mode);
-            const int i = s_i[s];
-            if (i >= 0) {
-                const size_t o = (size_t)s_t[s] * A.nsub + i;
+            const float2 sl = cog16<MODE>(bcol, C, A.tau);
+            const int4 inf = s_info[s];
+            if (inf.z >= 0) {
+                const size_t o = (size_t)inf.y * A.nsub + inf.z;
                 if (C == 0) reinterpret_cast<float2 *>(A.slopes)[o] = sl;
                 if (A.binned) {
 #pragma unroll
@@ -415,22 +485,28 @@ __global__ void __launch_bounds__(GEN_THREADS) wk_generic_kernel(const WkArgs A,
         for (int px = tid; px < D * D; px += GEN_THREADS) A.binned[o * D * D + px] = B[px];
 }
 
-template <int n>
-cudaError_t launch_special(const WkArgs &A, cudaStream_t st)
+template <int n, int MODE>
+cudaError_t launch_special_mode(const WkArgs &A, cudaStream_t st)
 {
     using Cfg = WkCfg<n>;
     static bool attr_set[64] = {false};
     int dev = 0;
     cudaGetDevice(&dev);
     if (dev >= 0 && dev < 64 && !attr_set[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(wk_measure_kernel<n>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(wk_measure_kernel<n, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
         attr_set[dev] = true;
     }
     const int grid = (A.total + Cfg::SPOTS - 1) / Cfg::SPOTS;
-    wk_measure_kernel<n><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(A);
+    wk_measure_kernel<n, MODE><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(A);
     return cudaGetLastError();
+}
+
+template <int n>
+cudaError_t launch_special(const WkArgs &A, cudaStream_t st)
+{
+    return A.mode == 0 ? launch_special_mode<n, 0>(A, st) : launch_special_mode<n, 1>(A, st);
 }
 
 }  // namespace
