@@ -171,51 +171,82 @@ __device__ __forceinline__ void load_row(const float *__restrict__ p, float (&r)
     }
 }
 
-/* G[lx] += e1[k] * conj(e2[k2]),  lx = k2 - k, all n^2 products of one row pair */
+/* G[lx] += e1[k] * conj(e2[k2]),  lx = k2 - k, all n^2 products of one row pair.  With e1 = a + ib,
+ * conj(e2) = c - id, s = a + b, t = c - d the product is (ac + bd) + i(st - ac + bd): three real products
+ * instead of four.  X = sum ac and Y = sum bd share one packed FFMA2 (sm_100a fma.rn.f32x2 on the
+ * (re,im) register pairs exactly as LDS.128 delivers them), Z = sum st is a scalar FFMA; G = (X + Y) +
+ * i(Z - X + Y) is formed once per lag row (lag_value).  3 FMA-pipe cycles and 2 issue slots per complex
+ * MAC instead of 4 and 4.                                                                                */
 template <int n>
-__device__ __forceinline__ void rowpair_acc(const float *__restrict__ p1, const float *__restrict__ p2,
-                                            float (&acc)[2 * (2 * n - 1)])
+struct LagAcc {
+    float2 xy[2 * n - 1];
+    float z[2 * n - 1];
+    __device__ __forceinline__ void clear()
+    {
+#pragma unroll
+        for (int a = 0; a < 2 * n - 1; ++a) { xy[a] = make_float2(0.f, 0.f); z[a] = 0.f; }
+    }
+    __device__ __forceinline__ float2 lag_value(int a) const
+    {
+        return make_float2(xy[a].x + xy[a].y, (z[a] - xy[a].x) + xy[a].y);
+    }
+};
+
+template <int n>
+__device__ __forceinline__ void load_row2(const float *__restrict__ p, float2 (&r)[n])
 {
-    float r1[2 * n], r2[2 * n];
-    load_row<n>(p1, r1);
-    load_row<n>(p2, r2);
+#pragma unroll
+    for (int q = 0; q < n / 2; ++q) {
+        const float4 v = reinterpret_cast<const float4 *>(p)[q];
+        r[2 * q] = make_float2(v.x, v.y);
+        r[2 * q + 1] = make_float2(v.z, v.w);
+    }
+}
+
+template <int n>
+__device__ __forceinline__ void rowpair_acc(const float *__restrict__ p1, const float *__restrict__ p2, LagAcc<n> &A)
+{
+    float2 e1[n], e2[n];
+    float s[n], t[n];
+    load_row2<n>(p1, e1);
+    load_row2<n>(p2, e2);
+#pragma unroll
+    for (int k = 0; k < n; ++k) { s[k] = e1[k].x + e1[k].y; t[k] = e2[k].x - e2[k].y; }
 #pragma unroll
     for (int k = 0; k < n; ++k) {
 #pragma unroll
         for (int k2 = 0; k2 < n; ++k2) {
             const int a = k2 - k + n - 1;
-            acc[2 * a] = fmaf(r1[2 * k], r2[2 * k2], acc[2 * a]);
-            acc[2 * a] = fmaf(r1[2 * k + 1], r2[2 * k2 + 1], acc[2 * a]);
-            acc[2 * a + 1] = fmaf(r1[2 * k + 1], r2[2 * k2], acc[2 * a + 1]);
-            acc[2 * a + 1] = fmaf(-r1[2 * k], r2[2 * k2 + 1], acc[2 * a + 1]);
+            A.xy[a] = __ffma2_rn(e1[k], e2[k2], A.xy[a]);
+            A.z[a] = fmaf(s[k], t[k2], A.z[a]);
         }
     }
 }
 
-/* lag row 0: the row against itself, lx >= 0 only */
+/* lag row 0: the row against itself, lx >= 0 only (G[0,-lx] = conj G[0,lx]; G[0,0] is real) */
 template <int n>
-__device__ __forceinline__ void rowself_acc(const float *__restrict__ p, float (&acc)[2 * (2 * n - 1)])
+__device__ __forceinline__ void rowself_acc(const float *__restrict__ p, LagAcc<n> &A)
 {
-    float r[2 * n];
-    load_row<n>(p, r);
+    float2 e[n];
+    float s[n], t[n];
+    load_row2<n>(p, e);
+#pragma unroll
+    for (int k = 0; k < n; ++k) { s[k] = e[k].x + e[k].y; t[k] = e[k].x - e[k].y; }
 #pragma unroll
     for (int k = 0; k < n; ++k) {
-        acc[2 * (n - 1)] = fmaf(r[2 * k], r[2 * k], acc[2 * (n - 1)]);
-        acc[2 * (n - 1)] = fmaf(r[2 * k + 1], r[2 * k + 1], acc[2 * (n - 1)]);
 #pragma unroll
-        for (int k2 = k + 1; k2 < n; ++k2) {
+        for (int k2 = 0; k2 < n; ++k2) {
+            if (k2 < k) continue;
             const int a = k2 - k + n - 1;
-            acc[2 * a] = fmaf(r[2 * k], r[2 * k2], acc[2 * a]);
-            acc[2 * a] = fmaf(r[2 * k + 1], r[2 * k2 + 1], acc[2 * a]);
-            acc[2 * a + 1] = fmaf(r[2 * k + 1], r[2 * k2], acc[2 * a + 1]);
-            acc[2 * a + 1] = fmaf(-r[2 * k], r[2 * k2 + 1], acc[2 * a + 1]);
+            A.xy[a] = __ffma2_rn(e[k], e[k2], A.xy[a]);
+            if (k2 > k) A.z[a] = fmaf(s[k], t[k2], A.z[a]);
         }
     }
 }
 
 /* S = G * M aliased onto lx mod 16, 16-point x-transform, H[ly][0..15] -> shared memory */
 template <int n>
-__device__ __forceinline__ void finish_row(const float (&acc)[2 * (2 * n - 1)], const float2 *__restrict__ Mrow,
+__device__ __forceinline__ void finish_row(const float2 (&acc)[2 * n - 1], const float2 *__restrict__ Mrow,
                                            float *__restrict__ hrow)
 {
     float sr[16], si[16];
@@ -229,7 +260,7 @@ __device__ __forceinline__ void finish_row(const float (&acc)[2 * (2 * n - 1)], 
             if (lx > n - 1 || lx < -(n - 1)) continue;
             const int a = lx + n - 1;
             const float2 mv = __ldg(Mrow + a);
-            const float gr = acc[2 * a], gi = acc[2 * a + 1];
+            const float gr = acc[a].x, gi = acc[a].y;
             if (first) {
                 sr[m] = fmaf(gr, mv.x, -gi * mv.y);
                 si[m] = fmaf(gr, mv.y, gi * mv.x);
@@ -327,20 +358,27 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
 #pragma unroll 1
         for (int pass = 0; pass < 2; ++pass) {
             const int ly = pass == 0 ? warp : (warp == 0 ? n / 2 : n - warp);
-            float acc[2 * Cfg::LX];
-#pragma unroll
-            for (int a = 0; a < 2 * Cfg::LX; ++a) acc[a] = 0.f;
+            LagAcc<n> L;
+            L.clear();
             if (ly == 0) {
 #pragma unroll 1
-                for (int j = 0; j < n; ++j) rowself_acc<n>(eb + j * 2 * n, acc);
-#pragma unroll
-                for (int lx = 1; lx < n; ++lx) {
-                    acc[2 * (n - 1 - lx)] = acc[2 * (n - 1 + lx)];
-                    acc[2 * (n - 1 - lx) + 1] = -acc[2 * (n - 1 + lx) + 1];
-                }
+                for (int j = 0; j < n; ++j) rowself_acc<n>(eb + j * 2 * n, L);
             } else {
 #pragma unroll 1
-                for (int j = 0; j < n - ly; ++j) rowpair_acc<n>(eb + j * 2 * n, eb + (j + ly) * 2 * n, acc);
+                for (int j = 0; j < n - ly; ++j) rowpair_acc<n>(eb + j * 2 * n, eb + (j + ly) * 2 * n, L);
+            }
+            float2 acc[Cfg::LX];
+            if (ly == 0) {
+                acc[n - 1] = make_float2(L.xy[n - 1].x + L.xy[n - 1].y, 0.f);
+#pragma unroll
+                for (int lx = 1; lx < n; ++lx) {
+                    const float2 g = L.lag_value(n - 1 + lx);
+                    acc[n - 1 + lx] = g;
+                    acc[n - 1 - lx] = make_float2(g.x, -g.y);
+                }
+            } else {
+#pragma unroll
+                for (int a = 0; a < Cfg::LX; ++a) acc[a] = L.lag_value(a);
             }
             finish_row<n>(acc, Mi + ly * Cfg::LX, hb + ly * 32);
         }
