@@ -39,8 +39,10 @@ F_NOM = {1: 10240, 2: 51200, 3: 153600, 4: 153600, 5: 737280}
 # (profiles/r01_fp32_peak.md).
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+# `ncu --set full` captures (profiles/r01_{wk10,wk16,lit32}_full_v4.md), keyed by config; None where no
+# capture of that config's kernel exists.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: 129148416 + 3808256, 3: 206536448 + 7660288, 4: 206536448 + 7660288,
+                                5: 506635264 + 7373568}
 
 
 def _dist_env():
@@ -225,8 +227,9 @@ def run_ours(args):
         spots_per_launch = frames * nsub
         ach = F_ALG[c.cfg] * spots_per_launch / (kern_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                    "frac": ach / FP32_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
-                    "kernel": f"wk_measure_kernel<{c.n}>" if sensors[0].algorithm == B.ALGO_WK else f"algo{sensors[0].algorithm}",
+                    "frac": ach / FP32_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(c.cfg),
+                    "kernel": {B.ALGO_WK: f"wk_measure_kernel<{c.n}>", B.ALGO_PRUNED_FFT: f"pruned_fft_kernel<{c.P}>",
+                               B.ALGO_LITERAL: f"literal_kernel<{c.P}>"}.get(sensors[0].algorithm, f"algo{sensors[0].algorithm}"),
                     "kernel_ms": kern_ms, "spots_per_launch": spots_per_launch,
                     "flops_per_spot": F_ALG[c.cfg], "flops_basis": "F_alg (SURVEY.md 8(d))",
                     "frac_nominal_fft_flops": F_NOM[c.cfg] * spots_per_launch / (kern_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,

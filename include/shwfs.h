@@ -55,6 +55,8 @@ extern "C" {
 #define SHWFS_ALGO_WK       2    /* Wiener-Khinchin lag-domain form: autocorrelation of the field, x   */
                                  /* precomputed (kernel MTF x bin x centre) table, D x D real transform */
 #define SHWFS_ALGO_WK_GENERIC 3  /* same form, size-generic unspecialised kernel                       */
+#define SHWFS_ALGO_PRUNED_FFT 4  /* no elongation kernels, D = 16: one input-pruned P x P FFT per spot,   */
+                                 /* half-warp per spot, bin + threshold + CoG in registers             */
 
 typedef struct shwfs_handle shwfs_handle;              /* opaque */
 

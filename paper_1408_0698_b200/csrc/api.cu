@@ -59,6 +59,7 @@ int pick_auto(const shwfs_handle *h)
     /* without kernels one P x P FFT is cheaper than the autocorrelation once
      * n >= 16; with kernels the lag-domain form always wins.  Fall back along the chain. */
     const bool wk = shwfs_wk_supported(h, 0), lit = shwfs_literal_supported(h);
+    if (shwfs_pruned_fft_supported(h) && (h->n >= 16 || !wk)) return SHWFS_ALGO_PRUNED_FFT;
     if (!h->has_kernels && lit && (h->n >= 16 || !wk)) return SHWFS_ALGO_LITERAL;
     if (wk) return SHWFS_ALGO_WK;
     if (shwfs_wk_supported(h, 1)) return SHWFS_ALGO_WK_GENERIC;
@@ -154,7 +155,7 @@ int shwfs_create(const shwfs_geometry *g, float lambda_m, int32_t pad, int32_t b
 
     int rc = SHWFS_OK;
     CU_TRY(cudaGetDevice(&h->device), "cudaGetDevice");
-    if (!shwfs_wk_supported(h, 0) && !shwfs_wk_supported(h, 1) && !shwfs_literal_supported(h)) { rc = SHWFS_EUNSUPPORTED; goto fail; }
+    if (!shwfs_wk_supported(h, 0) && !shwfs_wk_supported(h, 1) && !shwfs_literal_supported(h) && !shwfs_pruned_fft_supported(h)) { rc = SHWFS_EUNSUPPORTED; goto fail; }
     h->algo = pick_auto(h);
     if (h->algo < 0) { rc = SHWFS_EUNSUPPORTED; goto fail; }
 
@@ -224,6 +225,7 @@ int shwfs_set_algorithm(shwfs_handle *h, int32_t algo)
         break;
     case SHWFS_ALGO_WK: if (!shwfs_wk_supported(h, 0)) return SHWFS_EUNSUPPORTED; break;
     case SHWFS_ALGO_WK_GENERIC: if (!shwfs_wk_supported(h, 1)) return SHWFS_EUNSUPPORTED; break;
+    case SHWFS_ALGO_PRUNED_FFT: if (!shwfs_pruned_fft_supported(h)) return SHWFS_EUNSUPPORTED; break;
     default: return SHWFS_EINVAL;
     }
     h->algo = a;
@@ -256,6 +258,8 @@ static int run_path(shwfs_handle *h, const float *phase_dev, int T, float *slope
         e = shwfs_literal_launch(h, phase_dev, T, slopes_dev, stage, img, st);
     } else if (h->algo == SHWFS_ALGO_LITERAL) {
         e = shwfs_literal_launch(h, phase_dev, T, slopes_dev, stage, img, st);
+    } else if (h->algo == SHWFS_ALGO_PRUNED_FFT) {
+        e = shwfs_pruned_fft_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr, st);
     } else {
         e = shwfs_wk_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr,
                             h->algo == SHWFS_ALGO_WK_GENERIC, st);

@@ -64,6 +64,11 @@ cudaError_t shwfs_literal_launch(shwfs_handle *h, const float *phase, int T, flo
 cudaError_t shwfs_literal_build_khat(shwfs_handle *h, cudaStream_t st);
 int shwfs_literal_supported(const shwfs_handle *h);
 
+/* Pruned-FFT path (no elongation kernels, D = 16): slopes and optionally the binned image */
+cudaError_t shwfs_pruned_fft_launch(shwfs_handle *h, const float *phase, int T, float *slopes,
+                                    float *binned_or_null, cudaStream_t st);
+int shwfs_pruned_fft_supported(const shwfs_handle *h);
+
 void shwfs_note_cuda_error(cudaError_t e, const char *where);
 
 #endif /* SHWFS_INTERNAL_H_ */

@@ -22,6 +22,7 @@
 #include "internal.h"
 #include "fft_regs.cuh"
 #include "field.cuh"
+#include "cog.cuh"
 
 namespace {
 
@@ -85,37 +86,6 @@ __global__ void wk_table_kernel(const float *__restrict__ K, int has_k, int n, i
         M[(size_t)i * n * LX + idx] = make_float2((float)((zr * br - zi * bi) * scale),
                                                   (float)((zr * bi + zi * br) * scale));
     }
-}
-
-/* H7 + H8 on a half-warp: lane C (0..15) holds column C of B as bcol[R].  Returns slopes in lane 0
- * of the half-warp.  Shuffles use xor offsets < 16, so the two halves of a warp stay separate.    */
-template <int MODE>
-__device__ __forceinline__ float2 cog16(const float (&bcol)[16], int C, float tau)
-{
-    float mx = bcol[0];
-#pragma unroll
-    for (int R = 1; R < 16; ++R) mx = fmaxf(mx, bcol[R]);
-#pragma unroll
-    for (int o = 8; o >= 1; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-    const float thr = tau * mx;
-    float sw = 0.f, sy = 0.f;
-#pragma unroll
-    for (int R = 0; R < 16; ++R) {
-        const float v = bcol[R];
-        const float w = MODE == 0 ? fmaxf(v - thr, 0.f) : (v >= thr ? v : 0.f);
-        sw += w;
-        sy = fmaf(w, (float)R - 7.5f, sy);
-    }
-    float sx = sw * ((float)C - 7.5f);
-#pragma unroll
-    for (int o = 8; o >= 1; o >>= 1) {
-        sw += __shfl_xor_sync(0xffffffffu, sw, o);
-        sx += __shfl_xor_sync(0xffffffffu, sx, o);
-        sy += __shfl_xor_sync(0xffffffffu, sy, o);
-    }
-    if (sw == 0.f) return make_float2(0.f, 0.f);
-    const float inv = 1.0f / sw;
-    return make_float2(sx * inv, sy * inv);
 }
 
 /* ------------------------------------------------------------------------------------------------
