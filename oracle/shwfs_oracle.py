@@ -19,16 +19,17 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "shwfs_oracle.c"
+_SRCS = [_SRC, _HERE / "shwfs_oracle_lgs.c"]
 _LIB = _HERE / "libshwfs_oracle.so"
 _lib = None
 
 
 def build(force: bool = False) -> Path:
     """Compile shwfs_oracle.c -> libshwfs_oracle.so with gcc -O2 -fopenmp (the oracle as it stands)."""
-    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+    if force or not _LIB.exists() or any(_LIB.stat().st_mtime < f.stat().st_mtime for f in _SRCS):
         tmp = _LIB.with_suffix(f".tmp{os.getpid()}.so")
         cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
-               "-o", str(tmp), str(_SRC), "-lm"]
+               "-o", str(tmp), *map(str, _SRCS), "-lm"]
         subprocess.run(cmd, check=True)
         os.replace(tmp, _LIB)
     return _LIB
@@ -73,6 +74,23 @@ def lib():
         L.shwfs_oracle_measure.restype = C.c_int
         L.shwfs_oracle_max_threads.argtypes = []
         L.shwfs_oracle_max_threads.restype = C.c_int
+        u32p = np.ctypeslib.ndpointer(dtype=np.uint32, flags="C_CONTIGUOUS")
+        L.shwfs_oracle_field_layer.argtypes = [_f32p, _f32p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int] + \
+            [C.c_double] * 7 + [_f64p]
+        L.shwfs_oracle_field_layer.restype = None
+        L.shwfs_oracle_philox4x32.argtypes = [u32p, u32p, u32p]
+        L.shwfs_oracle_philox4x32.restype = None
+        L.shwfs_oracle_normal4.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, _f64p]
+        L.shwfs_oracle_normal4.restype = None
+        L.shwfs_oracle_add_noise.argtypes = [_f64p, C.c_int, C.c_double, C.c_double, C.c_uint64, C.c_uint32,
+                                             C.c_uint32, _f64p]
+        L.shwfs_oracle_add_noise.restype = None
+        L.shwfs_oracle_measure_lgs.argtypes = [_f32p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
+                                               _f32p, _i32p, C.c_int, C.c_double, C.c_double, _f64p, _f64p,
+                                               _f64p, _f64p, C.c_double, C.c_double, C.c_double, C.c_int,
+                                               C.c_void_p, C.c_double, C.c_double, C.c_uint64, _f64p, C.c_int,
+                                               C.c_void_p, C.c_int]
+        L.shwfs_oracle_measure_lgs.restype = C.c_int
         _lib = L
     return _lib
 
@@ -216,4 +234,85 @@ def measure(phase, amplitude, valid_yx, n, P, b, *, c_phi=1.0, tau=0.0, mode=0, 
                                     kptr, int(bool(conv_direct)), slopes, int(stage), iptr, int(nthreads))
     if rc:
         raise RuntimeError(f"shwfs_oracle_measure failed with code {rc}")
+    return (slopes, images) if stage >= 0 else slopes
+
+
+# ---- paper's full LGS model: sodium sub-layers (f1) and detector noise (f2), oracle/shwfs_oracle_lgs.c ----
+
+def field_layer(phase_frame, amplitude, n, P, sy, sx, dx, *, c_phi=1.0, defocus=0.0, cx=0.0, cy=0.0,
+                tilt_x=0.0, tilt_y=0.0):
+    """L1: complex P x P field of one sodium sub-layer (wavefront + a|r-r_c|^2 + g.r)."""
+    ph = _c(phase_frame, np.float32)
+    am = _c(amplitude, np.float32)
+    N = ph.shape[-1]
+    out = np.zeros((P, 2 * P), dtype=np.float64)
+    lib().shwfs_oracle_field_layer(ph, am, N, n, P, sy, sx, float(c_phi), float(dx), float(defocus), float(cx),
+                                   float(cy), float(tilt_x), float(tilt_y), out)
+    return out.view(np.complex128).reshape(P, P)
+
+
+def philox4x32(ctr, key):
+    """L5: one Philox4x32-10 block; ctr = 4 uint32, key = 2 uint32 -> 4 uint32."""
+    out = np.zeros(4, dtype=np.uint32)
+    lib().shwfs_oracle_philox4x32(_c(ctr, np.uint32), _c(key, np.uint32), out)
+    return out
+
+
+def normal4(seed, t, i, blk):
+    """L5: the four N(0,1) deviates of Philox block `blk` of spot (t, i)."""
+    z = np.zeros(4, dtype=np.float64)
+    lib().shwfs_oracle_normal4(int(seed), int(t), int(i), int(blk), z)
+    return z
+
+
+def add_noise(B, F, ron, seed, t, i):
+    """L4: counts = F*B + sqrt(max(F*B,0)+ron^2)*z on a D x D binned image (F <= 0: unchanged)."""
+    B = _c(B, np.float64)
+    out = np.zeros_like(B)
+    lib().shwfs_oracle_add_noise(B, B.shape[0], float(F), float(ron), int(seed), int(t), int(i), out)
+    return out
+
+
+def measure_lgs(phase, amplitude, valid_yx, n, P, b, dx, *, weight, defocus, tilt_x=None, tilt_y=None,
+                cx=0.0, cy=0.0, c_phi=1.0, tau=0.0, mode=0, kernels=None, flux=0.0, ron=0.0, seed=0,
+                stage=-1, nthreads=0):
+    """L1..L6 for every frame and valid subaperture.
+
+    phase [T,L,N,N] fp32, or [T,N,N] shared by the L = len(weight) sub-layers.  weight, defocus [rad/m^2],
+    tilt_x, tilt_y [rad/m]: per sub-layer; (cx, cy) [m] centre of the quadratic.  flux = F (<= 0: no noise).
+    Returns slopes [T,nsub,2] float64, or (slopes, images[T,nsub,D,D]) for stage 2 (before noise) / 3 (after).
+    """
+    ph = _c(phase, np.float32)
+    w = _c(weight, np.float64)
+    L = w.shape[0]
+    shared = ph.ndim == 3
+    if shared:
+        T, N, _ = ph.shape
+    else:
+        T, L2, N, _ = ph.shape
+        assert L2 == L
+    am = _c(amplitude, np.float32)
+    yx = _c(valid_yx, np.int32)
+    nsub = yx.shape[0]
+    de = _c(defocus, np.float64)
+    tx = _c(tilt_x if tilt_x is not None else np.zeros(L), np.float64)
+    ty = _c(tilt_y if tilt_y is not None else np.zeros(L), np.float64)
+    assert de.shape == (L,) and tx.shape == (L,) and ty.shape == (L,)
+    slopes = np.zeros((T, nsub, 2), dtype=np.float64)
+    kptr = None
+    if kernels is not None:
+        kernels = _c(kernels, np.float32)
+        assert kernels.shape == (nsub, P, P), kernels.shape
+        kptr = kernels.ctypes.data_as(C.c_void_p)
+    images, iptr = None, None
+    if stage >= 0:
+        D = P // b
+        images = np.zeros((T, nsub, D, D), dtype=np.float64)
+        iptr = images.ctypes.data_as(C.c_void_p)
+    rc = lib().shwfs_oracle_measure_lgs(ph, T, L, int(shared), N, n, P, b, am, yx, nsub, float(c_phi), float(dx),
+                                        w, de, tx, ty, float(cx), float(cy), float(tau), int(mode), kptr,
+                                        float(flux), float(ron), int(seed), slopes, int(stage), iptr,
+                                        int(nthreads))
+    if rc:
+        raise RuntimeError(f"shwfs_oracle_measure_lgs failed with code {rc}")
     return (slopes, images) if stage >= 0 else slopes
