@@ -58,6 +58,8 @@ extern "C" {
 #define SHWFS_ALGO_PRUNED_FFT 4  /* no elongation kernels, D = 16: one input-pruned P x P FFT per spot,   */
                                  /* half-warp per spot, bin + threshold + CoG in registers             */
 
+#define SHWFS_MAX_LAYERS 8        /* sodium sub-layers per LGS ("1 to 5 typically")            */
+
 typedef struct shwfs_handle shwfs_handle;              /* opaque */
 
 typedef struct {
@@ -114,11 +116,54 @@ int shwfs_get_algorithm(const shwfs_handle *h, int32_t *algo);
 /* Number of kernels this handle has launched since shwfs_create (bench.py's gpu_launches). */
 int shwfs_launch_count(const shwfs_handle *h, int64_t *count);
 
+/* ---- the paper's full LGS model ------------------------
+ * "In the code a laser guide star WF is the results of different, 1 to 5 typically, projections of the beam
+ *  on as many sub-layers of the sodium layer [...] For each sub-layer the proper phase shift in Tip Tilt and
+ *  Defocus is considered and the spot array multiplied by the corresponding value of the sodium thickness
+ *  level profile. [...] Finally the sub-layer arrays are piled-up and the centroid computed on the final
+ *  noise-added image to retrieve the slopes."
+ * With a sodium model set, H2..H4 run once per sub-layer l on the pupil phase
+ *      phase_to_rad * phase_l(r) + defocus[l] * |r - r_c|^2 + tilt[l] . r        (r = pixel centre, metres
+ *      from the pupil centre, x = (column + 1/2 - N/2) * dx),
+ * the intensities are summed with weights weight[l] >= 0, then H5 (one Gaussian per subaperture), H6, the
+ * optional noise, H7 and H8 follow.  A source at altitude h_l seen by a sensor conjugated to h_0 from a
+ * launch telescope at r_c has defocus[l] = (pi / lambda) (1/h_0 - 1/h_l).  Requires the lag-domain
+ * algorithm (EUNSUPPORTED if the handle's sizes have no such instance); selects it if needed.          */
+typedef struct {
+  int32_t n_layers;         /* L in [1, SHWFS_MAX_LAYERS]                                             */
+  int32_t shared_phase;     /* 0: shwfs_measure reads phase as [T,L,N,N]; 1: [T,N,N] shared by all l  */
+  const float *weight;      /* HOST [L] sodium profile value w_l >= 0, used as given                  */
+  const float *defocus;     /* HOST [L] a_l, rad / m^2                                                */
+  const float *tilt_x;      /* HOST [L] rad / m, or NULL for zeros (uplink tip-tilt)                  */
+  const float *tilt_y;      /* HOST [L] rad / m, or NULL                                              */
+  float centre_x_m;         /* r_c: centre of the quadratic (launch telescope), metres from the       */
+  float centre_y_m;         /*      pupil centre                                                      */
+} shwfs_sodium;
+/* s == NULL returns to the single-layer sensor.  Arrays are copied.  Errors: EINVAL, EUNSUPPORTED, ENOMEM. */
+int shwfs_set_sodium(shwfs_handle *h, const shwfs_sodium *s);
+
+/* Detector noise on the binned image B before H7 (reading B4):
+ *      counts = flux * B + sqrt(max(flux * B, 0) + read_noise^2) * z,   z ~ N(0,1)
+ * (photon noise in its Gaussian limit plus read noise), z from Philox4x32-10 with key = seed and counter =
+ * (p/4, i, first_frame + t, 0), p = C*D + R the column-major pixel index, Box-Muller on the output pairs
+ * (csrc/noise.cuh).  flux = photo-electrons per unit of B (a fully lit subaperture of unit amplitude and
+ * unit weights has sum B = n^2 sum K).  nz == NULL or flux <= 0 switches the noise off.  first_frame lets
+ * successive calls continue one noise stream.  Requires the lag-domain algorithm, as shwfs_set_sodium.   */
+typedef struct {
+  float    flux;
+  float    read_noise;      /* electrons rms, >= 0 */
+  uint64_t seed;
+  uint32_t first_frame;
+} shwfs_noise;
+int shwfs_set_noise(shwfs_handle *h, const shwfs_noise *nz);
+
 /* ---- debug (parity on images; not on the timed path) ------------------------------------------- */
 /* stage 0: centred intensity  roll(I)  DEVICE out [T*nsub*P*P]
  * stage 1: centred image after elongation  Sh  [T*nsub*P*P]  (== stage 0 without kernels)
  * stage 2: binned image B  [T*nsub*D*D], D = P/b -- produced by the handle's CURRENT algorithm, so it
- *          is the image the timed path thresholds; stages 0 and 1 exist only in the literal chain.   */
+ *          is the image the timed path thresholds; stages 0 and 1 exist only in the literal chain
+ *          (single-layer sensor only).
+ * stage 3: binned image after the detector noise  [T*nsub*D*D]  (== stage 2 when the noise is off).   */
 int shwfs_debug_spots(shwfs_handle *h, const float *phase_dev, int32_t T, int32_t stage,
                       float *out_dev, void *cuda_stream);
 

@@ -4,7 +4,7 @@
  *
  * TEST INFRASTRUCTURE, NOT PRODUCT (same rules as shwfs_oracle.c, whose stage functions it calls:
  * only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may build,
- * load or call it; nothing is shared with paper_1408_0698_b200/csrc/).
+ * load or call it; nothing is shared with the CUDA library).
  *
  * Passage followed, PAPER.md:91 (section 4, "LGS Shack Hartmann wavefront sensor"), in its order:
  *   "We divided the sodium layer into different sub-layers.  The LGS wavefront sensor module has as input

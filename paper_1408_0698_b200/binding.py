@@ -25,7 +25,8 @@ ALGO_AUTO, ALGO_LITERAL, ALGO_WK, ALGO_WK_GENERIC, ALGO_PRUNED_FFT = 0, 1, 2, 3,
 EXPORTS = ["shwfs_create", "shwfs_measure", "shwfs_measure_host", "shwfs_destroy", "shwfs_num_subaps",
            "shwfs_valid_list", "shwfs_pixel_scale", "shwfs_set_algorithm", "shwfs_get_algorithm",
            "shwfs_launch_count", "shwfs_debug_spots", "shwfs_strerror", "shwfs_last_cuda_error",
-           "shwfs_version"]
+           "shwfs_version", "shwfs_set_sodium", "shwfs_set_noise"]
+SHWFS_MAX_LAYERS = 8
 
 
 class ShwfsGeometry(C.Structure):
@@ -34,6 +35,18 @@ class ShwfsGeometry(C.Structure):
                 ("pixel_size_m", C.c_float), ("amplitude", C.POINTER(C.c_float)), ("min_illum", C.c_float),
                 ("valid_yx", C.POINTER(C.c_int32)), ("n_valid", C.c_int32), ("threshold_frac", C.c_float),
                 ("threshold_mode", C.c_int32), ("phase_to_rad", C.c_float)]
+
+
+class ShwfsSodium(C.Structure):
+    """struct shwfs_sodium of include/shwfs.h."""
+    _fields_ = [("n_layers", C.c_int32), ("shared_phase", C.c_int32), ("weight", C.POINTER(C.c_float)),
+                ("defocus", C.POINTER(C.c_float)), ("tilt_x", C.POINTER(C.c_float)),
+                ("tilt_y", C.POINTER(C.c_float)), ("centre_x_m", C.c_float), ("centre_y_m", C.c_float)]
+
+
+class ShwfsNoise(C.Structure):
+    """struct shwfs_noise of include/shwfs.h."""
+    _fields_ = [("flux", C.c_float), ("read_noise", C.c_float), ("seed", C.c_uint64), ("first_frame", C.c_uint32)]
 
 
 class ShwfsError(RuntimeError):
@@ -71,6 +84,8 @@ def load():
     L.shwfs_last_cuda_error.argtypes = []
     L.shwfs_last_cuda_error.restype = C.c_char_p
     L.shwfs_version.argtypes = []
+    L.shwfs_set_sodium.argtypes = [vp, C.POINTER(ShwfsSodium)]
+    L.shwfs_set_noise.argtypes = [vp, C.POINTER(ShwfsNoise)]
     for name in EXPORTS:
         if name not in ("shwfs_strerror", "shwfs_last_cuda_error"):
             getattr(L, name).restype = C.c_int
@@ -187,12 +202,47 @@ class Shwfs:
         _check(load().shwfs_launch_count(self._h, C.byref(v)), "shwfs_launch_count")
         return v.value
 
+    # -- the paper's full LGS model (include/shwfs.h: shwfs_set_sodium, shwfs_set_noise)
+    def set_sodium(self, weight=None, defocus=None, tilt_x=None, tilt_y=None, centre=(0.0, 0.0),
+                   shared_phase: bool = False):
+        """Sodium sub-layers: weight[L], defocus[L] rad/m^2, tilt_x/tilt_y[L] rad/m, centre (x,y) in metres.
+        weight=None returns to the single-layer sensor.  With shared_phase=False, measure() takes
+        phase [T,L,N,N]."""
+        if weight is None:
+            _check(load().shwfs_set_sodium(self._h, None), "shwfs_set_sodium")
+            self._layers = 1
+            return
+        f = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+        w, d = f(weight), f(defocus)
+        sd = ShwfsSodium()
+        sd.n_layers, sd.shared_phase = w.shape[0], int(bool(shared_phase))
+        fp = C.POINTER(C.c_float)
+        sd.weight, sd.defocus = w.ctypes.data_as(fp), d.ctypes.data_as(fp)
+        keep = [w, d]
+        for name, arr in (("tilt_x", tilt_x), ("tilt_y", tilt_y)):
+            if arr is not None:
+                a = f(arr)
+                keep.append(a)
+                setattr(sd, name, a.ctypes.data_as(fp))
+        if d.shape != w.shape or any(a.shape != w.shape for a in keep):
+            raise ValueError("weight, defocus, tilt_x, tilt_y must have the same length L")
+        sd.centre_x_m, sd.centre_y_m = float(centre[0]), float(centre[1])
+        _check(load().shwfs_set_sodium(self._h, C.byref(sd)), "shwfs_set_sodium")
+        self._layers = 1 if shared_phase else int(w.shape[0])
+
+    def set_noise(self, flux: float = 0.0, read_noise: float = 0.0, seed: int = 0, first_frame: int = 0):
+        """Detector noise before the centroid (flux <= 0 switches it off)."""
+        nz = ShwfsNoise(float(flux), float(read_noise), int(seed), int(first_frame))
+        _check(load().shwfs_set_noise(self._h, C.byref(nz)), "shwfs_set_noise")
+
     # -- the hot path
     def _check_phase(self, phase):
         import torch
+        L = getattr(self, "_layers", 1)
+        shape = (self.N, self.N) if L == 1 else (L, self.N, self.N)
         if not (isinstance(phase, torch.Tensor) and phase.is_cuda and phase.dtype == torch.float32
-                and phase.is_contiguous() and phase.dim() == 3 and phase.shape[1] == self.N and phase.shape[2] == self.N):
-            raise ValueError(f"phase must be a contiguous float32 CUDA tensor [T,{self.N},{self.N}]")
+                and phase.is_contiguous() and tuple(phase.shape[1:]) == shape):
+            raise ValueError(f"phase must be a contiguous float32 CUDA tensor [T,{','.join(map(str, shape))}]")
 
     def measure(self, phase, out=None, stream=None):
         """phase: CUDA float32 [T,N,N] -> slopes CUDA float32 [T,nsub,2] (enqueued on `stream`)."""
@@ -224,17 +274,20 @@ class Shwfs:
             if out is None:
                 out = np.empty((T, self.nsub, 2), dtype=np.float32)
             optr = out.ctypes.data
-        if tuple(phase_host.shape[1:]) != (self.N, self.N):
-            raise ValueError(f"phase_host must be [T,{self.N},{self.N}]")
+        L = getattr(self, "_layers", 1)
+        shape = (self.N, self.N) if L == 1 else (L, self.N, self.N)
+        if tuple(phase_host.shape[1:]) != shape:
+            raise ValueError(f"phase_host must be [T,{','.join(map(str, shape))}]")
         shwfs_measure_host(self._h, ptr, T, optr)
         return out
 
     def debug_spots(self, phase, stage: int, stream=None):
-        """Images of stage 0 / 1 ([T,nsub,P,P]) or 2 ([T,nsub,D,D]) as a CUDA tensor (parity only)."""
+        """Images of stage 0 / 1 ([T,nsub,P,P]) or 2 / 3 ([T,nsub,D,D]; 3 = after the detector noise) as a
+        CUDA tensor (parity only)."""
         import torch
         self._check_phase(phase)
         T = phase.shape[0]
-        side = self.D if stage == 2 else self.P
+        side = self.D if stage >= 2 else self.P
         out = torch.empty((T, self.nsub, side, side), dtype=torch.float32, device=phase.device)
         st = (stream if stream is not None else torch.cuda.current_stream(phase.device)).cuda_stream
         shwfs_debug_spots(self._h, phase.data_ptr(), T, stage, out.data_ptr(), st)
@@ -266,7 +319,7 @@ def from_config(cfg, wfs: int = 0, *, kernels="auto", **overrides) -> "Shwfs":
     kw = dict(min_illum=cfg.min_illum, threshold_frac=cfg.tau)
     kw.update(overrides)
     k = None
-    if kernels == "auto" and cfg.elong_max_arcsec > 0:
+    if isinstance(kernels, str) and kernels == "auto" and cfg.elong_max_arcsec > 0:
         import torch
         with Shwfs(amp, cfg.S, cfg.n, cfg.dx, W.LAMBDA_M, cfg.P, cfg.b, **kw) as probe:
             yx = probe.valid_yx            # the library's own H0 valid list (no kernels needed for it)

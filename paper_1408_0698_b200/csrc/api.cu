@@ -38,6 +38,7 @@ void free_handle(shwfs_handle *h)
     cudaFree(h->d_kernels);
     cudaFree(h->d_wk_table);
     cudaFree(h->d_khat);
+    cudaFree(h->d_sod_g);
     for (int k = 0; k < 2; ++k) {
         if (h->h_pin[k]) cudaFreeHost(h->h_pin[k]);
         cudaFree(h->d_phase[k]);
@@ -246,23 +247,107 @@ int shwfs_launch_count(const shwfs_handle *h, int64_t *count)
     return SHWFS_OK;
 }
 
+int shwfs_set_sodium(shwfs_handle *h, const shwfs_sodium *sd)
+{
+    if (!h) return SHWFS_EINVAL;
+    if (!sd) { h->sod_L = 0; h->sod_shared = 0; return SHWFS_OK; }
+    const int L = sd->n_layers;
+    if (L < 1 || L > SHWFS_MAX_LAYERS || !sd->weight || !sd->defocus) return SHWFS_EINVAL;
+    if (!isfinite(sd->centre_x_m) || !isfinite(sd->centre_y_m)) return SHWFS_EINVAL;
+    for (int l = 0; l < L; ++l) {
+        if (!(sd->weight[l] >= 0.f) || !isfinite(sd->weight[l]) || !isfinite(sd->defocus[l])) return SHWFS_EINVAL;
+        if ((sd->tilt_x && !isfinite(sd->tilt_x[l])) || (sd->tilt_y && !isfinite(sd->tilt_y[l]))) return SHWFS_EINVAL;
+    }
+    if (!shwfs_wk_supported(h, 0) && !shwfs_wk_supported(h, 1)) return SHWFS_EUNSUPPORTED;
+    /* reading B1, expanded about each subaperture centre r_i (float64 on the host): over the patch the
+     * sub-layer's analytic phase is piston + (2 a (r_i - r_c) + g) . d + a |d|^2, d = offset from r_i.   */
+    const size_t cnt = (size_t)L * h->nsub;
+    float2 *g = (float2 *)malloc(sizeof(float2) * cnt);
+    if (!g) return SHWFS_ENOMEM;
+    const double two_pi = 6.283185307179586476925286766559, dx = (double)h->dx;
+    for (int l = 0; l < L; ++l) {
+        const double a = (double)sd->defocus[l];
+        const double tx = sd->tilt_x ? (double)sd->tilt_x[l] : 0.0, ty = sd->tilt_y ? (double)sd->tilt_y[l] : 0.0;
+        for (int i = 0; i < h->nsub; ++i) {
+            const double yc = (((double)h->h_valid[2 * i] + 0.5) * h->n - 0.5 * h->N) * dx;
+            const double xc = (((double)h->h_valid[2 * i + 1] + 0.5) * h->n - 0.5 * h->N) * dx;
+            double gx = (2.0 * a * (xc - (double)sd->centre_x_m) + tx) * dx / two_pi;
+            double gy = (2.0 * a * (yc - (double)sd->centre_y_m) + ty) * dx / two_pi;
+            /* whole turns per pixel alias to a piston on the half-integer pixel offsets: drop them */
+            gx -= nearbyint(gx); gy -= nearbyint(gy);
+            g[(size_t)l * h->nsub + i] = make_float2((float)gx, (float)gy);
+        }
+    }
+    int rc = SHWFS_OK;
+    int prev = -1;
+    cudaGetDevice(&prev);
+    if (prev != h->device) cudaSetDevice(h->device);
+    float2 *d_new = nullptr;
+    cudaError_t e = cudaMalloc(&d_new, sizeof(float2) * cnt);
+    if (e == cudaSuccess) e = cudaMemcpy(d_new, g, sizeof(float2) * cnt, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        shwfs_note_cuda_error(e, "shwfs_set_sodium");
+        cudaFree(d_new);
+        rc = (e == cudaErrorMemoryAllocation) ? SHWFS_ENOMEM : SHWFS_ECUDA;
+    } else {
+        cudaDeviceSynchronize();                 /* nothing in flight may still read the old table */
+        cudaFree(h->d_sod_g);
+        h->d_sod_g = d_new;
+        h->sod_L = L; h->sod_shared = sd->shared_phase != 0;
+        for (int l = 0; l < SHWFS_MAX_LAYERS; ++l) {
+            h->sod_q[l] = l < L ? (float)((double)sd->defocus[l] * dx * dx / two_pi) : 0.f;
+            h->sod_sw[l] = l < L ? (float)sqrt((double)sd->weight[l]) : 0.f;
+        }
+    }
+    if (prev >= 0 && prev != h->device) cudaSetDevice(prev);
+    free(g);
+    return rc;
+}
+
+int shwfs_set_noise(shwfs_handle *h, const shwfs_noise *nz)
+{
+    if (!h) return SHWFS_EINVAL;
+    if (!nz || !(nz->flux > 0.f)) { h->nz_flux = 0.f; return SHWFS_OK; }
+    if (!isfinite(nz->flux) || !(nz->read_noise >= 0.f) || !isfinite(nz->read_noise)) return SHWFS_EINVAL;
+    if (!shwfs_wk_supported(h, 0) && !shwfs_wk_supported(h, 1)) return SHWFS_EUNSUPPORTED;
+    h->nz_flux = nz->flux; h->nz_ron = nz->read_noise; h->nz_seed = nz->seed; h->nz_first_frame = nz->first_frame;
+    return SHWFS_OK;
+}
+
+static bool ext_on(const shwfs_handle *h) { return h->sod_L > 0 || h->nz_flux > 0.f; }
+
+/* frames of phase per time step t: L when every sub-layer has its own wavefront */
+static int frames_per_step(const shwfs_handle *h) { return (h->sod_L > 0 && !h->sod_shared) ? h->sod_L : 1; }
+
 static int run_path(shwfs_handle *h, const float *phase_dev, int T, float *slopes_dev, int stage, float *img,
-                    cudaStream_t st)
+                    unsigned t_base, cudaStream_t st)
 {
     if ((long long)T * h->nsub > 0x7fffffffLL / 2) return SHWFS_EINVAL;
     cudaError_t e;
-    if (stage == 0 || stage == 1) {
+    if (stage == 3 && !(h->nz_flux > 0.f)) stage = 2;      /* no noise: the final image is the binned one */
+    if (ext_on(h)) {
+        /* sub-layers / noise live in the lag-domain kernels only (shwfs_set_sodium made sure one exists) */
+        if (stage == 0 || stage == 1) return SHWFS_EUNSUPPORTED;
+        const int generic = (h->algo == SHWFS_ALGO_WK_GENERIC) || !shwfs_wk_supported(h, 0);
+        e = shwfs_wk_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr, stage == 3 ? img : nullptr,
+                            t_base, generic, st);
+    } else if (stage == 0 || stage == 1) {
         int rc = ensure_khat(h);
         if (rc) return rc;
         if (!shwfs_literal_supported(h)) return SHWFS_EUNSUPPORTED;
         e = shwfs_literal_launch(h, phase_dev, T, slopes_dev, stage, img, st);
     } else if (h->algo == SHWFS_ALGO_LITERAL) {
-        e = shwfs_literal_launch(h, phase_dev, T, slopes_dev, stage, img, st);
+        e = shwfs_literal_launch(h, phase_dev, T, slopes_dev, stage == 3 ? 2 : stage, img, st);
     } else if (h->algo == SHWFS_ALGO_PRUNED_FFT) {
-        e = shwfs_pruned_fft_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr, st);
+        e = shwfs_pruned_fft_launch(h, phase_dev, T, slopes_dev, (stage == 2 || stage == 3) ? img : nullptr, st);
     } else {
-        e = shwfs_wk_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr,
-                            h->algo == SHWFS_ALGO_WK_GENERIC, st);
+        if (stage == 3) stage = 2;
+        if (h->algo == SHWFS_ALGO_PRUNED_FFT) {
+            e = shwfs_pruned_fft_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr, st);
+        } else {
+            e = shwfs_wk_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr, nullptr, t_base,
+                                h->algo == SHWFS_ALGO_WK_GENERIC, st);
+        }
     }
     if (e != cudaSuccess) { shwfs_note_cuda_error(e, "kernel launch"); return SHWFS_ECUDA; }
     return SHWFS_OK;
@@ -273,13 +358,13 @@ int shwfs_measure(shwfs_handle *h, const float *phase_dev, int32_t T, float *slo
     if (!h || T < 0) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
     if (!phase_dev || !slopes_dev) return SHWFS_EINVAL;
-    return run_path(h, phase_dev, T, slopes_dev, -1, nullptr, (cudaStream_t)cuda_stream);
+    return run_path(h, phase_dev, T, slopes_dev, -1, nullptr, 0u, (cudaStream_t)cuda_stream);
 }
 
 int shwfs_debug_spots(shwfs_handle *h, const float *phase_dev, int32_t T, int32_t stage, float *out_dev,
                       void *cuda_stream)
 {
-    if (!h || T < 0 || stage < 0 || stage > 2) return SHWFS_EINVAL;
+    if (!h || T < 0 || stage < 0 || stage > 3) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
     if (!phase_dev || !out_dev) return SHWFS_EINVAL;
     /* the debug path needs somewhere to put the slopes it also computes */
@@ -291,7 +376,7 @@ int shwfs_debug_spots(shwfs_handle *h, const float *phase_dev, int32_t T, int32_
         if (e != cudaSuccess) { shwfs_note_cuda_error(e, "cudaMalloc(debug slopes)"); return SHWFS_ENOMEM; }
         h->d_slopes_cap = need;
     }
-    return run_path(h, phase_dev, T, h->d_slopes, stage, out_dev, (cudaStream_t)cuda_stream);
+    return run_path(h, phase_dev, T, h->d_slopes, stage, out_dev, 0u, (cudaStream_t)cuda_stream);
 }
 
 }  // extern "C"
@@ -308,9 +393,11 @@ int host_init(shwfs_handle *h)
 {
     if (h->host_ready) return SHWFS_OK;
     int rc = SHWFS_OK;
+    /* one "frame" of the pipeline = one time step = up to SHWFS_MAX_LAYERS wavefronts, so that a later
+     * shwfs_set_sodium never outgrows the buffers */
     const size_t frame_bytes = sizeof(float) * (size_t)h->N * h->N;
     size_t chunk = ((size_t)64 << 20) / frame_bytes;
-    if (chunk < 1) chunk = 1;
+    if (chunk < SHWFS_MAX_LAYERS) chunk = SHWFS_MAX_LAYERS;
     if (chunk > 256) chunk = 256;
     h->chunk_frames = (int)chunk;
     CU_TRY(cudaStreamCreateWithFlags(&h->st_copy, cudaStreamNonBlocking), "cudaStreamCreate");
@@ -348,7 +435,9 @@ extern "C" int shwfs_measure_host(shwfs_handle *h, const float *phase_host, int3
     {
         rc = host_init(h);
         if (rc) goto fail;
-        const size_t frame_elems = (size_t)h->N * h->N, frame_bytes = sizeof(float) * frame_elems;
+        const int fps = frames_per_step(h);
+        const int chunk_steps = h->chunk_frames / fps;          /* >= 1: chunk_frames >= SHWFS_MAX_LAYERS */
+        const size_t frame_elems = (size_t)h->N * h->N * fps, frame_bytes = sizeof(float) * frame_elems;
         const size_t n_slopes = 2 * (size_t)T * h->nsub;
         if (h->d_slopes_cap < n_slopes) {
             cudaStreamSynchronize(h->st_comp);
@@ -359,11 +448,11 @@ extern "C" int shwfs_measure_host(shwfs_handle *h, const float *phase_host, int3
         const bool pinned_in = is_pinned(phase_host);
         if (!pinned_in)
             for (int k = 0; k < 2; ++k)
-                if (!h->h_pin[k]) CU_TRY(cudaHostAlloc(&h->h_pin[k], frame_bytes * h->chunk_frames, cudaHostAllocDefault), "cudaHostAlloc");
+                if (!h->h_pin[k]) CU_TRY(cudaHostAlloc(&h->h_pin[k], sizeof(float) * (size_t)h->N * h->N * h->chunk_frames, cudaHostAllocDefault), "cudaHostAlloc");
         int c = 0;
-        for (int t0 = 0; t0 < T; t0 += h->chunk_frames, ++c) {
+        for (int t0 = 0; t0 < T; t0 += chunk_steps, ++c) {
             const int k = c & 1;
-            const int tc = (T - t0 < h->chunk_frames) ? T - t0 : h->chunk_frames;
+            const int tc = (T - t0 < chunk_steps) ? T - t0 : chunk_steps;
             const float *src = phase_host + (size_t)t0 * frame_elems;
             if (!pinned_in) {
                 CU_TRY(cudaEventSynchronize(h->ev_h2d[k]), "cudaEventSynchronize");   /* staging buffer free again */
@@ -374,7 +463,7 @@ extern "C" int shwfs_measure_host(shwfs_handle *h, const float *phase_host, int3
             CU_TRY(cudaMemcpyAsync(h->d_phase[k], src, frame_bytes * tc, cudaMemcpyHostToDevice, h->st_copy), "cudaMemcpyAsync(H2D)");
             CU_TRY(cudaEventRecord(h->ev_h2d[k], h->st_copy), "cudaEventRecord");
             CU_TRY(cudaStreamWaitEvent(h->st_comp, h->ev_h2d[k], 0), "cudaStreamWaitEvent");
-            rc = run_path(h, h->d_phase[k], tc, h->d_slopes + 2 * (size_t)t0 * h->nsub, -1, nullptr, h->st_comp);
+            rc = run_path(h, h->d_phase[k], tc, h->d_slopes + 2 * (size_t)t0 * h->nsub, -1, nullptr, (unsigned)t0, h->st_comp);
             if (rc) goto fail;
             CU_TRY(cudaEventRecord(h->ev_done[k], h->st_comp), "cudaEventRecord");
         }

@@ -32,6 +32,15 @@ struct shwfs_handle {
     int     wk_table_stride; /* elements between subapertures: n*(2n-1), or 0 when shared      */
     float2 *d_khat;        /* literal chain: DFT of the re-centred kernel, [nsub][P][P]; lazy  */
 
+    /* paper's full LGS model (shwfs_set_sodium / shwfs_set_noise); sod_L == 0: plain single-layer sensor */
+    int     sod_L, sod_shared;
+    float   sod_q[SHWFS_MAX_LAYERS];    /* a_l dx^2 / 2pi, turns/pixel^2 */
+    float   sod_sw[SHWFS_MAX_LAYERS];   /* sqrt(w_l) */
+    float2 *d_sod_g;                    /* [L][nsub] (2 a_l (r_i - r_c) + g_l) dx / 2pi, turns/pixel */
+    float   nz_flux, nz_ron;
+    uint64_t nz_seed;
+    uint32_t nz_first_frame;
+
     /* host copies for queries */
     int32_t *h_valid;      /* [nsub*2] (sy,sx) */
 
@@ -54,7 +63,8 @@ cudaError_t shwfs_wk_build_table(shwfs_handle *h, cudaStream_t st);
 
 /* Wiener-Khinchin path: slopes (and optionally the binned image B, [T*nsub*D*D]) */
 cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *slopes,
-                            float *binned_or_null, int generic, cudaStream_t st);
+                            float *binned_or_null, float *noisy_or_null, unsigned t_base, int generic,
+                            cudaStream_t st);
 int shwfs_wk_supported(const shwfs_handle *h, int generic);
 
 /* Literal chain: P x P FFT(s) in shared memory/registers.  stage < 0: slopes only.

@@ -23,6 +23,7 @@
 #include "fft_regs.cuh"
 #include "field.cuh"
 #include "cog.cuh"
+#include "noise.cuh"
 
 namespace {
 
@@ -129,6 +130,16 @@ struct WkArgs {
     long long frame_stride;
     int T, N, nsub, mstride, total, mode;
     float tau, turns, ramp_unit;
+    /* paper's full LGS model (EXT instances only): sodium sub-layers and detector noise */
+    const float2 *sod_g;         /* [L][nsub] local gradient of the sub-layer's analytic phase, turns/pixel */
+    float *noisy;                /* stage-3 debug image (binned, after noise) or null                       */
+    long long layer_stride;      /* elements between sub-layers of one frame (0: shared wavefront)          */
+    int L;
+    float sod_q[SHWFS_MAX_LAYERS];   /* curvature a_l dx^2 / 2pi, turns/pixel^2                             */
+    float sod_sw[SHWFS_MAX_LAYERS];  /* sqrt(w_l): folded into the amplitude                                */
+    float flux, ron2;
+    uint2 key;
+    unsigned t0;
 };
 
 template <int n>
@@ -217,7 +228,7 @@ __device__ __forceinline__ void rowself_acc(const float *__restrict__ p, LagAcc<
 /* S = G * M aliased onto lx mod 16, 16-point x-transform, H[ly][0..15] -> shared memory */
 template <int n>
 __device__ __forceinline__ void finish_row(const float2 (&acc)[2 * n - 1], const float2 *__restrict__ Mrow,
-                                           float *__restrict__ hrow)
+                                           float *__restrict__ hrow, bool accumulate = false)
 {
     float sr[16], si[16];
 #pragma unroll
@@ -245,11 +256,16 @@ __device__ __forceinline__ void finish_row(const float2 (&acc)[2 * n - 1], const
 #pragma unroll
     for (int C = 0; C < 16; C += 2) {
         const int p0 = fft_out_index<16>(C), p1 = fft_out_index<16>(C + 1);
-        reinterpret_cast<float4 *>(hrow)[C / 2] = make_float4(sr[p0], si[p0], sr[p1], si[p1]);
+        float4 v = make_float4(sr[p0], si[p0], sr[p1], si[p1]);
+        if (accumulate) {                        /* sub-layer arrays are piled up (linear up to H) */
+            const float4 o = reinterpret_cast<float4 *>(hrow)[C / 2];
+            v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w;
+        }
+        reinterpret_cast<float4 *>(hrow)[C / 2] = v;
     }
 }
 
-template <int n, int MODE>
+template <int n, int MODE, bool EXT>
 __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_measure_kernel(const WkArgs A)
 {
     using Cfg = WkCfg<n>;
@@ -274,6 +290,10 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
     }
     __syncthreads();
 
+    const int n_layers = EXT ? A.L : 1;
+#pragma unroll 1
+    for (int layer = 0; layer < n_layers; ++layer) {
+    if (EXT && layer > 0) __syncthreads();        /* every warp is done reading the previous layer's field */
     /* ---- phase 0: H1 gather + H2 field.  Thread = pixel pair q2 of the spots sg, sg+SG, ... ---- */
     {
         const int sg = tid / Cfg::NP, q2 = tid - sg * Cfg::NP;
@@ -281,6 +301,10 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
             const int j = q2 / (n / 2), kk = q2 - j * (n / 2);
             const int poff = j * A.N + 2 * kk;
             const float ramp0 = (float)(j + 2 * kk) * A.ramp_unit, ramp1 = ramp0 + A.ramp_unit;
+            /* EXT: pixel offsets from the patch centre and the sub-layer's curvature term (reading B1) */
+            const float dj = (float)j - 0.5f * (float)(n - 1), dk0 = (float)(2 * kk) - 0.5f * (float)(n - 1);
+            const float lq = EXT ? A.sod_q[layer] : 0.f, lsw = EXT ? A.sod_sw[layer] : 1.f;
+            const float quad0 = lq * (dj * dj + dk0 * dk0), quad1 = lq * (dj * dj + (dk0 + 1.f) * (dk0 + 1.f));
             float2 ph[Cfg::ITEMS];
             int aoff[Cfg::ITEMS];
 #pragma unroll
@@ -292,7 +316,8 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
                     const int4 inf = s_info[s];
                     if (inf.z >= 0) {
                         aoff[r] = inf.x + poff;
-                        ph[r] = __ldg(reinterpret_cast<const float2 *>(A.phase + (size_t)inf.y * A.frame_stride + aoff[r]));
+                        ph[r] = __ldg(reinterpret_cast<const float2 *>(A.phase + (size_t)inf.y * A.frame_stride
+                                                                       + (EXT ? (size_t)layer * A.layer_stride : 0) + aoff[r]));
                     }
                 }
             }
@@ -308,8 +333,16 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
                             acur = aoff[r];
                             am = __ldg(reinterpret_cast<const float2 *>(A.amp + acur));
                         }
-                        const float2 e0 = field_value(ph[r].x, am.x, A.turns, ramp0);
-                        const float2 e1 = field_value(ph[r].y, am.y, A.turns, ramp1);
+                        float2 e0, e1;
+                        if (EXT) {
+                            const float2 g = __ldg(A.sod_g + (size_t)layer * A.nsub + s_info[s].z);
+                            const float lin = fmaf(g.x, dk0, g.y * dj);
+                            e0 = field_value(ph[r].x, am.x * lsw, A.turns, ramp0 - (lin + quad0));
+                            e1 = field_value(ph[r].y, am.y * lsw, A.turns, ramp1 - (lin + g.x + quad1));
+                        } else {
+                            e0 = field_value(ph[r].x, am.x, A.turns, ramp0);
+                            e1 = field_value(ph[r].y, am.y, A.turns, ramp1);
+                        }
                         e = make_float4(e0.x, e0.y, e1.x, e1.y);
                     }
                     reinterpret_cast<float4 *>(ebuf + s * Cfg::ES)[q2] = e;
@@ -350,9 +383,10 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
 #pragma unroll
                 for (int a = 0; a < Cfg::LX; ++a) acc[a] = L.lag_value(a);
             }
-            finish_row<n>(acc, Mi + ly * Cfg::LX, hb + ly * 32);
+            finish_row<n>(acc, Mi + ly * Cfg::LX, hb + ly * 32, EXT && layer > 0);
         }
     }
+    }   /* sub-layers */
     __syncthreads();
 
     /* ---- phase 2: y-transform (real part), threshold, centre of gravity ---- */
@@ -372,16 +406,21 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
             float bcol[16];
 #pragma unroll
             for (int R = 0; R < 16; ++R) bcol[R] = yr[fft_out_index<16>(R)];
-            const float2 sl = cog16<MODE>(bcol, C, A.tau);
             const int4 inf = s_info[s];
-            if (inf.z >= 0) {
-                const size_t o = (size_t)inf.y * A.nsub + inf.z;
-                if (C == 0) reinterpret_cast<float2 *>(A.slopes)[o] = sl;
-                if (A.binned) {
+            const size_t o = (size_t)inf.y * A.nsub + max(inf.z, 0);
+            if (inf.z >= 0 && A.binned) {
 #pragma unroll
-                    for (int R = 0; R < 16; ++R) A.binned[(o * 16 + R) * 16 + C] = bcol[R];
+                for (int R = 0; R < 16; ++R) A.binned[(o * 16 + R) * 16 + C] = bcol[R];
+            }
+            if (EXT && A.flux > 0.f) {
+                add_noise_col16(bcol, C, A.key, A.t0 + (unsigned)inf.y, (unsigned)max(inf.z, 0), A.flux, A.ron2);
+                if (inf.z >= 0 && A.noisy) {
+#pragma unroll
+                    for (int R = 0; R < 16; ++R) A.noisy[(o * 16 + R) * 16 + C] = bcol[R];
                 }
             }
+            const float2 sl = cog16<MODE>(bcol, C, A.tau);
+            if (inf.z >= 0 && C == 0) reinterpret_cast<float2 *>(A.slopes)[o] = sl;
         }
     }
 }
@@ -409,19 +448,29 @@ __global__ void __launch_bounds__(GEN_THREADS) wk_generic_kernel(const WkArgs A,
     const int2 yx = A.valid[i];
     const int off = yx.x * n * A.N + yx.y * n;
 
-    for (int q = tid; q < n * n; q += GEN_THREADS) {
-        const int j = q / n, k = q - j * n, o = off + j * A.N + k;
-        e[q] = field_value(A.phase[(size_t)t * A.frame_stride + o], A.amp[o], A.turns,
-                           (float)(j + k) * A.ramp_unit);
-    }
     for (int m = tid; m < D; m += GEN_THREADS) {
         float s, c;
         sincospif(2.f * (float)m / (float)D, &s, &c);
         tw[m] = make_float2(c, s);
     }
+    const float2 *Mi = A.M + (size_t)i * A.mstride;
+    const int n_layers = A.L > 0 ? A.L : 1;                /* A.L == 0: the plain single-layer sensor */
+    for (int layer = 0; layer < n_layers; ++layer) {
+    __syncthreads();
+    for (int q = tid; q < n * n; q += GEN_THREADS) {
+        const int j = q / n, k = q - j * n, o = off + j * A.N + k;
+        float extra = 0.f, sw = 1.f;
+        if (A.L > 0) {                                     /* sub-layer's analytic phase, turns (reading B1) */
+            const float2 g = A.sod_g[(size_t)layer * A.nsub + i];
+            const float dj = (float)j - 0.5f * (float)(n - 1), dk = (float)k - 0.5f * (float)(n - 1);
+            extra = g.x * dk + g.y * dj + A.sod_q[layer] * (dj * dj + dk * dk);
+            sw = A.sod_sw[layer];
+        }
+        e[q] = field_value(A.phase[(size_t)t * A.frame_stride + (size_t)layer * A.layer_stride + o], A.amp[o] * sw,
+                           A.turns, (float)(j + k) * A.ramp_unit - extra);
+    }
     __syncthreads();
 
-    const float2 *Mi = A.M + (size_t)i * A.mstride;
     for (int idx = tid; idx < n * LX; idx += GEN_THREADS) {
         const int ly = idx / LX, lx = idx - ly * LX - (n - 1);
         const int k_lo = lx < 0 ? -lx : 0, k_hi = lx < 0 ? n : n - lx;
@@ -433,8 +482,11 @@ __global__ void __launch_bounds__(GEN_THREADS) wk_generic_kernel(const WkArgs A,
                 gi = fmaf(u.y, v.x, fmaf(-u.x, v.y, gi));
             }
         const float2 mv = Mi[idx];
-        S[idx] = make_float2(gr * mv.x - gi * mv.y, gr * mv.y + gi * mv.x);
+        float2 sv = make_float2(gr * mv.x - gi * mv.y, gr * mv.y + gi * mv.x);
+        if (layer > 0) { sv.x += S[idx].x; sv.y += S[idx].y; }      /* sub-layer arrays piled up */
+        S[idx] = sv;
     }
+    }   /* sub-layers */
     __syncthreads();
 
     for (int px = tid; px < D * D; px += GEN_THREADS) {
@@ -450,6 +502,19 @@ __global__ void __launch_bounds__(GEN_THREADS) wk_generic_kernel(const WkArgs A,
         B[px] = acc;
     }
     __syncthreads();
+    const size_t o = (size_t)t * A.nsub + i;
+    if (A.binned)
+        for (int px = tid; px < D * D; px += GEN_THREADS) A.binned[o * D * D + px] = B[px];
+    if (A.flux > 0.f) {                                    /* detector noise, pixel p = C*D + R (noise.cuh) */
+        for (int px = tid; px < D * D; px += GEN_THREADS) {
+            const int R = px / D, C = px - R * D, p = C * D + R;
+            float z[4];
+            normal4(A.key, A.t0 + (unsigned)t, (unsigned)i, (unsigned)(p >> 2), z);
+            B[px] = noisy_count(B[px], A.flux, A.ron2, z[p & 3]);
+            if (A.noisy) A.noisy[o * D * D + px] = B[px];
+        }
+        __syncthreads();
+    }
 
     /* H7: peak */
     float mx = -INFINITY;
@@ -483,17 +548,14 @@ __global__ void __launch_bounds__(GEN_THREADS) wk_generic_kernel(const WkArgs A,
         }
         __syncthreads();
     }
-    const size_t o = (size_t)t * A.nsub + i;
     if (tid == 0) {
         const float w = red[0];
         A.slopes[2 * o] = w == 0.f ? 0.f : red[GEN_THREADS] / w;
         A.slopes[2 * o + 1] = w == 0.f ? 0.f : red[2 * GEN_THREADS] / w;
     }
-    if (A.binned)
-        for (int px = tid; px < D * D; px += GEN_THREADS) A.binned[o * D * D + px] = B[px];
 }
 
-template <int n, int MODE>
+template <int n, int MODE, bool EXT>
 cudaError_t launch_special_mode(const WkArgs &A, cudaStream_t st)
 {
     using Cfg = WkCfg<n>;
@@ -501,20 +563,22 @@ cudaError_t launch_special_mode(const WkArgs &A, cudaStream_t st)
     int dev = 0;
     cudaGetDevice(&dev);
     if (dev >= 0 && dev < 64 && !attr_set[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(wk_measure_kernel<n, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(wk_measure_kernel<n, MODE, EXT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
         attr_set[dev] = true;
     }
     const int grid = (A.total + Cfg::SPOTS - 1) / Cfg::SPOTS;
-    wk_measure_kernel<n, MODE><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(A);
+    wk_measure_kernel<n, MODE, EXT><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(A);
     return cudaGetLastError();
 }
 
 template <int n>
 cudaError_t launch_special(const WkArgs &A, cudaStream_t st)
 {
-    return A.mode == 0 ? launch_special_mode<n, 0>(A, st) : launch_special_mode<n, 1>(A, st);
+    if (A.L > 0 || A.flux > 0.f)
+        return A.mode == 0 ? launch_special_mode<n, 0, true>(A, st) : launch_special_mode<n, 1, true>(A, st);
+    return A.mode == 0 ? launch_special_mode<n, 0, false>(A, st) : launch_special_mode<n, 1, false>(A, st);
 }
 
 }  // namespace
@@ -539,12 +603,18 @@ cudaError_t shwfs_wk_build_table(shwfs_handle *h, cudaStream_t st)
 }
 
 cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *slopes, float *binned,
-                            int generic, cudaStream_t st)
+                            float *noisy, unsigned t_base, int generic, cudaStream_t st)
 {
     WkArgs A;
     A.phase = phase; A.amp = h->d_amp; A.valid = h->d_valid; A.M = h->d_wk_table;
     A.slopes = slopes; A.binned = binned;
     A.frame_stride = (long long)h->N * h->N;
+    A.sod_g = h->d_sod_g; A.noisy = noisy; A.layer_stride = 0; A.L = h->sod_L;
+    for (int l = 0; l < SHWFS_MAX_LAYERS; ++l) { A.sod_q[l] = h->sod_q[l]; A.sod_sw[l] = h->sod_sw[l]; }
+    if (h->sod_L > 0 && !h->sod_shared) { A.layer_stride = A.frame_stride; A.frame_stride *= h->sod_L; }
+    A.flux = h->nz_flux; A.ron2 = h->nz_ron * h->nz_ron;
+    A.key = make_uint2((unsigned)h->nz_seed, (unsigned)(h->nz_seed >> 32));
+    A.t0 = h->nz_first_frame + t_base;
     A.T = T; A.N = h->N; A.nsub = h->nsub; A.mstride = h->wk_table_stride;
     A.total = T * h->nsub; A.mode = h->mode;
     A.tau = h->tau;

@@ -177,6 +177,32 @@ def elongation_kernels(c: WfsConfig, wfs: int, valid_yx: np.ndarray, subset=None
     return out
 
 
+def sodium_layers(c: WfsConfig, wfs: int, L: int, h0_m: float = 90e3, fwhm_m: float = 10e3):
+    """Inputs of the paper's sub-layer model (reading B2): L equal slabs
+    spanning +-fwhm_m about the focus altitude h0_m, at their mid altitudes h_l, with a Gaussian sodium
+    profile of FWHM fwhm_m as weights (normalised to sum 1), defocus a_l = (pi/lambda)(1/h0 - 1/h_l)
+    [rad/m^2] about the launch point of WFS `wfs`, and a seeded uplink tip-tilt of 0.05 arcsec rms per
+    sub-layer [rad/m of phase gradient].  Returns a dict of float64 arrays / floats."""
+    edges = np.linspace(-fwhm_m, fwhm_m, L + 1)
+    dh = 0.5 * (edges[:-1] + edges[1:])
+    h = h0_m + dh
+    w = np.exp(-4.0 * math.log(2.0) * (dh / fwhm_m) ** 2)
+    w = w / w.sum()
+    a = (math.pi / LAMBDA_M) * (1.0 / h0_m - 1.0 / h)
+    tt = np.random.default_rng(seed_for(c.cfg, wfs, 0) + 777).normal(0.0, 0.05 * ARCSEC, (2, L))
+    cx, cy = launch_point(c, wfs)
+    return dict(weight=w, defocus=a, tilt_x=tt[0] * 2.0 * math.pi / LAMBDA_M,
+                tilt_y=tt[1] * 2.0 * math.pi / LAMBDA_M, cx=cx, cy=cy, altitude=h)
+
+
+def spot_size_kernels(c: WfsConfig, valid_yx: np.ndarray, device=None):
+    """Round Gaussian of FWHM fwhm_short_arcsec for every subaperture (the laser-spot size; with sub-layers
+    the elongation comes from the geometry).  Same evaluation as elongation_kernels."""
+    from dataclasses import replace
+    return elongation_kernels(replace(c, elong_max_arcsec=c.fwhm_short_arcsec * (1.0 + 1e-9)), 0, valid_yx,
+                              device=device)
+
+
 def phase_frames_device(c: WfsConfig, wfs: int, frames, device, out=None):
     """Same von Karman recipe as phase_screen, evaluated with torch on `device` (float64 FFT, cast to fp32).
 

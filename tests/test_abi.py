@@ -31,19 +31,22 @@ def test_library_exports_every_declared_symbol(libshwfs):
     assert b"invalid" in L.shwfs_strerror(-1)
 
 
-def test_ctypes_struct_matches_the_header(tmp_path):
-    """sizeof / offsetof of shwfs_geometry as gcc sees the header == the ctypes mirror in the binding."""
-    from paper_1408_0698_b200.binding import ShwfsGeometry
-    fields = [f[0] for f in ShwfsGeometry._fields_]
+@pytest.mark.parametrize("cname,pyname", [("shwfs_geometry", "ShwfsGeometry"), ("shwfs_sodium", "ShwfsSodium"),
+                                          ("shwfs_noise", "ShwfsNoise")])
+def test_ctypes_struct_matches_the_header(tmp_path, cname, pyname):
+    """sizeof / offsetof of each ABI struct as gcc sees the header == the ctypes mirror in the binding."""
+    from paper_1408_0698_b200 import binding
+    St = getattr(binding, pyname)
+    fields = [f[0] for f in St._fields_]
     src = tmp_path / "layout.c"
-    body = "".join(f'printf("%zu\\n", offsetof(shwfs_geometry, {f}));' for f in fields)
+    body = "".join(f'printf("%zu\\n", offsetof({cname}, {f}));' for f in fields)
     src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "shwfs.h"\n'
-                   'int main(void){printf("%zu\\n", sizeof(shwfs_geometry));' + body + "return 0;}\n")
+                   f'int main(void){{printf("%zu\\n", sizeof({cname}));' + body + "return 0;}\n")
     exe = tmp_path / "layout"
     subprocess.run(["gcc", "-std=c99", "-I", str(ROOT / "include"), str(src), "-o", str(exe)], check=True)
     out = [int(v) for v in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()]
-    assert out[0] == C.sizeof(ShwfsGeometry)
-    assert out[1:] == [getattr(ShwfsGeometry, f).offset for f in fields]
+    assert out[0] == C.sizeof(St)
+    assert out[1:] == [getattr(St, f).offset for f in fields]
 
 
 def test_header_compiles_as_c_and_cxx(tmp_path):
@@ -146,7 +149,7 @@ def test_measure_rejects_bad_arguments_and_queries(gpu):
         assert L.shwfs_measure(s._h, ph.data_ptr(), 2, None, None) == B.SHWFS_EINVAL
         assert L.shwfs_measure(s._h, ph.data_ptr(), -1, out.data_ptr(), None) == B.SHWFS_EINVAL
         assert L.shwfs_measure(s._h, None, 0, None, None) == B.SHWFS_OK
-        assert L.shwfs_debug_spots(s._h, ph.data_ptr(), 2, 3, out.data_ptr(), None) == B.SHWFS_EINVAL
+        assert L.shwfs_debug_spots(s._h, ph.data_ptr(), 2, 4, out.data_ptr(), None) == B.SHWFS_EINVAL
         assert L.shwfs_set_algorithm(s._h, 99) == B.SHWFS_EINVAL
         assert L.shwfs_num_subaps(s._h, None) == B.SHWFS_EINVAL
         assert s.nsub == 80
