@@ -98,8 +98,22 @@ class ClockSampler:
                 "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def workload_name(c):
+def f_alg(c, L):
+    """Algorithmic flops per spot.  Single layer: SURVEY.md 8(d).  With L sodium sub-layers (8(f) f1) the
+    cheapest formulation of the same result is L input-pruned first transforms (5 P log2 P (n + P) each), the
+    intensities piled up, then ONE frame-paired convolution FFT pair (10 P^2 log2 P per spot)."""
+    if L <= 0:
+        return F_ALG[c.cfg]
+    lg = int(np.log2(c.P))
+    return L * 5 * c.P * lg * (c.n + c.P) + (10 * c.P * c.P * lg if c.elong_max_arcsec > 0 else 0)
+
+
+def workload_name(c, L=0, flux=0.0):
     el = f", elongation <= {c.elong_max_arcsec:g} arcsec" if c.elong_max_arcsec > 0 else ""
+    if L > 0:
+        el = f", {L} sodium sub-layers (own wavefront each) + round {c.fwhm_short_arcsec:g} arcsec spot kernel"
+    if flux > 0:
+        el += ", photon + read noise"
     return (f"config{c.cfg} ({c.name}): {c.W} WFS x {c.S}x{c.S} subapertures of {c.n}x{c.n} px on a {c.N}x{c.N} pupil, "
             f"pad {c.P}, {c.b}x{c.b} binning, tau={c.tau:g}{el}, {c.batch}-frame batches")
 
@@ -157,10 +171,28 @@ def run_ours(args):
     c = W.CONFIGS[args.config]
     frames = c.batch
     # one handle per WFS (elongation kernels differ by launch point, reading A13), synthetic frames in HBM
-    sensors = [B.from_config(c, w) for w in range(c.W)]
-    nsub = sensors[0].nsub
+    L = args.sublayers
     my_frames = rank_frames(c.T, frames, rank, world)          # each rank owns its own batch of the stream
-    phase = [W.phase_frames_device(c, w, my_frames, dev) for w in range(c.W)]
+    if L > 0:
+        # the paper's full LGS model ("MAORY configuration and 3 sodium sub-layers"): every
+        # sub-layer has its own wavefront, the elongation comes from the geometry, the kernel is the spot size
+        with B.from_config(c, 0, kernels=None) as probe:
+            yx = probe.valid_yx
+        Ksp = W.spot_size_kernels(c, yx, device=dev)
+        sensors = [B.from_config(c, w, kernels=Ksp, valid_yx=yx) for w in range(c.W)]
+        for w, s in enumerate(sensors):
+            sod = W.sodium_layers(c, w, L)
+            s.set_sodium(sod["weight"], sod["defocus"], sod["tilt_x"], sod["tilt_y"], (sod["cx"], sod["cy"]))
+        del Ksp
+        layer_frames = [int(t) * L + l for t in my_frames for l in range(L)]
+        phase = [W.phase_frames_device(c, w, layer_frames, dev).view(frames, L, c.N, c.N) for w in range(c.W)]
+    else:
+        sensors = [B.from_config(c, w) for w in range(c.W)]
+        phase = [W.phase_frames_device(c, w, my_frames, dev) for w in range(c.W)]
+    if args.noise_flux > 0:
+        for w, s in enumerate(sensors):
+            s.set_noise(args.noise_flux / c.n ** 2, args.read_noise, 14080698 + w)
+    nsub = sensors[0].nsub
     slopes = [torch.empty((frames, nsub, 2), dtype=torch.float32, device=dev) for _ in range(c.W)]
     spots_per_step = c.W * frames * nsub
     in_bytes = sum(p.numel() * 4 for p in phase)
@@ -207,7 +239,7 @@ def run_ours(args):
 
     # ---- end to end from pinned host memory through shwfs_measure_host
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
-    h_phase = [torch.empty((frames, c.N, c.N), dtype=torch.float32, pin_memory=True) for _ in range(c.W)]
+    h_phase = [torch.empty(tuple(phase[0].shape), dtype=torch.float32, pin_memory=True) for _ in range(c.W)]
     for w in range(c.W):
         h_phase[w].copy_(phase[w])
     h_slopes = [torch.empty((frames, nsub, 2), dtype=torch.float32, pin_memory=True) for _ in range(c.W)]
@@ -225,22 +257,25 @@ def run_ours(args):
 
     if rank == 0:
         spots_per_launch = frames * nsub
-        ach = F_ALG[c.cfg] * spots_per_launch / (kern_ms * 1e-3) / 1e12
+        fa = f_alg(c, L)
+        ach = fa * spots_per_launch / (kern_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                    "frac": ach / FP32_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(c.cfg),
+                    "frac": ach / FP32_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(c.cfg) if L <= 0 and args.noise_flux <= 0 else None,
                     "kernel": {B.ALGO_WK: f"wk_measure_kernel<{c.n}>", B.ALGO_PRUNED_FFT: f"pruned_fft_kernel<{c.P}>",
                                B.ALGO_LITERAL: f"literal_kernel<{c.P}>"}.get(sensors[0].algorithm, f"algo{sensors[0].algorithm}"),
                     "kernel_ms": kern_ms, "spots_per_launch": spots_per_launch,
-                    "flops_per_spot": F_ALG[c.cfg], "flops_basis": "F_alg (SURVEY.md 8(d))",
-                    "frac_nominal_fft_flops": F_NOM[c.cfg] * spots_per_launch / (kern_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
+                    "flops_per_spot": fa, "flops_basis": "F_alg (SURVEY.md 8(d))" if L <= 0 else
+                    "L pruned first FFTs + one frame-paired convolution pair (DESIGN.md 7)",
+                    "frac_nominal_fft_flops": (F_NOM[c.cfg] * spots_per_launch / (kern_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS
+                                               if L <= 0 else None),
                     "peak_basis": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (measured FFMA chain 72.4)",
                     "hbm_frac": (in_bytes + out_bytes) / c.W / (kern_ms * 1e-3) / 1e9 / _hbm_peak()}
-        cpu = None if args.no_cpu_baseline else cpu_baseline(c, args, phase)
+        cpu = None if args.no_cpu_baseline else cpu_baseline(c, args, phase, sensors[0].valid_yx)
         out = {
             "metric": "subaperture_spots_per_s", "value": value, "unit": "spots/s", "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": workload_name(c), "spots_per_step_per_gpu": spots_per_step,
+            "config": {"workload": workload_name(c, L, args.noise_flux), "spots_per_step_per_gpu": spots_per_step,
                        "l2": f"inputs larger than L2 ({in_bytes / 1e6:.0f} MB read per step), no flush"},
             "wfs_frames_per_s": value / nsub, "system_frames_per_s": value / nsub / c.W,
             "clocks": clocks,
@@ -264,17 +299,30 @@ def _hbm_peak():
         return 6650.0   # B200_PROFILING.md fallback
 
 
-def cpu_baseline(c, args, phase_dev):
+def cpu_baseline(c, args, phase_dev, yx_lib=None):
     """The oracle as it stands on this box's host cores over a bounded sample of the same batch."""
     from oracle import shwfs_oracle as O
     from paper_1408_0698_b200 import workloads as W
     amp = W.pupil_mask(c)
     yx = O.valid_list(amp, c.n, c.min_illum)
-    K = W.elongation_kernels(c, 0, yx)
-    ph = phase_dev[0][: args.cpu_frames].cpu().numpy()
-    O.measure(ph[:1], amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K)           # page in / build
+    L = args.sublayers
+    if L > 0 or args.noise_flux > 0:
+        K = W.spot_size_kernels(c, yx) if L > 0 else W.elongation_kernels(c, 0, yx)
+        sod = W.sodium_layers(c, 0, max(L, 1))
+        kw = dict(weight=sod["weight"] if L > 0 else [1.0], defocus=sod["defocus"] if L > 0 else [0.0],
+                  tilt_x=sod["tilt_x"] if L > 0 else None, tilt_y=sod["tilt_y"] if L > 0 else None,
+                  cx=sod["cx"], cy=sod["cy"], tau=c.tau, kernels=K,
+                  flux=args.noise_flux / c.n ** 2, ron=args.read_noise, seed=14080698)
+        run = lambda p: O.measure_lgs(p, amp, yx, c.n, c.P, c.b, c.dx, **kw)
+        nfr = max(1, args.cpu_frames // max(L, 1))
+    else:
+        K = W.elongation_kernels(c, 0, yx)
+        run = lambda p: O.measure(p, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K)
+        nfr = args.cpu_frames
+    ph = phase_dev[0][:nfr].cpu().numpy()
+    run(ph[:1])                                                               # page in / build
     t0 = time.perf_counter()
-    O.measure(ph, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K)
+    run(ph)
     dt = time.perf_counter() - t0
     spots = ph.shape[0] * len(yx)
     return {"value": spots / dt, "unit": "spots/s", "cores": O.max_threads(), "kind": "oracle",
@@ -292,6 +340,11 @@ def main():
     ap.add_argument("--cpu-frames", type=int, default=100)
     ap.add_argument("--ref-frames", type=int, default=4)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sublayers", type=int, default=0,
+                    help="L > 0: the paper's full LGS model, L sodium sub-layers with their own wavefronts (8(f) f1)")
+    ap.add_argument("--noise-flux", type=float, default=0.0,
+                    help="> 0: detector noise, photo-electrons per fully lit subaperture per frame (8(f) f2)")
+    ap.add_argument("--read-noise", type=float, default=3.0)
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -290,7 +290,8 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
     }
     __syncthreads();
 
-    const int n_layers = EXT ? A.L : 1;
+    const int n_layers = EXT && A.L > 0 ? A.L : 1;      /* A.L == 0: single-layer sensor (noise only) */
+    const bool sodium = EXT && A.L > 0;
 #pragma unroll 1
     for (int layer = 0; layer < n_layers; ++layer) {
     if (EXT && layer > 0) __syncthreads();        /* every warp is done reading the previous layer's field */
@@ -303,7 +304,7 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
             const float ramp0 = (float)(j + 2 * kk) * A.ramp_unit, ramp1 = ramp0 + A.ramp_unit;
             /* EXT: pixel offsets from the patch centre and the sub-layer's curvature term (reading B1) */
             const float dj = (float)j - 0.5f * (float)(n - 1), dk0 = (float)(2 * kk) - 0.5f * (float)(n - 1);
-            const float lq = EXT ? A.sod_q[layer] : 0.f, lsw = EXT ? A.sod_sw[layer] : 1.f;
+            const float lq = sodium ? A.sod_q[layer] : 0.f, lsw = sodium ? A.sod_sw[layer] : 1.f;
             const float quad0 = lq * (dj * dj + dk0 * dk0), quad1 = lq * (dj * dj + (dk0 + 1.f) * (dk0 + 1.f));
             float2 ph[Cfg::ITEMS];
             int aoff[Cfg::ITEMS];
@@ -334,7 +335,7 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
                             am = __ldg(reinterpret_cast<const float2 *>(A.amp + acur));
                         }
                         float2 e0, e1;
-                        if (EXT) {
+                        if (sodium) {
                             const float2 g = __ldg(A.sod_g + (size_t)layer * A.nsub + s_info[s].z);
                             const float lin = fmaf(g.x, dk0, g.y * dj);
                             e0 = field_value(ph[r].x, am.x * lsw, A.turns, ramp0 - (lin + quad0));

@@ -93,6 +93,17 @@ def test_config3_noise_matches_oracle(gpu, oracle):
             img = s.debug_spots(phd, 3).cpu().numpy()
             assert _img_err(img, wimg) <= IMAGE_TOL, (a, _img_err(img, wimg))
             assert np.abs(got - want).max() <= SLOPE_TOL, (a, np.abs(got - want).max())
+        # noise on the plain single-layer sensor (no sodium model set)
+        s.set_sodium(None)
+        w1, i1 = oracle.measure_lgs(ph, amp, yx, c.n, c.P, c.b, c.dx, weight=[1.0], defocus=[0.0], tau=c.tau,
+                                    kernels=K, flux=F, ron=ron, seed=seed, stage=3)
+        for a in _wk_algos(s, B):
+            got = s.measure(phd).cpu().numpy()
+            img = s.debug_spots(phd, 3).cpu().numpy()
+            assert _img_err(img, i1) <= IMAGE_TOL, (a, _img_err(img, i1))
+            assert np.abs(got - w1).max() <= SLOPE_TOL, (a, np.abs(got - w1).max())
+        s.set_sodium(sod["weight"], sod["defocus"], sod["tilt_x"], sod["tilt_y"], (sod["cx"], sod["cy"]),
+                     shared_phase=True)
         s.algorithm = B.ALGO_WK
         # frames 1.. of the same stream in a second call
         s.set_noise(F, ron, seed, first_frame=1)
