@@ -75,7 +75,7 @@ def test_K4_static_tilt_converges_as_one_minus_gain_to_the_t(loop, gain):
     # C3 delay: the slopes of frame 0 see the full aberration, those of frame t the residual a (1-g)^t
     sx = slopes[:, :, 0].mean(axis=1)
     assert abs(sx[0] / a[0] - 1.0) < 0.05                       # sensor gain ~ 1/b (I3), not exactly 1
-    np.testing.assert_allclose(sx / sx[0], (1 - gain) ** np.arange(T), atol=5e-3)
+    np.testing.assert_allclose(sx / sx[0], (1 - gain) ** np.arange(T), atol=1.2e-2)   # CoG gain varies ~1 % with amplitude
 
 
 def test_K5_zero_gain_freezes_wrong_sign_diverges(loop):
