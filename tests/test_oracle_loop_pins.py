@@ -59,23 +59,23 @@ def test_K3_einsum_restatement_and_slope_order(loop):
 @pytest.mark.parametrize("gain", [0.3, 0.6, 1.0])
 def test_K4_static_tilt_converges_as_one_minus_gain_to_the_t(loop, gain):
     """Pure integrator on a static aberration a: c_t = a (1 - (1-g)^t), so the residual coefficient is
-    a (1-g)^t (sensor in its linear range: 0.3 px tilts, plain CoG)."""
+    a (1-g)^t (sensor in its linear range: 0.06 px tilts, plain CoG)."""
     n, P, b = 8, 16, 1
     N, amp, yx, modes = _setup(n, P, b)
     D = loop.interaction_matrix(modes, amp, yx, n, P, b)
     R = np.linalg.pinv(D)
-    a = np.array([0.30, -0.22])
+    a = np.array([0.06, -0.045])                                # near the calibration amplitude: linear
     T = 7
     ph = np.broadcast_to(np.einsum("m,myx->yx", a, modes), (T, N, N)).astype(np.float32)
     slopes, hist, cT = loop.closed_loop(ph, modes, R, gain, np.zeros(2), amp, yx, n, P, b)
     want = a[None, :] * (1 - (1 - gain) ** np.arange(T))[:, None]
-    np.testing.assert_allclose(hist, want, atol=4e-3)
-    np.testing.assert_allclose(cT, a * (1 - (1 - gain) ** T), atol=4e-3)
+    np.testing.assert_allclose(hist, want, atol=5e-4)
+    np.testing.assert_allclose(cT, a * (1 - (1 - gain) ** T), atol=5e-4)
     assert hist[0].tolist() == [0.0, 0.0]                       # C4: hist[t] is what shaped frame t
     # C3 delay: the slopes of frame 0 see the full aberration, those of frame t the residual a (1-g)^t
     sx = slopes[:, :, 0].mean(axis=1)
     assert abs(sx[0] / a[0] - 1.0) < 0.05                       # sensor gain ~ 1/b (I3), not exactly 1
-    np.testing.assert_allclose(sx / sx[0], (1 - gain) ** np.arange(T), atol=1.2e-2)   # CoG gain varies ~1 % with amplitude
+    np.testing.assert_allclose(sx / sx[0], (1 - gain) ** np.arange(T), atol=4e-3)
 
 
 def test_K5_zero_gain_freezes_wrong_sign_diverges(loop):
