@@ -157,6 +157,40 @@ typedef struct {
 } shwfs_noise;
 int shwfs_set_noise(shwfs_handle *h, const shwfs_noise *nz);
 
+/* ---- closed-loop neighbours of the path -------------------------
+ * "The WFS modules compute the vector signals (X-and Y- slopes) from the residual phase (the open loop
+ *  wavefront subtracted by the DM).  Vector slopes multiplied by the control matrix returns the vector
+ *  coefficients for the modal base linear composition, in the form of the differential coefficients to be
+ *  added to the one defining the existing mirror shape. [...] a pure integrator scheme".
+ * DM phase of frame t = sum_m coef[t][m] * modes[m] (units of the wavefront input); residual = wavefront - DM.
+ * Requires the lag-domain algorithm (EUNSUPPORTED otherwise), like shwfs_set_sodium; with sub-layers the
+ * same DM phase is subtracted from every sub-layer's wavefront.
+ *
+ * shwfs_set_dm: modes_dev DEVICE [M*N*N] fp32; the library keeps its own per-subaperture re-layout
+ * (nsub * ceil4(M) * n*n floats) and does not reference modes_dev after the call returns (it synchronises).
+ * M == 0 or modes_dev == NULL drops the DM.  Errors: EINVAL, EUNSUPPORTED, ENOMEM, ECUDA.               */
+int shwfs_set_dm(shwfs_handle *h, const float *modes_dev, int32_t M);
+
+/* shwfs_measure on the residual phase: coef_dev DEVICE [T*M].  The subtraction happens inside the gather of
+ * the sensor kernel: the residual is never written to memory.  Enqueues on cuda_stream; may (re)allocate a
+ * T*ceil4(M) scratch the first time a larger T is seen (that call synchronises the stream once).
+ * Errors: EINVAL (no DM set, null pointers, T < 0), ENOMEM, ECUDA.                                      */
+int shwfs_measure_residual(shwfs_handle *h, const float *phase_dev, const float *coef_dev, int32_t T,
+                           float *slopes_dev, void *cuda_stream);
+
+/* coef[t][m] += gain * sum_k R[m][k] * slopes[t][k],  k = 2*i + axis  (the layout of slopes[t][i][:]).
+ * R_dev DEVICE [M * 2*nsub] row-major, slopes_dev DEVICE [T*nsub*2], coef_dev DEVICE [T*M] in/out.
+ * M is the count given to shwfs_set_dm.  Enqueues on cuda_stream.  Errors: EINVAL, ECUDA.               */
+int shwfs_reconstruct(shwfs_handle *h, const float *R_dev, const float *slopes_dev, int32_t T, float gain,
+                      float *coef_dev, void *cuda_stream);
+
+/* T sequential frames of the pure-integrator loop, all enqueued on cuda_stream (two kernels per frame):
+ *     s_t = slopes(phase[t] - DM(c_t));  hist[t] = c_t;  c_{t+1} = c_t + gain * R s_t
+ * coef_dev DEVICE [M]: c_0 on entry, c_T on exit.  slopes_dev DEVICE [T*nsub*2].  coef_hist_dev DEVICE [T*M]
+ * or NULL.  With a noise model, frame t uses counter first_frame + t.  Errors: EINVAL, ECUDA.           */
+int shwfs_closed_loop(shwfs_handle *h, const float *phase_dev, const float *R_dev, float gain, float *coef_dev,
+                      int32_t T, float *slopes_dev, float *coef_hist_dev, void *cuda_stream);
+
 /* ---- debug (parity on images; not on the timed path) ------------------------------------------- */
 /* stage 0: centred intensity  roll(I)  DEVICE out [T*nsub*P*P]
  * stage 1: centred image after elongation  Sh  [T*nsub*P*P]  (== stage 0 without kernels)

@@ -25,7 +25,8 @@ ALGO_AUTO, ALGO_LITERAL, ALGO_WK, ALGO_WK_GENERIC, ALGO_PRUNED_FFT = 0, 1, 2, 3,
 EXPORTS = ["shwfs_create", "shwfs_measure", "shwfs_measure_host", "shwfs_destroy", "shwfs_num_subaps",
            "shwfs_valid_list", "shwfs_pixel_scale", "shwfs_set_algorithm", "shwfs_get_algorithm",
            "shwfs_launch_count", "shwfs_debug_spots", "shwfs_strerror", "shwfs_last_cuda_error",
-           "shwfs_version", "shwfs_set_sodium", "shwfs_set_noise"]
+           "shwfs_version", "shwfs_set_sodium", "shwfs_set_noise", "shwfs_set_dm",
+           "shwfs_measure_residual", "shwfs_reconstruct", "shwfs_closed_loop"]
 SHWFS_MAX_LAYERS = 8
 
 
@@ -86,6 +87,10 @@ def load():
     L.shwfs_version.argtypes = []
     L.shwfs_set_sodium.argtypes = [vp, C.POINTER(ShwfsSodium)]
     L.shwfs_set_noise.argtypes = [vp, C.POINTER(ShwfsNoise)]
+    L.shwfs_set_dm.argtypes = [vp, vp, i32]
+    L.shwfs_measure_residual.argtypes = [vp, vp, vp, i32, vp, vp]
+    L.shwfs_reconstruct.argtypes = [vp, vp, vp, i32, C.c_float, vp, vp]
+    L.shwfs_closed_loop.argtypes = [vp, vp, vp, C.c_float, vp, i32, vp, vp, vp]
     for name in EXPORTS:
         if name not in ("shwfs_strerror", "shwfs_last_cuda_error"):
             getattr(L, name).restype = C.c_int
@@ -234,6 +239,67 @@ class Shwfs:
         """Detector noise before the centroid (flux <= 0 switches it off)."""
         nz = ShwfsNoise(float(flux), float(read_noise), int(seed), int(first_frame))
         _check(load().shwfs_set_noise(self._h, C.byref(nz)), "shwfs_set_noise")
+
+    # -- closed-loop neighbours (include/shwfs.h: shwfs_set_dm, shwfs_measure_residual, shwfs_reconstruct,
+    #    shwfs_closed_loop)
+    def set_dm(self, modes):
+        """modes: CUDA float32 [M,N,N] (None drops the DM).  The library keeps its own re-layout."""
+        if modes is None:
+            _check(load().shwfs_set_dm(self._h, None, 0), "shwfs_set_dm")
+            self.M = 0
+            return
+        self._f32_cuda(modes, (None, self.N, self.N), "modes")
+        _check(load().shwfs_set_dm(self._h, modes.data_ptr(), int(modes.shape[0])), "shwfs_set_dm")
+        self.M = int(modes.shape[0])
+
+    @staticmethod
+    def _f32_cuda(x, shape, name):
+        import torch
+        ok = isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() \
+            and x.dim() == len(shape) and all(s is None or s == d for s, d in zip(shape, x.shape))
+        if not ok:
+            raise ValueError(f"{name} must be a contiguous float32 CUDA tensor of shape {shape}")
+
+    def _stream(self, stream, like):
+        import torch
+        return (stream if stream is not None else torch.cuda.current_stream(like.device)).cuda_stream
+
+    def measure_residual(self, phase, coef, out=None, stream=None):
+        """Slopes of phase[t] - sum_m coef[t,m] modes[m]; coef CUDA float32 [T,M]."""
+        import torch
+        self._check_phase(phase)
+        T = phase.shape[0]
+        self._f32_cuda(coef, (T, self.M), "coef")
+        if out is None:
+            out = torch.empty((T, self.nsub, 2), dtype=torch.float32, device=phase.device)
+        _check(load().shwfs_measure_residual(self._h, phase.data_ptr(), coef.data_ptr(), T, out.data_ptr(),
+                                             self._stream(stream, phase)), "shwfs_measure_residual")
+        return out
+
+    def reconstruct(self, R, slopes, coef, gain: float = 1.0, stream=None):
+        """coef[t,m] += gain * sum_k R[m,k] slopes[t,k] in place; R CUDA float32 [M, 2*nsub]."""
+        T = slopes.shape[0]
+        self._f32_cuda(R, (self.M, 2 * self.nsub), "R")
+        self._f32_cuda(slopes, (T, self.nsub, 2), "slopes")
+        self._f32_cuda(coef, (T, self.M), "coef")
+        _check(load().shwfs_reconstruct(self._h, R.data_ptr(), slopes.data_ptr(), T, float(gain), coef.data_ptr(),
+                                        self._stream(stream, slopes)), "shwfs_reconstruct")
+        return coef
+
+    def closed_loop(self, phase, R, gain: float, coef, want_history: bool = True, stream=None):
+        """T sequential pure-integrator frames.  coef CUDA float32 [M] is c_0 on entry and c_T on return.
+        Returns (slopes [T,nsub,2], hist [T,M] or None) with hist[t] = c_t."""
+        import torch
+        self._check_phase(phase)
+        T = phase.shape[0]
+        self._f32_cuda(R, (self.M, 2 * self.nsub), "R")
+        self._f32_cuda(coef, (self.M,), "coef")
+        slopes = torch.empty((T, self.nsub, 2), dtype=torch.float32, device=phase.device)
+        hist = torch.empty((T, self.M), dtype=torch.float32, device=phase.device) if want_history else None
+        _check(load().shwfs_closed_loop(self._h, phase.data_ptr(), R.data_ptr(), float(gain), coef.data_ptr(), T,
+                                        slopes.data_ptr(), hist.data_ptr() if want_history else None,
+                                        self._stream(stream, phase)), "shwfs_closed_loop")
+        return slopes, hist
 
     # -- the hot path
     def _check_phase(self, phase):

@@ -203,6 +203,27 @@ def spot_size_kernels(c: WfsConfig, valid_yx: np.ndarray, device=None):
                               device=device)
 
 
+def dm_modes(c: WfsConfig, M: int) -> np.ndarray:
+    """Stand-in for the paper's modal base (Zernike or Karhunen-Loeve modes fitted by the
+    actuators): mode 0 and 1 are x and y tilt of one unbinned pixel of spot motion (2 pi / P rad per pupil
+    pixel); the others are seeded von Karman screens (same recipe as phase_screen, seeds of "WFS" 900+m)
+    scaled to 1 rad rms over the pupil -- smooth, turbulence-like shapes.  fp32 [M,N,N]."""
+    amp = pupil_mask(c) > 0
+    ax = np.arange(c.N, dtype=np.float64) + 0.5 - c.N / 2.0
+    out = np.empty((M, c.N, c.N), dtype=np.float32)
+    for m in range(M):
+        if m == 0:
+            md = np.broadcast_to(ax[None, :] * (2.0 * math.pi / c.P), (c.N, c.N))
+        elif m == 1:
+            md = np.broadcast_to(ax[:, None] * (2.0 * math.pi / c.P), (c.N, c.N))
+        else:
+            md = phase_screen(c, 900 + m, 0).astype(np.float64)
+            md = md - md[amp].mean()
+            md = md / md[amp].std()
+        out[m] = md
+    return out
+
+
 def phase_frames_device(c: WfsConfig, wfs: int, frames, device, out=None):
     """Same von Karman recipe as phase_screen, evaluated with torch on `device` (float64 FFT, cast to fp32).
 
