@@ -199,11 +199,29 @@ def run_ours(args):
     out_bytes = sum(s.numel() * 4 for s in slopes)
     stream = torch.cuda.Stream(dev)
 
+    # closed-loop neighbours: DM of --dm-modes modes, residual fused into the gather
+    Mdm = args.dm_modes
+    if Mdm > 0:
+        modes = W.dm_modes_device(c, Mdm, dev)
+        for s in sensors:
+            s.set_dm(modes)
+        del modes
+        gen = torch.Generator(device=dev); gen.manual_seed(1408)
+        coef = [torch.randn((frames, Mdm), device=dev, generator=gen) * 0.2 for _ in range(c.W)]
+        Rmat = [torch.randn((Mdm, 2 * nsub), device=dev, generator=gen) / nsub for _ in range(c.W)]
+        cstate = [torch.zeros(Mdm, device=dev) for _ in range(c.W)]
+
     def step(events=None):
         for w, s in enumerate(sensors):
             if events is not None:
                 e0 = torch.cuda.Event(enable_timing=True); e0.record(stream)
-            s.measure(phase[w], out=slopes[w], stream=stream)
+            if Mdm > 0 and args.closed_loop:
+                with torch.cuda.stream(stream):
+                    s.closed_loop(phase[w], Rmat[w], 0.3, cstate[w], want_history=False, stream=stream)
+            elif Mdm > 0:
+                s.measure_residual(phase[w], coef[w], out=slopes[w], stream=stream)
+            else:
+                s.measure(phase[w], out=slopes[w], stream=stream)
             if events is not None:
                 e1 = torch.cuda.Event(enable_timing=True); e1.record(stream)
                 events.append((e0, e1))
@@ -236,6 +254,28 @@ def run_ours(args):
     kern_ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
     ms_total = max_over_ranks(ms_total, dev)
     value = job_throughput(spots_per_step, args.steps, ms_total, world)
+
+    if Mdm > 0:
+        # no host-buffer entry point for the loop calls: report the device-resident numbers only
+        if rank == 0:
+            spots_per_launch = frames * nsub
+            print(json.dumps({
+                "metric": "subaperture_spots_per_s", "value": value, "unit": "spots/s", "n_gpus": world,
+                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": workload_name(c, L, args.noise_flux) + f", DM of {Mdm} modes, " +
+                           ("sequential pure-integrator loop (shwfs_closed_loop)" if args.closed_loop
+                            else "residual fused into the gather (shwfs_measure_residual)"),
+                           "spots_per_step_per_gpu": spots_per_step},
+                "wfs_frames_per_s": value / nsub, "loop_steps_per_s_per_wfs": value / nsub if args.closed_loop else None,
+                "ms_per_wfs_call": kern_ms, "clocks": clocks, "e2e": None, "gpu_launches": int(launches),
+                "dm_flops_per_spot": 2 * Mdm * c.n * c.n,
+                "dm_tflops": 2 * Mdm * c.n * c.n * spots_per_launch / (kern_ms * 1e-3) / 1e12}))
+        for s in sensors:
+            s.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return
 
     # ---- end to end from pinned host memory through shwfs_measure_host
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
@@ -345,6 +385,10 @@ def main():
     ap.add_argument("--noise-flux", type=float, default=0.0,
                     help="> 0: detector noise, photo-electrons per fully lit subaperture per frame (8(f) f2)")
     ap.add_argument("--read-noise", type=float, default=3.0)
+    ap.add_argument("--dm-modes", type=int, default=0,
+                    help="M > 0: subtract a DM of M modes inside the gather (8(f) f3, shwfs_measure_residual)")
+    ap.add_argument("--closed-loop", action="store_true",
+                    help="with --dm-modes: run the batch as sequential pure-integrator frames (shwfs_closed_loop)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

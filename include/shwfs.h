@@ -167,13 +167,14 @@ int shwfs_set_noise(shwfs_handle *h, const shwfs_noise *nz);
  * same DM phase is subtracted from every sub-layer's wavefront.
  *
  * shwfs_set_dm: modes_dev DEVICE [M*N*N] fp32; the library keeps its own per-subaperture re-layout
- * (nsub * ceil4(M) * n*n floats) and does not reference modes_dev after the call returns (it synchronises).
+ * (nsub * M * n*n floats) and does not reference modes_dev after the call returns (it synchronises).
  * M == 0 or modes_dev == NULL drops the DM.  Errors: EINVAL, EUNSUPPORTED, ENOMEM, ECUDA.               */
 int shwfs_set_dm(shwfs_handle *h, const float *modes_dev, int32_t M);
 
-/* shwfs_measure on the residual phase: coef_dev DEVICE [T*M].  The subtraction happens inside the gather of
- * the sensor kernel: the residual is never written to memory.  Enqueues on cuda_stream; may (re)allocate a
- * T*ceil4(M) scratch the first time a larger T is seen (that call synchronises the stream once).
+/* shwfs_measure on the residual phase: coef_dev DEVICE [T*M].  Two kernels: the DM phase on the valid
+ * subapertures (a batched GEMM into a T*nsub*n*n scratch in patch layout), then the sensor kernel, whose
+ * gather subtracts it: the full-frame residual is never written to memory.  Enqueues on cuda_stream; may
+ * (re)allocate the scratch the first time a larger T is seen (that call synchronises the stream once).
  * Errors: EINVAL (no DM set, null pointers, T < 0), ENOMEM, ECUDA.                                      */
 int shwfs_measure_residual(shwfs_handle *h, const float *phase_dev, const float *coef_dev, int32_t T,
                            float *slopes_dev, void *cuda_stream);
@@ -184,7 +185,7 @@ int shwfs_measure_residual(shwfs_handle *h, const float *phase_dev, const float 
 int shwfs_reconstruct(shwfs_handle *h, const float *R_dev, const float *slopes_dev, int32_t T, float gain,
                       float *coef_dev, void *cuda_stream);
 
-/* T sequential frames of the pure-integrator loop, all enqueued on cuda_stream (two kernels per frame):
+/* T sequential frames of the pure-integrator loop, all enqueued on cuda_stream (three kernels per frame):
  *     s_t = slopes(phase[t] - DM(c_t));  hist[t] = c_t;  c_{t+1} = c_t + gain * R s_t
  * coef_dev DEVICE [M]: c_0 on entry, c_T on exit.  slopes_dev DEVICE [T*nsub*2].  coef_hist_dev DEVICE [T*M]
  * or NULL.  With a noise model, frame t uses counter first_frame + t.  Errors: EINVAL, ECUDA.           */

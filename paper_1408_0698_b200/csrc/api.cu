@@ -40,8 +40,7 @@ void free_handle(shwfs_handle *h)
     cudaFree(h->d_khat);
     cudaFree(h->d_sod_g);
     cudaFree(h->d_dm_modes);
-    cudaFree(h->d_coef_pad);
-    cudaFree(h->d_loop_coef);
+    cudaFree(h->d_dm_patch);
     for (int k = 0; k < 2; ++k) {
         if (h->h_pin[k]) cudaFreeHost(h->h_pin[k]);
         cudaFree(h->d_phase[k]);
@@ -326,16 +325,13 @@ int shwfs_set_dm(shwfs_handle *h, const float *modes_dev, int32_t M)
     int rc = SHWFS_OK;
     cudaDeviceSynchronize();                     /* nothing in flight may still read the old tables */
     cudaFree(h->d_dm_modes); h->d_dm_modes = nullptr;
-    cudaFree(h->d_loop_coef); h->d_loop_coef = nullptr;
-    cudaFree(h->d_coef_pad); h->d_coef_pad = nullptr; h->coef_pad_cap = 0;
-    h->dm_M = 0; h->dm_Mp = 0;
+    cudaFree(h->d_dm_patch); h->d_dm_patch = nullptr; h->dm_patch_cap = 0;
+    h->dm_M = 0;
     if (M > 0 && modes_dev) {
         if (!shwfs_wk_supported(h, 0) && !shwfs_wk_supported(h, 1)) { rc = SHWFS_EUNSUPPORTED; goto done; }
-        const int Mp = (M + 3) & ~3;
-        h->dm_Mp = Mp;
-        CU_TRY(cudaMalloc(&h->d_dm_modes, sizeof(float) * (size_t)h->nsub * Mp * h->n * h->n), "cudaMalloc(dm modes)");
-        CU_TRY(cudaMalloc(&h->d_loop_coef, sizeof(float) * (size_t)Mp), "cudaMalloc(loop coef)");
-        CU_TRY(cudaMemset(h->d_loop_coef, 0, sizeof(float) * (size_t)Mp), "cudaMemset(loop coef)");
+        CU_TRY(cudaMalloc(&h->d_dm_modes, sizeof(float) * (size_t)h->nsub * M * h->n * h->n), "cudaMalloc(dm modes)");
+        h->dm_patch_cap = (size_t)h->nsub * h->n * h->n;          /* one frame: enough for the loop */
+        CU_TRY(cudaMalloc(&h->d_dm_patch, sizeof(float) * h->dm_patch_cap), "cudaMalloc(dm patch)");
         CU_TRY(shwfs_loop_relayout_modes(h, modes_dev, M, 0), "relayout_modes");
         CU_TRY(cudaStreamSynchronize(0), "set_dm sync");
         h->dm_M = M;
@@ -343,8 +339,8 @@ int shwfs_set_dm(shwfs_handle *h, const float *modes_dev, int32_t M)
     goto done;
 fail:
     cudaFree(h->d_dm_modes); h->d_dm_modes = nullptr;
-    cudaFree(h->d_loop_coef); h->d_loop_coef = nullptr;
-    h->dm_M = 0; h->dm_Mp = 0;
+    cudaFree(h->d_dm_patch); h->d_dm_patch = nullptr; h->dm_patch_cap = 0;
+    h->dm_M = 0;
 done:
     if (prev >= 0 && prev != h->device) cudaSetDevice(prev);
     return rc;
@@ -356,17 +352,17 @@ static bool ext_on(const shwfs_handle *h) { return h->sod_L > 0 || h->nz_flux > 
 static int frames_per_step(const shwfs_handle *h) { return (h->sod_L > 0 && !h->sod_shared) ? h->sod_L : 1; }
 
 static int run_path(shwfs_handle *h, const float *phase_dev, int T, float *slopes_dev, int stage, float *img,
-                    unsigned t_base, cudaStream_t st, const float *dm_coef = nullptr)
+                    unsigned t_base, cudaStream_t st, const float *dm_patch = nullptr)
 {
     if ((long long)T * h->nsub > 0x7fffffffLL / 2) return SHWFS_EINVAL;
     cudaError_t e;
     if (stage == 3 && !(h->nz_flux > 0.f)) stage = 2;      /* no noise: the final image is the binned one */
-    if (ext_on(h) || dm_coef) {
+    if (ext_on(h) || dm_patch) {
         /* sub-layers / noise / DM live in the lag-domain kernels only (shwfs_set_sodium made sure one exists) */
         if (stage == 0 || stage == 1) return SHWFS_EUNSUPPORTED;
         const int generic = (h->algo == SHWFS_ALGO_WK_GENERIC) || !shwfs_wk_supported(h, 0);
         e = shwfs_wk_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr, stage == 3 ? img : nullptr,
-                            t_base, dm_coef, generic, st);
+                            t_base, dm_patch, generic, st);
     } else if (stage == 0 || stage == 1) {
         int rc = ensure_khat(h);
         if (rc) return rc;
@@ -404,18 +400,18 @@ int shwfs_measure_residual(shwfs_handle *h, const float *phase_dev, const float 
     if (T == 0) return SHWFS_OK;
     if (!phase_dev || !coef_dev || !slopes_dev) return SHWFS_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const size_t need = (size_t)T * h->dm_Mp;
-    if (h->coef_pad_cap < need) {
+    const size_t need = (size_t)T * h->nsub * h->n * h->n;
+    if (h->dm_patch_cap < need) {
         cudaStreamSynchronize(st);
-        cudaFree(h->d_coef_pad); h->d_coef_pad = nullptr; h->coef_pad_cap = 0;
-        cudaError_t e = cudaMalloc(&h->d_coef_pad, sizeof(float) * need);
-        if (e != cudaSuccess) { shwfs_note_cuda_error(e, "cudaMalloc(coef pad)"); return SHWFS_ENOMEM; }
-        h->coef_pad_cap = need;
+        cudaFree(h->d_dm_patch); h->d_dm_patch = nullptr; h->dm_patch_cap = 0;
+        cudaError_t e = cudaMalloc(&h->d_dm_patch, sizeof(float) * need);
+        if (e != cudaSuccess) { shwfs_note_cuda_error(e, "cudaMalloc(dm patch)"); return SHWFS_ENOMEM; }
+        h->dm_patch_cap = need;
     }
-    cudaError_t e = shwfs_loop_pad_coef(coef_dev, T, h->dm_M, h->dm_Mp, h->d_coef_pad, st);
-    if (e != cudaSuccess) { shwfs_note_cuda_error(e, "pad_coef"); return SHWFS_ECUDA; }
+    cudaError_t e = shwfs_loop_dm_phase(h, coef_dev, h->dm_M, T, h->d_dm_patch, st);
+    if (e != cudaSuccess) { shwfs_note_cuda_error(e, "dm_phase"); return SHWFS_ECUDA; }
     h->launches += 1;
-    return run_path(h, phase_dev, T, slopes_dev, -1, nullptr, 0u, st, h->d_coef_pad);
+    return run_path(h, phase_dev, T, slopes_dev, -1, nullptr, 0u, st, h->d_dm_patch);
 }
 
 int shwfs_reconstruct(shwfs_handle *h, const float *R_dev, const float *slopes_dev, int32_t T, float gain,
@@ -440,18 +436,19 @@ int shwfs_closed_loop(shwfs_handle *h, const float *phase_dev, const float *R_de
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t step = (size_t)h->N * h->N * frames_per_step(h);
     const int K = 2 * h->nsub;
-    /* the integrator state lives in the handle's padded vector (its tail stays zero) */
-    cudaError_t e = shwfs_loop_unpad_coef(coef_dev, h->dm_M, h->d_loop_coef, st);
-    h->launches += 1;
+    /* per frame: DM phase of c_t on the valid patches, sensor on the residual, c_{t+1} = c_t + gain R s_t */
+    cudaError_t e = cudaSuccess;
     for (int t = 0; t < T && e == cudaSuccess; ++t) {
+        e = shwfs_loop_dm_phase(h, coef_dev, h->dm_M, 1, h->d_dm_patch, st);
+        if (e != cudaSuccess) break;
+        h->launches += 1;
         int rc = run_path(h, phase_dev + (size_t)t * step, 1, slopes_dev + (size_t)t * K, -1, nullptr, (unsigned)t,
-                          st, h->d_loop_coef);
+                          st, h->d_dm_patch);
         if (rc) return rc;
-        e = shwfs_loop_reconstruct(R_dev, slopes_dev + (size_t)t * K, 1, K, h->dm_M, gain, h->d_loop_coef, h->dm_Mp,
+        e = shwfs_loop_reconstruct(R_dev, slopes_dev + (size_t)t * K, 1, K, h->dm_M, gain, coef_dev, h->dm_M,
                                    coef_hist_dev ? coef_hist_dev + (size_t)t * h->dm_M : nullptr, st);
         h->launches += 1;
     }
-    if (e == cudaSuccess) { e = shwfs_loop_unpad_coef(h->d_loop_coef, h->dm_M, coef_dev, st); h->launches += 1; }
     if (e != cudaSuccess) { shwfs_note_cuda_error(e, "closed_loop"); return SHWFS_ECUDA; }
     return SHWFS_OK;
 }

@@ -42,11 +42,10 @@ struct shwfs_handle {
     uint32_t nz_first_frame;
 
     /* closed-loop neighbours (shwfs_set_dm ...): modes re-laid per subaperture, padded coefficient buffers */
-    float  *d_dm_modes;                 /* [nsub][Mp][n*n] */
-    int     dm_M, dm_Mp;                /* Mp = M rounded up to a multiple of 4 */
-    float  *d_coef_pad;                 /* [cap_T][Mp] padded copy of the caller's coef[T][M] */
-    size_t  coef_pad_cap;               /* floats */
-    float  *d_loop_coef;                /* [Mp] integrator state of shwfs_closed_loop */
+    float  *d_dm_modes;                 /* [nsub][M][n*n] modes re-laid per subaperture */
+    int     dm_M;
+    float  *d_dm_patch;                 /* [cap_T][nsub][n*n] DM phase of the current call, patch layout */
+    size_t  dm_patch_cap;               /* floats */
 
     /* host copies for queries */
     int32_t *h_valid;      /* [nsub*2] (sy,sx) */
@@ -71,12 +70,11 @@ cudaError_t shwfs_wk_build_table(shwfs_handle *h, cudaStream_t st);
 /* Wiener-Khinchin path: slopes (and optionally the binned image B, [T*nsub*D*D]) */
 cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *slopes,
                             float *binned_or_null, float *noisy_or_null, unsigned t_base,
-                            const float *dm_coef_padded_or_null, int generic, cudaStream_t st);
+                            const float *dm_patch_or_null, int generic, cudaStream_t st);
 
 /* loop.cu: closed-loop neighbours */
 cudaError_t shwfs_loop_relayout_modes(shwfs_handle *h, const float *modes_dev, int M, cudaStream_t st);
-cudaError_t shwfs_loop_pad_coef(const float *coef, int T, int M, int Mp, float *out, cudaStream_t st);
-cudaError_t shwfs_loop_unpad_coef(const float *padded, int M, float *out, cudaStream_t st);
+cudaError_t shwfs_loop_dm_phase(shwfs_handle *h, const float *coef, int ldc, int T, float *out, cudaStream_t st);
 cudaError_t shwfs_loop_reconstruct(const float *R, const float *slopes, int T, int K, int M, float gain,
                                    float *coef, int ldc, float *hist_or_null, cudaStream_t st);
 int shwfs_wk_supported(const shwfs_handle *h, int generic);

@@ -140,10 +140,9 @@ struct WkArgs {
     float flux, ron2;
     uint2 key;
     unsigned t0;
-    /* closed-loop neighbour (EXT instances only): residual = wavefront - sum_m coef[t][m] * mode[m]   */
-    const float *dm_modes;       /* [nsub][Mp][n*n] modes re-laid per subaperture, or null              */
-    const float *dm_coef;        /* [T][Mp] coefficients, zero padded to Mp (multiple of 4)             */
-    int dm_Mp;
+    /* closed-loop neighbour (EXT instances only): residual = wavefront - DM phase.  The DM
+     * phase sum_m coef[t][m] * mode[m] arrives in patch layout from dm_phase_kernel (loop.cu).          */
+    const float *dm_patch;       /* [T][nsub][n*n] or null */
 };
 
 template <int n>
@@ -326,31 +325,16 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
                     }
                 }
             }
-            if (EXT && A.dm_modes != nullptr) {
-                /* PAPER.md:76 "the residual phase (the open loop wavefront subtracted by the DM)": four modes
-                 * per step; a thread's spots mostly share one subaperture, whose mode values are then reused */
-                const int m4n = A.dm_Mp >> 2;
-                const float4 *coef4 = reinterpret_cast<const float4 *>(A.dm_coef);
-#pragma unroll 1
-                for (int m4 = 0; m4 < m4n; ++m4) {
-                    int cur = -1;
-                    float2 mv0 = make_float2(0.f, 0.f), mv1 = mv0, mv2 = mv0, mv3 = mv0;
+            if (EXT && A.dm_patch != nullptr) {
+                /* PAPER.md:76 "the residual phase (the open loop wavefront subtracted by the DM)" */
 #pragma unroll
-                    for (int r = 0; r < Cfg::ITEMS; ++r) {
-                        const int s = sg + r * Cfg::SG;
-                        if (s < Cfg::SPOTS && aoff[r] >= 0) {
-                            const int4 inf = s_info[s];
-                            if (inf.z != cur) {
-                                cur = inf.z;
-                                const float2 *mp = reinterpret_cast<const float2 *>(A.dm_modes)
-                                                   + ((size_t)cur * A.dm_Mp + 4 * m4) * Cfg::NP + q2;
-                                mv0 = __ldg(mp); mv1 = __ldg(mp + Cfg::NP);
-                                mv2 = __ldg(mp + 2 * Cfg::NP); mv3 = __ldg(mp + 3 * Cfg::NP);
-                            }
-                            const float4 c = __ldg(coef4 + (size_t)inf.y * m4n + m4);
-                            ph[r].x -= fmaf(c.x, mv0.x, fmaf(c.y, mv1.x, fmaf(c.z, mv2.x, c.w * mv3.x)));
-                            ph[r].y -= fmaf(c.x, mv0.y, fmaf(c.y, mv1.y, fmaf(c.z, mv2.y, c.w * mv3.y)));
-                        }
+                for (int r = 0; r < Cfg::ITEMS; ++r) {
+                    const int s = sg + r * Cfg::SG;
+                    if (s < Cfg::SPOTS && aoff[r] >= 0) {
+                        const int4 inf = s_info[s];
+                        const float2 d = __ldg(reinterpret_cast<const float2 *>(A.dm_patch)
+                                               + ((size_t)inf.y * A.nsub + inf.z) * Cfg::NP + q2);
+                        ph[r].x -= d.x; ph[r].y -= d.y;
                     }
                 }
             }
@@ -500,13 +484,7 @@ __global__ void __launch_bounds__(GEN_THREADS) wk_generic_kernel(const WkArgs A,
             sw = A.sod_sw[layer];
         }
         float pv = A.phase[(size_t)t * A.frame_stride + (size_t)layer * A.layer_stride + o];
-        if (A.dm_modes != nullptr) {                       /* residual phase */
-            const float *mp = A.dm_modes + (size_t)i * A.dm_Mp * (n * n) + q;
-            const float *cp = A.dm_coef + (size_t)t * A.dm_Mp;
-            float dm = 0.f;
-            for (int m = 0; m < A.dm_Mp; ++m) dm = fmaf(cp[m], mp[(size_t)m * (n * n)], dm);
-            pv -= dm;
-        }
+        if (A.dm_patch != nullptr) pv -= A.dm_patch[((size_t)t * A.nsub + i) * (n * n) + q];   /* residual */
         e[q] = field_value(pv, A.amp[o] * sw, A.turns, (float)(j + k) * A.ramp_unit - extra);
     }
     __syncthreads();
@@ -616,7 +594,7 @@ cudaError_t launch_special_mode(const WkArgs &A, cudaStream_t st)
 template <int n>
 cudaError_t launch_special(const WkArgs &A, cudaStream_t st)
 {
-    if (A.L > 0 || A.flux > 0.f || A.dm_modes != nullptr)
+    if (A.L > 0 || A.flux > 0.f || A.dm_patch != nullptr)
         return A.mode == 0 ? launch_special_mode<n, 0, true>(A, st) : launch_special_mode<n, 1, true>(A, st);
     return A.mode == 0 ? launch_special_mode<n, 0, false>(A, st) : launch_special_mode<n, 1, false>(A, st);
 }
@@ -643,7 +621,7 @@ cudaError_t shwfs_wk_build_table(shwfs_handle *h, cudaStream_t st)
 }
 
 cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *slopes, float *binned,
-                            float *noisy, unsigned t_base, const float *dm_coef, int generic, cudaStream_t st)
+                            float *noisy, unsigned t_base, const float *dm_patch, int generic, cudaStream_t st)
 {
     WkArgs A;
     A.phase = phase; A.amp = h->d_amp; A.valid = h->d_valid; A.M = h->d_wk_table;
@@ -655,7 +633,7 @@ cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *s
     A.flux = h->nz_flux; A.ron2 = h->nz_ron * h->nz_ron;
     A.key = make_uint2((unsigned)h->nz_seed, (unsigned)(h->nz_seed >> 32));
     A.t0 = h->nz_first_frame + t_base;
-    A.dm_modes = dm_coef ? h->d_dm_modes : nullptr; A.dm_coef = dm_coef; A.dm_Mp = h->dm_Mp;
+    A.dm_patch = dm_patch;
     A.T = T; A.N = h->N; A.nsub = h->nsub; A.mstride = h->wk_table_stride;
     A.total = T * h->nsub; A.mode = h->mode;
     A.tau = h->tau;

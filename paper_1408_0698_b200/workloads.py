@@ -224,6 +224,23 @@ def dm_modes(c: WfsConfig, M: int) -> np.ndarray:
     return out
 
 
+def dm_modes_device(c: WfsConfig, M: int, device):
+    """dm_modes with the screens generated on `device` (phase_frames_device, "WFS" 900): timing runs only."""
+    import torch
+    out = torch.empty((M, c.N, c.N), dtype=torch.float32, device=device)
+    ax = (torch.arange(c.N, dtype=torch.float64, device=device) + 0.5 - c.N / 2.0) * (2.0 * math.pi / c.P)
+    out[0] = ax[None, :].expand(c.N, c.N).to(torch.float32)
+    if M > 1:
+        out[1] = ax[:, None].expand(c.N, c.N).to(torch.float32)
+    if M > 2:
+        phase_frames_device(c, 900, range(2, M), device, out=out[2:])
+        amp = torch.as_tensor(pupil_mask(c) > 0, device=device)
+        for m in range(2, M):
+            v = out[m][amp]
+            out[m] = (out[m] - v.mean()) / v.std()
+    return out
+
+
 def phase_frames_device(c: WfsConfig, wfs: int, frames, device, out=None):
     """Same von Karman recipe as phase_screen, evaluated with torch on `device` (float64 FFT, cast to fp32).
 

@@ -104,7 +104,7 @@ def test_closed_loop_matches_oracle(gpu, oracle, loop, cfg_id, M, T, noise):
         cd = torch.from_numpy(c0.copy()).cuda()
         l0 = s.launch_count
         got_s, got_h = s.closed_loop(torch.from_numpy(ph).cuda(), torch.from_numpy(R).cuda(), gain, cd)
-        assert s.launch_count - l0 == 2 * T + 2
+        assert s.launch_count - l0 == 3 * T
         scale = max(np.abs(want_h).max(), 1e-3)
         assert np.abs(got_s.cpu().numpy() - want_s).max() <= SLOPE_TOL
         np.testing.assert_allclose(got_h.cpu().numpy(), want_h, rtol=0, atol=2e-4 * scale)
