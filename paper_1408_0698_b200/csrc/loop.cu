@@ -12,10 +12,12 @@
  *                     shwfs_set_dm (contiguous, coalesced, L2-friendly); the sensor kernel's gather (wk.cu,
  *                     EXT instances) subtracts it from the wavefront, so the full-frame residual never
  *                     exists in memory;
- *   after the path    d[t,m] = sum_k R[m,k] s[t,k] (k = 2 i + axis), c += gain * d: recon_kernel, one warp
- *                     per mode, the slope vector streamed with 8-byte loads, warp-shuffle reduction.
+ *   after the path    d[t,m] = sum_k R[m,k] s[t,k] (k = 2 i + axis), c += gain * d: recon_kernel, one CTA
+ *                     per mode, the row of R split over its threads, shuffle + shared-memory reduction.
  * shwfs_closed_loop chains the two, frame after frame, on the caller's stream (readings C1..C4 of DESIGN.md).
  */
+#include <cuda_pipeline.h>
+
 #include "internal.h"
 
 namespace {
@@ -36,58 +38,75 @@ __global__ void relayout_modes_kernel(const float *__restrict__ modes, const int
 /* DM phase in patch layout: out[t][i][q] = sum_m coef[t*ldc + m] * modes_sub[i][m][q], q < n*n (n*n % 4 == 0).
  * CTA = (subaperture i, tile of TT = 8*FT frames), 256 threads = 8 frame groups x 32 float4 columns; modes
  * of MC at a time go through shared memory (one contiguous, coalesced block of the re-laid table), the
- * coefficient tile transposed so that a thread's FT frames are one 16-byte broadcast load.  FT = 4 for
- * batches (register tile 4 frames x 4 pixels, 16 FFMA per two LDS.128), FT = 1 for the T = 1 loop step,
+ * coefficient tile transposed so that a thread's FT frames are one 16-byte broadcast load; two stages filled
+ * by cp.async so that the loads of chunk c+1 overlap the arithmetic of chunk c.  FT = 8 for
+ * batches (register tile 8 frames x 4 pixels, FT = 4 up to 32 frames; n*n is a template parameter so that every shared-memory
+ * offset is an immediate and the k loop is branch-free), FT = 1 for the T = 1 loop step,
  * which is bound by streaming the mode table.                                                          */
 constexpr int DM_MC = 16;
 
-template <int FT>
+template <int FT, int NN>
 __global__ void __launch_bounds__(256) dm_phase_kernel(const float *__restrict__ coef, int ldc,
-                                                       const float *__restrict__ modes_sub, int T, int nsub, int nn,
-                                                       int M, float *__restrict__ out)
+                                                       const float *__restrict__ modes_sub, int T, int nsub, int M,
+                                                       float *__restrict__ out)
 {
-    constexpr int TT = 8 * FT;
+    constexpr int TT = 8 * FT, NQ = NN / 4, MAXQ = (NQ + 31) / 32;
+    constexpr int TS = TT + 4;                              /* padded row of the transposed coefficient tile */
+    constexpr int STAGE = DM_MC * NN + DM_MC * TS;          /* [DM_MC][NN] modes, then [DM_MC][TS] coefficients */
     extern __shared__ __align__(16) float dm_smem[];
-    float *sm_modes = dm_smem;                      /* [DM_MC][nn]  */
-    float *sm_coef = dm_smem + DM_MC * nn;          /* [DM_MC][TT]  */
-    const int i = blockIdx.x, t0 = blockIdx.y * TT;
-    const int tid = threadIdx.x, fy = tid >> 5, lane = tid & 31;
-    const int NQ = nn >> 2;
-    constexpr int MAXQ = 2;                         /* columns per lane: nn <= 256 */
+    const int i = blockIdx.y, t0 = blockIdx.x * TT;        /* frame tiles of one subaperture are neighbours: */
+    const int tid = threadIdx.x, fy = tid >> 5, lane = tid & 31;   /* its mode slice is re-read from L2       */
     float4 acc[MAXQ][FT];
 #pragma unroll
     for (int c = 0; c < MAXQ; ++c)
 #pragma unroll
         for (int f = 0; f < FT; ++f) acc[c][f] = make_float4(0.f, 0.f, 0.f, 0.f);
-    const float *mi = modes_sub + (size_t)i * M * nn;
-    for (int m0 = 0; m0 < M; m0 += DM_MC) {
+    const float *mi = modes_sub + (size_t)i * M * NN;
+
+    /* cp.async (LDGSTS) one chunk of modes and the transposed coefficient tile into stage `st`; rows past M
+     * and frames past T are zero-filled so that the arithmetic below needs no bounds */
+    auto issue = [&](int st, int m0) {
+        float *sm_modes = dm_smem + st * STAGE, *sm_coef = sm_modes + DM_MC * NN;
         const int mc = min(DM_MC, M - m0);
-        __syncthreads();
-        {
-            const float4 *src = reinterpret_cast<const float4 *>(mi + (size_t)m0 * nn);
-            float4 *dst = reinterpret_cast<float4 *>(sm_modes);
-            for (int q = tid; q < mc * NQ; q += 256) dst[q] = __ldg(src + q);
-            for (int q = tid; q < DM_MC * TT; q += 256) {
-                const int k = q / TT, f = q - k * TT;
-                sm_coef[q] = (k < mc && t0 + f < T) ? __ldg(coef + (size_t)(t0 + f) * ldc + m0 + k) : 0.f;
-            }
+        const float4 *src = reinterpret_cast<const float4 *>(mi + (size_t)m0 * NN);
+        for (int q = tid; q < DM_MC * NQ; q += 256) {
+            const bool ok = q < mc * NQ;
+            __pipeline_memcpy_async(reinterpret_cast<float4 *>(sm_modes) + q, ok ? src + q : src, 16, ok ? 0 : 16);
         }
+        for (int q = tid; q < DM_MC * TT; q += 256) {
+            const int f = q / DM_MC, k = q - f * DM_MC;      /* consecutive threads: consecutive modes of a frame */
+            const bool ok = k < mc && t0 + f < T;
+            __pipeline_memcpy_async(sm_coef + k * TS + f, ok ? coef + (size_t)(t0 + f) * ldc + m0 + k : coef, 4,
+                                    ok ? 0 : 4);
+        }
+        __pipeline_commit();
+    };
+
+    const int nchunk = (M + DM_MC - 1) / DM_MC;
+    issue(0, 0);
+    for (int ch = 0; ch < nchunk; ++ch) {
+        if (ch + 1 < nchunk) { issue((ch + 1) & 1, (ch + 1) * DM_MC); __pipeline_wait_prior(1); }
+        else __pipeline_wait_prior(0);
         __syncthreads();
-#pragma unroll 4
-        for (int k = 0; k < mc; ++k) {
+        const float *sm_modes = dm_smem + (ch & 1) * STAGE, *sm_coef = sm_modes + DM_MC * NN;
+#pragma unroll
+        for (int k = 0; k < DM_MC; ++k) {
             float a[FT];
-            if (FT == 4) {
-                const float4 v = *reinterpret_cast<const float4 *>(sm_coef + k * TT + fy * FT);
-                a[0] = v.x; a[1 % FT] = v.y; a[2 % FT] = v.z; a[3 % FT] = v.w;
+            if (FT % 4 == 0) {
+#pragma unroll
+                for (int f4 = 0; f4 < FT / 4; ++f4) {
+                    const float4 v = *reinterpret_cast<const float4 *>(sm_coef + k * TS + fy * FT + 4 * f4);
+                    a[(4 * f4) % FT] = v.x; a[(4 * f4 + 1) % FT] = v.y; a[(4 * f4 + 2) % FT] = v.z; a[(4 * f4 + 3) % FT] = v.w;
+                }
             } else {
 #pragma unroll
-                for (int f = 0; f < FT; ++f) a[f] = sm_coef[k * TT + fy * FT + f];
+                for (int f = 0; f < FT; ++f) a[f] = sm_coef[k * TS + fy * FT + f];
             }
 #pragma unroll
             for (int c = 0; c < MAXQ; ++c) {
                 const int cq = lane + 32 * c;
-                if (cq < NQ) {
-                    const float4 b = *reinterpret_cast<const float4 *>(sm_modes + k * nn + 4 * cq);
+                if ((c + 1) * 32 <= NQ || cq < NQ) {
+                    const float4 b = *reinterpret_cast<const float4 *>(sm_modes + k * NN + 4 * cq);
 #pragma unroll
                     for (int f = 0; f < FT; ++f) {
                         acc[c][f].x = fmaf(a[f], b.x, acc[c][f].x); acc[c][f].y = fmaf(a[f], b.y, acc[c][f].y);
@@ -96,6 +115,7 @@ __global__ void __launch_bounds__(256) dm_phase_kernel(const float *__restrict__
                 }
             }
         }
+        __syncthreads();                                    /* stage (ch & 1) is refilled two chunks later */
     }
 #pragma unroll
     for (int c = 0; c < MAXQ; ++c) {
@@ -104,13 +124,37 @@ __global__ void __launch_bounds__(256) dm_phase_kernel(const float *__restrict__
 #pragma unroll
             for (int f = 0; f < FT; ++f) {
                 const int t = t0 + fy * FT + f;
-                if (t < T) reinterpret_cast<float4 *>(out + ((size_t)t * nsub + i) * nn)[cq] = acc[c][f];
+                if (t < T) reinterpret_cast<float4 *>(out + ((size_t)t * nsub + i) * NN)[cq] = acc[c][f];
             }
         }
     }
 }
 
-/* any n (n*n not a multiple of 4, or > 256): one thread per output element */
+template <int FT, int NN>
+void launch_dm_phase(shwfs_handle *h, const float *coef, int ldc, int T, float *out, cudaStream_t st)
+{
+    constexpr int TT = 8 * FT;
+    const size_t smem = 2 * sizeof(float) * (size_t)(DM_MC * NN + DM_MC * (TT + 4));
+    dm_phase_kernel<FT, NN><<<dim3((unsigned)((T + TT - 1) / TT), (unsigned)h->nsub), 256, smem, st>>>(
+        coef, ldc, h->d_dm_modes, T, h->nsub, h->dm_M, out);
+}
+
+template <int NN>
+__global__ void dm_phase_gemv_kernel(const float *__restrict__ coef, int ldc, const float *__restrict__ modes_sub,
+                                     int T, int nsub, int M, float *__restrict__ out);
+
+template <int NN>
+void launch_dm_phase_n(shwfs_handle *h, const float *coef, int ldc, int T, float *out, cudaStream_t st)
+{
+    if (T <= 8 && (size_t)h->dm_M * 8 * sizeof(float) <= 48 * 1024) {
+        dm_phase_gemv_kernel<NN><<<(unsigned)((h->nsub + 7) / 8), 256, sizeof(float) * 8 * (size_t)h->dm_M, st>>>(
+            coef, ldc, h->d_dm_modes, T, h->nsub, h->dm_M, out);
+    } else if (T <= 8) launch_dm_phase<1, NN>(h, coef, ldc, T, out, st);
+    else if (T <= 32) launch_dm_phase<4, NN>(h, coef, ldc, T, out, st);
+    else launch_dm_phase<8, NN>(h, coef, ldc, T, out, st);
+}
+
+/* any other n: one thread per output element */
 __global__ void dm_phase_simple_kernel(const float *__restrict__ coef, int ldc, const float *__restrict__ modes_sub,
                                        int T, int nsub, int nn, int M, float *__restrict__ out)
 {
@@ -123,26 +167,76 @@ __global__ void dm_phase_simple_kernel(const float *__restrict__ coef, int ldc, 
     out[idx] = acc;
 }
 
-/* coef[t][m] += gain * sum_k R[m][k] * s[t][k].  One warp per mode m; frames in tiles of TT so that a row of
- * R is read once per tile.  hist (optional, T == 1 only): hist[m] = coef[m] BEFORE the update (reading C4). */
-constexpr int RC_WARPS = 4;
+/* Few frames (the T = 1 loop step): the product is a matrix-vector one, bound by streaming the mode table
+ * once.  One warp per subaperture, lane = float4 column, eight independent 16-byte loads in flight per lane,
+ * the coefficients of the <= 8 frames broadcast from shared memory.                                      */
+template <int NN>
+__global__ void __launch_bounds__(256) dm_phase_gemv_kernel(const float *__restrict__ coef, int ldc,
+                                                            const float *__restrict__ modes_sub, int T, int nsub,
+                                                            int M, float *__restrict__ out)
+{
+    constexpr int NQ = NN / 4, MAXQ = (NQ + 31) / 32, FMAX = 8, UN = 8;
+    extern __shared__ float gv_coef[];                       /* [M][FMAX] */
+    for (int q = threadIdx.x; q < M * FMAX; q += 256) {
+        const int m = q / FMAX, f = q - m * FMAX;
+        gv_coef[q] = f < T ? __ldg(coef + (size_t)f * ldc + m) : 0.f;
+    }
+    __syncthreads();
+    const int i = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (i >= nsub) return;
+    const float4 *mi = reinterpret_cast<const float4 *>(modes_sub + (size_t)i * M * NN);
+#pragma unroll
+    for (int c = 0; c < MAXQ; ++c) {
+        const int cq = lane + 32 * c;
+        if (cq >= NQ) continue;
+        float4 acc[FMAX];
+#pragma unroll
+        for (int f = 0; f < FMAX; ++f) acc[f] = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int m0 = 0; m0 < M; m0 += UN) {
+            float4 b[UN];
+#pragma unroll
+            for (int u = 0; u < UN; ++u)
+                b[u] = m0 + u < M ? __ldg(mi + (size_t)(m0 + u) * NQ + cq) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int u = 0; u < UN; ++u) {
+                if (m0 + u < M) {
+                    const float *a = gv_coef + (m0 + u) * FMAX;
+#pragma unroll
+                    for (int f = 0; f < FMAX; ++f) {
+                        if (f < T) {
+                            acc[f].x = fmaf(a[f], b[u].x, acc[f].x); acc[f].y = fmaf(a[f], b[u].y, acc[f].y);
+                            acc[f].z = fmaf(a[f], b[u].z, acc[f].z); acc[f].w = fmaf(a[f], b[u].w, acc[f].w);
+                        }
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int f = 0; f < FMAX; ++f)
+            if (f < T) reinterpret_cast<float4 *>(out + ((size_t)f * nsub + i) * NN)[cq] = acc[f];
+    }
+}
+
+/* coef[t][m] += gain * sum_k R[m][k] * s[t][k].  One CTA per mode m, its 256 threads split the row of R
+ * (8-byte loads, frames in register tiles of RC_TT so that the row is read once per tile), warp-shuffle then
+ * shared-memory reduction.  hist (optional): hist[t][m] = coef[t][m] BEFORE the update (reading C4).     */
+constexpr int RC_THREADS = 256;
 constexpr int RC_TT = 8;
 
-__global__ void __launch_bounds__(32 * RC_WARPS) recon_kernel(const float *__restrict__ R,
-                                                              const float *__restrict__ s, int T, int K, int M,
-                                                              float gain, float *__restrict__ coef, int ldc,
-                                                              float *__restrict__ hist)
+__global__ void __launch_bounds__(RC_THREADS) recon_kernel(const float *__restrict__ R, const float *__restrict__ s,
+                                                           int T, int K, int M, float gain,
+                                                           float *__restrict__ coef, int ldc, float *__restrict__ hist)
 {
-    const int lane = threadIdx.x & 31;
-    const int m = blockIdx.x * RC_WARPS + (threadIdx.x >> 5);
-    if (m >= M) return;
+    __shared__ float part[RC_THREADS / 32][RC_TT];
+    const int m = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const float2 *row = reinterpret_cast<const float2 *>(R + (size_t)m * K);
     const int K2 = K >> 1;                                   /* K = 2 * nsub is even */
     for (int t0 = 0; t0 < T; t0 += RC_TT) {
         float acc[RC_TT];
 #pragma unroll
         for (int q = 0; q < RC_TT; ++q) acc[q] = 0.f;
-        for (int k = lane; k < K2; k += 32) {
+#pragma unroll 4
+        for (int k = tid; k < K2; k += RC_THREADS) {
             const float2 r = __ldg(row + k);
 #pragma unroll
             for (int q = 0; q < RC_TT; ++q) {
@@ -157,16 +251,20 @@ __global__ void __launch_bounds__(32 * RC_WARPS) recon_kernel(const float *__res
 #pragma unroll
             for (int o = 16; o >= 1; o >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
         }
+        __syncthreads();                                     /* previous tile's partials are consumed */
         if (lane == 0) {
 #pragma unroll
-            for (int q = 0; q < RC_TT; ++q) {
-                if (t0 + q < T) {
-                    float *c = coef + (size_t)(t0 + q) * ldc + m;
-                    const float old = *c;
-                    if (hist) hist[(size_t)(t0 + q) * M + m] = old;
-                    *c = fmaf(gain, acc[q], old);
-                }
-            }
+            for (int q = 0; q < RC_TT; ++q) part[warp][q] = acc[q];
+        }
+        __syncthreads();
+        if (tid < RC_TT && t0 + tid < T) {
+            float d = 0.f;
+#pragma unroll
+            for (int w = 0; w < RC_THREADS / 32; ++w) d += part[w][tid];
+            float *c = coef + (size_t)(t0 + tid) * ldc + m;
+            const float old = *c;
+            if (hist) hist[(size_t)(t0 + tid) * M + m] = old;
+            *c = fmaf(gain, d, old);
         }
     }
 }
@@ -183,15 +281,11 @@ cudaError_t shwfs_loop_relayout_modes(shwfs_handle *h, const float *modes_dev, i
 cudaError_t shwfs_loop_dm_phase(shwfs_handle *h, const float *coef, int ldc, int T, float *out, cudaStream_t st)
 {
     const int nn = h->n * h->n, M = h->dm_M;
-    if (nn % 4 == 0 && nn <= 256) {
-        if (T <= 8) {
-            const size_t smem = sizeof(float) * (size_t)(DM_MC * nn + DM_MC * 8);
-            dm_phase_kernel<1><<<dim3((unsigned)h->nsub, (unsigned)((T + 7) / 8)), 256, smem, st>>>(
-                coef, ldc, h->d_dm_modes, T, h->nsub, nn, M, out);
-        } else {
-            const size_t smem = sizeof(float) * (size_t)(DM_MC * nn + DM_MC * 32);
-            dm_phase_kernel<4><<<dim3((unsigned)h->nsub, (unsigned)((T + 31) / 32)), 256, smem, st>>>(
-                coef, ldc, h->d_dm_modes, T, h->nsub, nn, M, out);
+    if (h->nsub <= 65535 && (nn == 64 || nn == 100 || nn == 256)) {
+        switch (nn) {
+        case 64: launch_dm_phase_n<64>(h, coef, ldc, T, out, st); break;
+        case 100: launch_dm_phase_n<100>(h, coef, ldc, T, out, st); break;
+        default: launch_dm_phase_n<256>(h, coef, ldc, T, out, st); break;
         }
     } else {
         const size_t total = (size_t)T * h->nsub * nn;
@@ -204,6 +298,6 @@ cudaError_t shwfs_loop_dm_phase(shwfs_handle *h, const float *coef, int ldc, int
 cudaError_t shwfs_loop_reconstruct(const float *R, const float *slopes, int T, int K, int M, float gain,
                                    float *coef, int ldc, float *hist, cudaStream_t st)
 {
-    recon_kernel<<<(M + RC_WARPS - 1) / RC_WARPS, 32 * RC_WARPS, 0, st>>>(R, slopes, T, K, M, gain, coef, ldc, hist);
+    recon_kernel<<<M, RC_THREADS, 0, st>>>(R, slopes, T, K, M, gain, coef, ldc, hist);
     return cudaGetLastError();
 }
