@@ -394,3 +394,114 @@ def from_config(cfg, wfs: int = 0, *, kernels="auto", **overrides) -> "Shwfs":
     elif kernels is not None and not isinstance(kernels, str):
         k = kernels
     return Shwfs(amp, cfg.S, cfg.n, cfg.dx, W.LAMBDA_M, cfg.P, cfg.b, elong_kernels=k, **kw)
+
+
+# ---- pyramid wavefront sensor (include/pyrwfs.h) -------------------------------------------------------
+
+PYR_EXPORTS = ["pyrwfs_create", "pyrwfs_destroy", "pyrwfs_num_pixels", "pyrwfs_valid_list", "pyrwfs_launch_count",
+               "pyrwfs_measure", "pyrwfs_debug_quadrants"]
+
+
+class PyrwfsConfig(C.Structure):
+    """struct pyrwfs_config of include/pyrwfs.h (field order and types must match)."""
+    _fields_ = [("n_pupil", C.c_int32), ("amplitude", C.POINTER(C.c_float)), ("min_illum", C.c_float),
+                ("pad", C.c_int32), ("separation", C.c_int32), ("bin", C.c_int32), ("mod_radius", C.c_float),
+                ("mod_points", C.c_int32), ("pupil_diameter_px", C.c_float), ("phase_to_rad", C.c_float)]
+
+
+def _pyr_lib():
+    L = load()
+    if not getattr(L, "_pyr_ready", False):
+        vp, i32 = C.c_void_p, C.c_int32
+        L.pyrwfs_create.argtypes = [C.POINTER(PyrwfsConfig), C.POINTER(vp)]
+        L.pyrwfs_destroy.argtypes = [vp]
+        L.pyrwfs_num_pixels.argtypes = [vp, C.POINTER(i32)]
+        L.pyrwfs_valid_list.argtypes = [vp, vp]
+        L.pyrwfs_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
+        L.pyrwfs_measure.argtypes = [vp, vp, i32, vp, vp]
+        L.pyrwfs_debug_quadrants.argtypes = [vp, vp, i32, vp, vp]
+        for name in PYR_EXPORTS:
+            getattr(L, name).restype = C.c_int
+        L._pyr_ready = True
+    return L
+
+
+class Pyrwfs:
+    """One pyramid sensor (one handle).  See include/pyrwfs.h for the meaning of every argument."""
+
+    def __init__(self, amplitude, pad: int, separation: int, bin: int, mod_radius: float, mod_points: int,
+                 pupil_diameter_px: float, *, min_illum: float = 0.5, phase_to_rad: float = 1.0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1408_0698_b200 needs a CUDA device (no CPU fallback)")
+        torch.empty(1, device="cuda")
+        amp = np.ascontiguousarray(amplitude, dtype=np.float32)
+        if amp.ndim != 2 or amp.shape[0] != amp.shape[1]:
+            raise ValueError("amplitude must be [N,N]")
+        cfg = PyrwfsConfig(amp.shape[0], amp.ctypes.data_as(C.POINTER(C.c_float)), min_illum, pad, separation, bin,
+                           mod_radius, mod_points, pupil_diameter_px, phase_to_rad)
+        out = C.c_void_p()
+        self._h = None
+        _check(_pyr_lib().pyrwfs_create(C.byref(cfg), C.byref(out)), "pyrwfs_create")
+        self._h = out.value
+        self.N, self.Np, self.s, self.bp, self.Sp = amp.shape[0], pad, separation, bin, amp.shape[0] // bin
+        nv = C.c_int32()
+        _check(_pyr_lib().pyrwfs_num_pixels(self._h, C.byref(nv)), "pyrwfs_num_pixels")
+        self.nvalid = nv.value
+
+    @property
+    def valid_yx(self) -> np.ndarray:
+        out = np.zeros((self.nvalid, 2), dtype=np.int32)
+        _check(_pyr_lib().pyrwfs_valid_list(self._h, out.ctypes.data_as(C.c_void_p)), "pyrwfs_valid_list")
+        return out
+
+    @property
+    def launch_count(self) -> int:
+        v = C.c_int64()
+        _check(_pyr_lib().pyrwfs_launch_count(self._h, C.byref(v)), "pyrwfs_launch_count")
+        return v.value
+
+    def _check_phase(self, phase):
+        import torch
+        if not (isinstance(phase, torch.Tensor) and phase.is_cuda and phase.dtype == torch.float32
+                and phase.is_contiguous() and tuple(phase.shape[1:]) == (self.N, self.N)):
+            raise ValueError(f"phase must be a contiguous float32 CUDA tensor [T,{self.N},{self.N}]")
+
+    def measure(self, phase, out=None, stream=None):
+        """phase CUDA float32 [T,N,N] -> signals CUDA float32 [T,nvalid,2]."""
+        import torch
+        self._check_phase(phase)
+        T = phase.shape[0]
+        if out is None:
+            out = torch.empty((T, self.nvalid, 2), dtype=torch.float32, device=phase.device)
+        st = (stream if stream is not None else torch.cuda.current_stream(phase.device)).cuda_stream
+        _check(_pyr_lib().pyrwfs_measure(self._h, phase.data_ptr(), T, out.data_ptr(), st), "pyrwfs_measure")
+        return out
+
+    def debug_quadrants(self, phase, stream=None):
+        """Binned quadrant images Q [T,2,2,Sp,Sp] (parity only)."""
+        import torch
+        self._check_phase(phase)
+        T = phase.shape[0]
+        out = torch.empty((T, 2, 2, self.Sp, self.Sp), dtype=torch.float32, device=phase.device)
+        st = (stream if stream is not None else torch.cuda.current_stream(phase.device)).cuda_stream
+        _check(_pyr_lib().pyrwfs_debug_quadrants(self._h, phase.data_ptr(), T, out.data_ptr(), st),
+               "pyrwfs_debug_quadrants")
+        return out
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _check(_pyr_lib().pyrwfs_destroy(self._h), "pyrwfs_destroy")
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()

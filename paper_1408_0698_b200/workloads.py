@@ -241,6 +241,47 @@ def dm_modes_device(c: WfsConfig, M: int, device):
     return out
 
 
+@dataclass(frozen=True)
+class PyramidConfig:
+    """Pyramid-WFS workload.  PAPER.md:96 describes the paper's pyramid test case on the
+    LBT: "a 400 modes correction using a modulated (3 lambda/D) pyramid on a seeing of 1 arcsec"; the LBT
+    pyramid has 30 x 30 subapertures on an 8.2 m pupil with an 11 % central obstruction."""
+    name: str
+    N: int              # pupil grid side (the pupil diameter spans it)
+    dx: float           # metres per pupil pixel
+    Np: int             # padded transform side
+    s: int              # pupil-copy separation
+    bp: int             # pupil pixels per detector pixel
+    r_mod: float        # lambda / D
+    K: int              # modulation points
+    obstruction: float  # linear central obstruction
+    screen_cfg: int     # WfsConfig whose screen recipe (grid, seeds) the frames come from
+
+    @property
+    def D_pix(self) -> float:
+        return float(self.N)
+
+
+PYRAMIDS = {
+    "tiny": PyramidConfig("tiny", 48, 0.17, 256, 64, 4, 3.0, 8, 0.11, 1),
+    "lbt": PyramidConfig("lbt", 240, 8.2 / 240, 1024, 256, 8, 3.0, 16, 0.11, 2),
+}
+
+
+def pyramid_mask(p: PyramidConfig) -> np.ndarray:
+    ax = np.arange(p.N, dtype=np.float64) + 0.5 - p.N / 2.0
+    r = np.hypot(ax[None, :], ax[:, None])
+    return ((r <= p.N / 2.0) & (r >= p.obstruction * p.N / 2.0)).astype(np.float32)
+
+
+def pyramid_frames(p: PyramidConfig, frames, scale: float = 1.0) -> np.ndarray:
+    """Seeded von Karman frames for the pyramid ([T,N,N] fp32): the screen recipe of config `screen_cfg`
+    (phase_screen, "WFS" 800), cropped to N x N and multiplied by `scale` (closed-loop residuals are a
+    fraction of the open-loop turbulence)."""
+    c = CONFIGS[p.screen_cfg]
+    return np.stack([phase_screen(c, 800, int(t))[: p.N, : p.N] * np.float32(scale) for t in frames], axis=0)
+
+
 def phase_frames_device(c: WfsConfig, wfs: int, frames, device, out=None):
     """Same von Karman recipe as phase_screen, evaluated with torch on `device` (float64 FFT, cast to fp32).
 

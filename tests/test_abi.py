@@ -32,7 +32,7 @@ def test_library_exports_every_declared_symbol(libshwfs):
 
 
 @pytest.mark.parametrize("cname,pyname", [("shwfs_geometry", "ShwfsGeometry"), ("shwfs_sodium", "ShwfsSodium"),
-                                          ("shwfs_noise", "ShwfsNoise")])
+                                          ("shwfs_noise", "ShwfsNoise"), ("pyrwfs_config", "PyrwfsConfig")])
 def test_ctypes_struct_matches_the_header(tmp_path, cname, pyname):
     """sizeof / offsetof of each ABI struct as gcc sees the header == the ctypes mirror in the binding."""
     from paper_1408_0698_b200 import binding
@@ -40,13 +40,23 @@ def test_ctypes_struct_matches_the_header(tmp_path, cname, pyname):
     fields = [f[0] for f in St._fields_]
     src = tmp_path / "layout.c"
     body = "".join(f'printf("%zu\\n", offsetof({cname}, {f}));' for f in fields)
-    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "shwfs.h"\n'
+    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "shwfs.h"\n#include "pyrwfs.h"\n'
                    f'int main(void){{printf("%zu\\n", sizeof({cname}));' + body + "return 0;}\n")
     exe = tmp_path / "layout"
     subprocess.run(["gcc", "-std=c99", "-I", str(ROOT / "include"), str(src), "-o", str(exe)], check=True)
     out = [int(v) for v in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()]
     assert out[0] == C.sizeof(St)
     assert out[1:] == [getattr(St, f).offset for f in fields]
+
+
+def test_library_exports_every_pyramid_symbol(libshwfs):
+    from paper_1408_0698_b200 import binding
+    text = re.sub(r"/\*.*?\*/", "", (ROOT / "include" / "pyrwfs.h").read_text(), flags=re.S)
+    names = sorted(set(re.findall(r"\b(pyrwfs_[a-z_]+)\s*\(", text)))
+    lib = C.CDLL(str(libshwfs))
+    for name in names:
+        assert hasattr(lib, name), f"{name} is declared in include/pyrwfs.h but not exported"
+    assert sorted(binding.PYR_EXPORTS) == names
 
 
 def test_header_compiles_as_c_and_cxx(tmp_path):
