@@ -332,6 +332,71 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_pyramid(args):
+    """Pyramid WFS: frames/s of pyrwfs_measure on a synthetic LBT-like workload, inputs
+    resident in HBM, CUDA events on the launching stream; the numpy oracle on the host cores beside it."""
+    import torch
+    from paper_1408_0698_b200 import binding as B, workloads as W
+    rank, local_rank, world = _dist_env()
+    if rank != 0:
+        return
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    p = W.PYRAMIDS[args.pyramid]
+    amp = W.pyramid_mask(p)
+    T = args.pyramid_frames
+    ph_host = W.pyramid_frames(p, range(min(T, 8)), 0.3)
+    ph = torch.from_numpy(ph_host).to(dev).repeat((T + ph_host.shape[0] - 1) // ph_host.shape[0], 1, 1)[:T].contiguous()
+    stream = torch.cuda.Stream(dev)
+    with B.Pyrwfs(amp, p.Np, p.s, p.bp, p.r_mod, p.K, p.D_pix) as s:
+        out = torch.empty((T, s.nvalid, 2), dtype=torch.float32, device=dev)
+        for _ in range(max(args.warmup, 3)):
+            s.measure(ph, out=out, stream=stream)
+        torch.cuda.synchronize(dev)
+        sampler = ClockSampler(local_rank)
+        l0 = s.launch_count
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sampler.start()
+        e0.record(stream)
+        for _ in range(args.steps):
+            s.measure(ph, out=out, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        clocks = sampler.stop()
+        ms = e0.elapsed_time(e1)
+        launches = s.launch_count - l0
+        nvalid = s.nvalid
+    value = T * args.steps / (ms * 1e-3)
+    Kp = max(p.K, 1)
+    lg = int(np.log2(p.Np))
+    # nominal flops per frame: per modulation point N pruned row lines, Np columns x 2 transforms, 2N output rows
+    lines = Kp * (p.N + 2 * p.Np + 2 * p.N)
+    flops = lines * 5 * p.Np * lg
+    ach = flops * value / 1e12
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import pyramid as OP
+        yx = OP.valid_pixels(amp, p.bp)
+        nfr = max(1, min(args.cpu_frames, 4))
+        t0 = time.perf_counter()
+        OP.measure(ph_host[:nfr], amp, yx, p.Np, p.s, p.bp, p.r_mod, p.K, p.D_pix)
+        dt = time.perf_counter() - t0
+        cpu = {"value": nfr / dt, "unit": "frames/s", "cores": 1, "kind": "oracle",
+               "sample": f"{nfr} frame(s), numpy fft2 oracle, {dt:.1f} s"}
+    print(json.dumps({
+        "metric": "pyramid_wfs_frames_per_s", "value": value, "unit": "frames/s", "n_gpus": 1, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"pyramid '{p.name}': pupil {p.N} px, pad {p.Np}, separation {p.s}, {p.bp}x{p.bp} binning "
+                               f"to {p.N // p.bp}x{p.N // p.bp}, modulation {p.r_mod:g} lambda/D in {p.K} points, "
+                               f"{nvalid} valid pixels, {T}-frame batches"},
+        "clocks": clocks, "e2e": None, "gpu_launches": int(launches),
+        "roofline": {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                     "frac": ach / FP32_PEAK_TFLOPS, "traffic": None, "kernel": "pyr_cols_kernel (+ rows, final)",
+                     "flops_per_frame": flops, "flops_basis": "5 L log2 L per line of the pruned passes (DESIGN.md 14)"},
+        "cpu_baseline": cpu}))
+
+
 def _hbm_peak():
     try:
         return float(json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["hbm_gbs"])
@@ -387,10 +452,15 @@ def main():
     ap.add_argument("--read-noise", type=float, default=3.0)
     ap.add_argument("--dm-modes", type=int, default=0,
                     help="M > 0: subtract a DM of M modes inside the gather (8(f) f3, shwfs_measure_residual)")
+    ap.add_argument("--pyramid", default=None, choices=["tiny", "lbt"],
+                    help="time the pyramid WFS (8(f) f4) on this workloads.PYRAMIDS entry instead of the SH path")
+    ap.add_argument("--pyramid-frames", type=int, default=32)
     ap.add_argument("--closed-loop", action="store_true",
                     help="with --dm-modes: run the batch as sequential pure-integrator frames (shwfs_closed_loop)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.pyramid:
+        run_pyramid(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
