@@ -166,7 +166,7 @@ __global__ void __launch_bounds__(PY_LINES * R) pyr_rows_kernel(const PyArgs A)
 
 /* ---- column half of Q2, Q3 mask, column half of Q4: grid (Np/8, Tc*Kp) ---------------------------------- */
 template <int R>
-__global__ void __launch_bounds__(PY_LINES * R) pyr_cols_kernel(const PyArgs A)
+__global__ void __launch_bounds__(PY_LINES * R, 2) pyr_cols_kernel(const PyArgs A)
 {
     constexpr int L = R * R, NZ = R / 2;
     extern __shared__ __align__(16) float2 py_smem[];
@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(PY_LINES * R) pyr_cols_kernel(const PyArgs A)
 
 /* ---- row half of Q4, |.|^2, Q5: grid (2N/8 rounded up, Tc) ---------------------------------------------- */
 template <int R>
-__global__ void __launch_bounds__(PY_LINES * R) pyr_final_kernel(const PyArgs A)
+__global__ void __launch_bounds__(PY_LINES * R, 2) pyr_final_kernel(const PyArgs A)
 {
     constexpr int L = R * R;
     extern __shared__ __align__(16) float2 py_smem[];
