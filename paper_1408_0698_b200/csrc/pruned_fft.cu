@@ -6,7 +6,8 @@
  * Steps H1 gather, H2 field, H3 zero-padded P x P DFT, H4 |.|^2/P^2, H6 centre + b x b bin, H7 threshold,
  * H8 centre of gravity of include/shwfs.h, D = P/b = 16 detector pixels per side.
  *
- * Thread mapping: 16 threads (a half-warp) per spot, 8 spots per CTA, no CTA-wide barrier.
+ * Thread mapping: 16 threads (a half-warp) per spot, 8 spots per tile, 4 tiles per CTA (the gather of the next
+ * tile is issued before the column pass of the current one), no CTA-wide barrier.
  *   row pass     thread r < n owns patch row r: 8-byte gathers, sincos, one P-point DIF FFT in registers
  *                whose inputs >= NZ are known zeros (first stage free); the n x P result goes to shared
  *                memory with the columns permuted (u -> (u mod b) * 16 + u / b) so that the column pass
@@ -55,6 +56,26 @@ struct PfCfg {
 template <int P>
 __host__ __device__ constexpr int col_pos(int u) { return (u % (P / 16)) * 16 + u / (P / 16); }
 
+/* H1 of one spot row: the NZ/2 pixel pairs of patch row r of spot g (zeros when the row does not exist) */
+template <int NZ>
+__device__ __forceinline__ void pf_gather(const PfArgs &A, int g, int r, float2 (&ph)[NZ / 2], float2 (&am)[NZ / 2])
+{
+#pragma unroll
+    for (int q = 0; q < NZ / 2; ++q) { ph[q] = make_float2(0.f, 0.f); am[q] = make_float2(0.f, 0.f); }
+    if (g < A.total && r < A.n) {
+        const int i = g / A.T, t = g - i * A.T;
+        const int2 yx = A.valid[i];
+        const size_t o = (size_t)(yx.x * A.n + r) * A.N + (size_t)yx.y * A.n;
+        const float2 *pp = reinterpret_cast<const float2 *>(A.phase + (size_t)t * A.frame_stride + o);
+        const float2 *pa = reinterpret_cast<const float2 *>(A.amp + o);
+#pragma unroll
+        for (int q = 0; q < NZ / 2; ++q)
+            if (2 * q < A.n) { ph[q] = __ldg(pp + q); am[q] = __ldg(pa + q); }
+    }
+}
+
+constexpr int PF_TILES = 4;     /* tiles of 8 spots per CTA: the gather of tile k+1 flies during the column pass of k */
+
 template <int P, int NZ, int MODE>
 __global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel(const PfArgs A)
 {
@@ -64,91 +85,90 @@ __global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel
     const int tid = threadIdx.x, sp = tid >> 4, r = tid & 15;
     float *tile = pf_smem + sp * Cfg::TILE;
 
-    const int g = blockIdx.x * PF_SPOTS + sp;
-    const bool live = g < A.total;
-    int i = 0, t = 0;
-    if (live) { i = g / A.T; t = g - i * A.T; }
+    float2 ph[NZ / 2], am[NZ / 2];
+    pf_gather<NZ>(A, (blockIdx.x * PF_TILES) * PF_SPOTS + sp, r, ph, am);
 
-    float re[P], im[P];
+#pragma unroll 1
+    for (int it = 0; it < PF_TILES; ++it) {
+        const int g = (blockIdx.x * PF_TILES + it) * PF_SPOTS + sp;
+        const bool live = g < A.total;
+        int i = 0, t = 0;
+        if (live) { i = g / A.T; t = g - i * A.T; }
 
-    /* ---- row pass: H1 gather, H2 field, P-point FFT of row r (inputs >= NZ are zero) ---- */
-    if (r < NZ) {
-        if (live && r < A.n) {
-            const int2 yx = A.valid[i];
-            const size_t o = (size_t)(yx.x * A.n + r) * A.N + (size_t)yx.y * A.n;
-            const float2 *pp = reinterpret_cast<const float2 *>(A.phase + (size_t)t * A.frame_stride + o);
-            const float2 *pa = reinterpret_cast<const float2 *>(A.amp + o);
-            float2 ph[NZ / 2], am[NZ / 2];
+        float re[P], im[P];
+
+        /* ---- row pass: H2 field, P-point FFT of row r (inputs >= NZ are zero) ---- */
+        if (r < NZ) {
+            if (live && r < A.n) {
 #pragma unroll
-            for (int q = 0; q < NZ / 2; ++q) {
-                ph[q] = make_float2(0.f, 0.f); am[q] = make_float2(0.f, 0.f);
-                if (2 * q < A.n) { ph[q] = __ldg(pp + q); am[q] = __ldg(pa + q); }
+                for (int q = 0; q < NZ / 2; ++q) {
+                    const float ramp = (float)(r + 2 * q) * A.ramp_unit;
+                    const float2 e0 = field_value(ph[q].x, am[q].x, A.turns, ramp);
+                    const float2 e1 = field_value(ph[q].y, am[q].y, A.turns, ramp + A.ramp_unit);
+                    re[2 * q] = e0.x; im[2 * q] = e0.y;
+                    re[2 * q + 1] = e1.x; im[2 * q + 1] = e1.y;
+                }
+#pragma unroll
+                for (int k = NZ; k < P; ++k) { re[k] = 0.f; im[k] = 0.f; }
+                fft_dif<P, -1, NZ>(re, im);
+            } else {
+#pragma unroll
+                for (int k = 0; k < P; ++k) { re[k] = 0.f; im[k] = 0.f; }
+            }
+            float4 *row = reinterpret_cast<float4 *>(tile + r * LD);
+#pragma unroll
+            for (int q = 0; q < P / 2; ++q) {
+                /* stored positions 2q, 2q+1 hold columns u0, u1 (inverse of col_pos) */
+                const int p0 = 2 * q, p1 = 2 * q + 1;
+                const int u0 = (p0 % 16) * b + p0 / 16, u1 = (p1 % 16) * b + p1 / 16;
+                const int x0 = fft_out_index<P>(u0), x1 = fft_out_index<P>(u1);
+                row[q] = make_float4(re[x0], im[x0], re[x1], im[x1]);
+            }
+        }
+        __syncwarp();
+        /* H1 of the next tile: in flight during the column pass */
+        if (it + 1 < PF_TILES) pf_gather<NZ>(A, g + PF_SPOTS, r, ph, am);
+
+        /* ---- column pass: b columns per thread, |.|^2 and the row half of the bin in registers ---- */
+        float acc[16];
+#pragma unroll
+        for (int R = 0; R < 16; ++R) acc[R] = 0.f;
+#pragma unroll
+        for (int be = 0; be < b; ++be) {
+            const float2 *colp = reinterpret_cast<const float2 *>(tile) + be * 16 + r;
+#pragma unroll
+            for (int v = 0; v < NZ; ++v) {
+                const float2 f = colp[v * (LD / 2)];
+                re[v] = f.x; im[v] = f.y;
             }
 #pragma unroll
-            for (int q = 0; q < NZ / 2; ++q) {
-                const float ramp = (float)(r + 2 * q) * A.ramp_unit;
-                const float2 e0 = field_value(ph[q].x, am[q].x, A.turns, ramp);
-                const float2 e1 = field_value(ph[q].y, am[q].y, A.turns, ramp + A.ramp_unit);
-                re[2 * q] = e0.x; im[2 * q] = e0.y;
-                re[2 * q + 1] = e1.x; im[2 * q + 1] = e1.y;
-            }
-#pragma unroll
-            for (int k = NZ; k < P; ++k) { re[k] = 0.f; im[k] = 0.f; }
+            for (int v = NZ; v < P; ++v) { re[v] = 0.f; im[v] = 0.f; }
             fft_dif<P, -1, NZ>(re, im);
-        } else {
 #pragma unroll
-            for (int k = 0; k < P; ++k) { re[k] = 0.f; im[k] = 0.f; }
-        }
-        float4 *row = reinterpret_cast<float4 *>(tile + r * LD);
+            for (int R = 0; R < 16; ++R) {
 #pragma unroll
-        for (int q = 0; q < P / 2; ++q) {
-            /* stored positions 2q, 2q+1 hold columns u0, u1 (inverse of col_pos) */
-            const int p0 = 2 * q, p1 = 2 * q + 1;
-            const int u0 = (p0 % 16) * b + p0 / 16, u1 = (p1 % 16) * b + p1 / 16;
-            const int x0 = fft_out_index<P>(u0), x1 = fft_out_index<P>(u1);
-            row[q] = make_float4(re[x0], im[x0], re[x1], im[x1]);
-        }
-    }
-    __syncwarp();
-
-    /* ---- column pass: b columns per thread, |.|^2 and the row half of the bin in registers ---- */
-    float acc[16];
-#pragma unroll
-    for (int R = 0; R < 16; ++R) acc[R] = 0.f;
-#pragma unroll
-    for (int be = 0; be < b; ++be) {
-        const float2 *colp = reinterpret_cast<const float2 *>(tile) + be * 16 + r;
-#pragma unroll
-        for (int v = 0; v < NZ; ++v) {
-            const float2 f = colp[v * (LD / 2)];
-            re[v] = f.x; im[v] = f.y;
-        }
-#pragma unroll
-        for (int v = NZ; v < P; ++v) { re[v] = 0.f; im[v] = 0.f; }
-        fft_dif<P, -1, NZ>(re, im);
-#pragma unroll
-        for (int R = 0; R < 16; ++R) {
-#pragma unroll
-            for (int al = 0; al < b; ++al) {
-                const int x = fft_out_index<P>((R * b + al) ^ HP);      /* H6: roll by P/2, then bin */
-                acc[R] = fmaf(re[x], re[x], fmaf(im[x], im[x], acc[R]));
+                for (int al = 0; al < b; ++al) {
+                    const int x = fft_out_index<P>((R * b + al) ^ HP);      /* H6: roll by P/2, then bin */
+                    acc[R] = fmaf(re[x], re[x], fmaf(im[x], im[x], acc[R]));
+                }
             }
         }
-    }
-    constexpr float inv_pp = 1.0f / ((float)P * (float)P);
+        constexpr float inv_pp = 1.0f / ((float)P * (float)P);
 #pragma unroll
-    for (int R = 0; R < 16; ++R) acc[R] *= inv_pp;
+        for (int R = 0; R < 16; ++R) acc[R] *= inv_pp;
 
-    /* ---- H7 + H8: thread r holds detector column C = r ^ 8 ---- */
-    const int C = r ^ 8;
-    const float2 sl = cog16<MODE>(acc, C, A.tau);
-    if (live) {
-        const size_t o = (size_t)t * A.nsub + i;
-        if (r == 0) reinterpret_cast<float2 *>(A.slopes)[o] = sl;
-        if (A.binned) {
+        /* ---- H7 + H8: thread r holds detector column C = r ^ 8 ---- */
+        const int C = r ^ 8;
+        const float2 sl = cog16<MODE>(acc, C, A.tau);
+        if (live) {
+            const size_t o = (size_t)t * A.nsub + i;
+            if (r == 0) reinterpret_cast<float2 *>(A.slopes)[o] = sl;
+            if (A.binned) {
 #pragma unroll
-            for (int R = 0; R < 16; ++R) A.binned[(o * 16 + R) * 16 + C] = acc[R];
+                for (int R = 0; R < 16; ++R) A.binned[(o * 16 + R) * 16 + C] = acc[R];
+            }
         }
+        __syncwarp();                                      /* the tile is rewritten by the next row pass */
     }
 }
 
@@ -161,7 +181,7 @@ cudaError_t launch_pf_mode(const PfArgs &A, cudaStream_t st)
                                              (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
     }
-    const int grid = (A.total + PF_SPOTS - 1) / PF_SPOTS;
+    const int grid = (A.total + PF_SPOTS * PF_TILES - 1) / (PF_SPOTS * PF_TILES);
     pruned_fft_kernel<P, NZ, MODE><<<grid, PF_THREADS, Cfg::SMEM, st>>>(A);
     return cudaGetLastError();
 }
