@@ -319,7 +319,11 @@ def run_ours(args):
                        "l2": f"inputs larger than L2 ({in_bytes / 1e6:.0f} MB read per step), no flush"},
             "wfs_frames_per_s": value / nsub, "system_frames_per_s": value / nsub / c.W,
             "clocks": clocks,
-            "e2e": {"value": e2e_value, "unit": "spots/s", "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes,
+            "e2e": {"value": e2e_value, "unit": "spots/s",
+                    "h2d_bytes_per_step": sum(s.host_bytes_per_frame * (p.numel() // (c.N * c.N)) for s, p in zip(sensors, phase)),
+                    "h2d_note": "only the column runs of valid subapertures cross the bus (shwfs_host_bytes_per_frame); "
+                                f"the pinned host tensors hold {in_bytes} bytes",
+                    "d2h_bytes_per_step": out_bytes,
                     "steps": e2e_steps, "api": "shwfs_measure_host", "max_abs_diff_vs_device_path": e2e_check},
             "gpu_launches": int(launches),
             "roofline": roofline,

@@ -99,6 +99,11 @@ int shwfs_measure(shwfs_handle *h, const float *phase_dev, int32_t T, float *slo
  * slopes have landed in slopes_host.  This is the end-to-end entry point timed as "e2e" by bench.py.   */
 int shwfs_measure_host(shwfs_handle *h, const float *phase_host, int32_t T, float *slopes_host);
 
+/* Bytes of one N x N wavefront that shwfs_measure_host actually moves to the device: only the bounding column
+ * extent of the valid subapertures of each lenslet row is copied (strided 3-D copies, rows of equal extent
+ * merged) when that saves at least a tenth of the frame; the rest is never read by H1.                  */
+int shwfs_host_bytes_per_frame(const shwfs_handle *h, int64_t *bytes);
+
 /* Frees everything the handle owns.  shwfs_destroy(NULL) returns 0. */
 int shwfs_destroy(shwfs_handle *h);
 

@@ -26,7 +26,7 @@ EXPORTS = ["shwfs_create", "shwfs_measure", "shwfs_measure_host", "shwfs_destroy
            "shwfs_valid_list", "shwfs_pixel_scale", "shwfs_set_algorithm", "shwfs_get_algorithm",
            "shwfs_launch_count", "shwfs_debug_spots", "shwfs_strerror", "shwfs_last_cuda_error",
            "shwfs_version", "shwfs_set_sodium", "shwfs_set_noise", "shwfs_set_dm",
-           "shwfs_measure_residual", "shwfs_reconstruct", "shwfs_closed_loop"]
+           "shwfs_measure_residual", "shwfs_reconstruct", "shwfs_closed_loop", "shwfs_host_bytes_per_frame"]
 SHWFS_MAX_LAYERS = 8
 
 
@@ -88,6 +88,7 @@ def load():
     L.shwfs_set_sodium.argtypes = [vp, C.POINTER(ShwfsSodium)]
     L.shwfs_set_noise.argtypes = [vp, C.POINTER(ShwfsNoise)]
     L.shwfs_set_dm.argtypes = [vp, vp, i32]
+    L.shwfs_host_bytes_per_frame.argtypes = [vp, C.POINTER(i64)]
     L.shwfs_measure_residual.argtypes = [vp, vp, vp, i32, vp, vp]
     L.shwfs_reconstruct.argtypes = [vp, vp, vp, i32, C.c_float, vp, vp]
     L.shwfs_closed_loop.argtypes = [vp, vp, vp, C.c_float, vp, i32, vp, vp, vp]
@@ -205,6 +206,13 @@ class Shwfs:
     def launch_count(self) -> int:
         v = C.c_int64()
         _check(load().shwfs_launch_count(self._h, C.byref(v)), "shwfs_launch_count")
+        return v.value
+
+    @property
+    def host_bytes_per_frame(self) -> int:
+        """Bytes of one wavefront that measure_host moves over the bus (valid column runs only)."""
+        v = C.c_int64()
+        _check(load().shwfs_host_bytes_per_frame(self._h, C.byref(v)), "shwfs_host_bytes_per_frame")
         return v.value
 
     # -- the paper's full LGS model (include/shwfs.h: shwfs_set_sodium, shwfs_set_noise)

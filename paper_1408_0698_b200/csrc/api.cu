@@ -52,6 +52,7 @@ void free_handle(shwfs_handle *h)
     if (h->st_copy) cudaStreamDestroy(h->st_copy);
     if (h->st_comp) cudaStreamDestroy(h->st_comp);
     free(h->h_valid);
+    free(h->h_runs);
     if (prev >= 0 && prev != h->device) cudaSetDevice(prev);
     delete h;
     cudaGetLastError();
@@ -155,6 +156,35 @@ int shwfs_create(const shwfs_geometry *g, float lambda_m, int32_t pad, int32_t b
     h->mode = g->threshold_mode; h->has_kernels = elong_kernels != nullptr;
     h->h_valid = valid;
     h->chunk_frames = 0;
+    {   /* bounding column extent of the valid subapertures of each lenslet row; consecutive rows with the same
+         * extent merge into one band = {first lenslet row, rows, first column, width in pixels} */
+        int *lo = (int *)malloc(sizeof(int) * (size_t)S), *hi = (int *)malloc(sizeof(int) * (size_t)S);
+        int *runs = (int *)malloc(sizeof(int) * 4 * (size_t)S);
+        if (lo && hi && runs) {
+            for (int sy = 0; sy < S; ++sy) { lo[sy] = S; hi[sy] = -1; }
+            for (int i = 0; i < nsub; ++i) {
+                const int sy = valid[2 * i], sx = valid[2 * i + 1];
+                if (sx < lo[sy]) lo[sy] = sx;
+                if (sx > hi[sy]) hi[sy] = sx;
+            }
+            int nr = 0;
+            long long px = 0;
+            for (int sy = 0; sy < S; ++sy) {
+                if (hi[sy] < 0) continue;
+                if (nr > 0 && runs[4 * (nr - 1)] + runs[4 * (nr - 1) + 1] == sy && runs[4 * (nr - 1) + 2] == lo[sy] * n &&
+                    runs[4 * (nr - 1) + 3] == (hi[sy] - lo[sy] + 1) * n) {
+                    runs[4 * (nr - 1) + 1] += 1;
+                } else {
+                    runs[4 * nr] = sy; runs[4 * nr + 1] = 1; runs[4 * nr + 2] = lo[sy] * n; runs[4 * nr + 3] = (hi[sy] - lo[sy] + 1) * n;
+                    ++nr;
+                }
+                px += (long long)(hi[sy] - lo[sy] + 1) * n * n;
+            }
+            /* worth it only if it saves a tenth of the bytes */
+            if (px * 10 <= (long long)N * N * 9) { h->h_runs = runs; h->n_runs = nr; h->run_pixels = px; runs = nullptr; }
+        }
+        free(lo); free(hi); free(runs);
+    }
 
     int rc = SHWFS_OK;
     CU_TRY(cudaGetDevice(&h->device), "cudaGetDevice");
@@ -239,6 +269,13 @@ int shwfs_get_algorithm(const shwfs_handle *h, int32_t *algo)
 {
     if (!h || !algo) return SHWFS_EINVAL;
     *algo = h->algo;
+    return SHWFS_OK;
+}
+
+int shwfs_host_bytes_per_frame(const shwfs_handle *h, int64_t *bytes)
+{
+    if (!h || !bytes) return SHWFS_EINVAL;
+    *bytes = (int64_t)sizeof(float) * (h->n_runs > 0 ? h->run_pixels : (long long)h->N * h->N);
     return SHWFS_OK;
 }
 
@@ -474,7 +511,7 @@ int shwfs_debug_spots(shwfs_handle *h, const float *phase_dev, int32_t T, int32_
 }  // extern "C"
 
 /* ------------------------------------------------------------------------------------------------
- * Host-buffer entry point: frames are cut into chunks of ~64 MiB, copied on st_copy into one of two
+ * Host-buffer entry point: frames are cut into chunks of ~128 MiB, copied on st_copy into one of two
  * device buffers and measured on st_comp, so the H2D copy of chunk c+1 overlaps the kernels of
  * chunk c.  A pinned (cudaHostAlloc / cudaHostRegister) caller buffer is copied from directly; a
  * pageable one goes through the handle's own two pinned staging buffers.
@@ -488,7 +525,7 @@ int host_init(shwfs_handle *h)
     /* one "frame" of the pipeline = one time step = up to SHWFS_MAX_LAYERS wavefronts, so that a later
      * shwfs_set_sodium never outgrows the buffers */
     const size_t frame_bytes = sizeof(float) * (size_t)h->N * h->N;
-    size_t chunk = ((size_t)64 << 20) / frame_bytes;
+    size_t chunk = ((size_t)128 << 20) / frame_bytes;
     if (chunk < SHWFS_MAX_LAYERS) chunk = SHWFS_MAX_LAYERS;
     if (chunk > 256) chunk = 256;
     h->chunk_frames = (int)chunk;
@@ -552,7 +589,24 @@ extern "C" int shwfs_measure_host(shwfs_handle *h, const float *phase_host, int3
                 src = h->h_pin[k];
             }
             CU_TRY(cudaStreamWaitEvent(h->st_copy, h->ev_done[k], 0), "cudaStreamWaitEvent");
-            CU_TRY(cudaMemcpyAsync(h->d_phase[k], src, frame_bytes * tc, cudaMemcpyHostToDevice, h->st_copy), "cudaMemcpyAsync(H2D)");
+            if (h->n_runs > 0) {
+                /* one strided 3-D copy per run: width x n rows x (frames of the chunk); the rest of the frame
+                 * (outside the pupil, central obstruction) never crosses the bus */
+                cudaMemcpy3DParms p;
+                memset(&p, 0, sizeof(p));
+                p.srcPtr = make_cudaPitchedPtr((void *)src, sizeof(float) * (size_t)h->N, (size_t)h->N, (size_t)h->N);
+                p.dstPtr = make_cudaPitchedPtr((void *)h->d_phase[k], sizeof(float) * (size_t)h->N, (size_t)h->N, (size_t)h->N);
+                p.kind = cudaMemcpyHostToDevice;
+                for (int q = 0; q < h->n_runs; ++q) {
+                    const int sy = h->h_runs[4 * q], rows = h->h_runs[4 * q + 1], x0 = h->h_runs[4 * q + 2], w = h->h_runs[4 * q + 3];
+                    p.srcPos = make_cudaPos(sizeof(float) * (size_t)x0, (size_t)sy * h->n, 0);
+                    p.dstPos = p.srcPos;
+                    p.extent = make_cudaExtent(sizeof(float) * (size_t)w, (size_t)rows * h->n, (size_t)tc * fps);
+                    CU_TRY(cudaMemcpy3DAsync(&p, h->st_copy), "cudaMemcpy3DAsync(H2D)");
+                }
+            } else {
+                CU_TRY(cudaMemcpyAsync(h->d_phase[k], src, frame_bytes * tc, cudaMemcpyHostToDevice, h->st_copy), "cudaMemcpyAsync(H2D)");
+            }
             CU_TRY(cudaEventRecord(h->ev_h2d[k], h->st_copy), "cudaEventRecord");
             CU_TRY(cudaStreamWaitEvent(h->st_comp, h->ev_h2d[k], 0), "cudaStreamWaitEvent");
             rc = run_path(h, h->d_phase[k], tc, h->d_slopes + 2 * (size_t)t0 * h->nsub, -1, nullptr, (unsigned)t0, h->st_comp);

@@ -56,6 +56,12 @@ struct shwfs_handle {
     float *d_slopes;       /* device slopes for the whole call, grown on demand */
     float *h_slopes_pin;   /* pinned landing buffer for slopes of a pageable caller */
     size_t d_slopes_cap;   /* floats */
+    /* bands of lenslet rows with one bounding column extent of their valid subapertures: the host pipeline
+     * copies only these (H1 never reads anything else).  band = {first lenslet row, rows, first column,
+     * width in pixels}; n_runs == 0: copy whole frames.                                                */
+    int   *h_runs;
+    int    n_runs;
+    long long run_pixels;  /* pixels per frame covered by the runs */
     int    chunk_frames;
     cudaStream_t st_copy, st_comp;
     cudaEvent_t ev_h2d[2], ev_done[2];

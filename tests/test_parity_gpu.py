@@ -253,3 +253,37 @@ def test_nan_stays_in_its_spot(gpu):
         mask = np.ones(got.shape[:2], bool)
         mask[1, 7] = False
         np.testing.assert_array_equal(got[mask], base[mask])
+
+
+@pytest.mark.parametrize("pinned", [True, False])
+def test_host_pipeline_copies_only_valid_runs(gpu, oracle, pinned):
+    """shwfs_measure_host moves only the column runs of valid subapertures (strided 3-D copies): bit-identical
+    to the device path on config 3 (annular pupil: two runs per lenslet row across the obstruction), from pinned
+    and from pageable memory, with NaN planted everywhere outside the valid subapertures of the host frames."""
+    torch, B = gpu
+    c = W.CONFIGS[3]
+    T = 30                                                    # 26-frame chunks: two chunks
+    ph = W.phase_frames(c, 0, [t % 3 for t in range(T)])
+    with B.from_config(c, 0) as s:
+        yx = s.valid_yx
+        lo = {sy: yx[yx[:, 0] == sy, 1].min() for sy in np.unique(yx[:, 0])}
+        hi = {sy: yx[yx[:, 0] == sy, 1].max() for sy in np.unique(yx[:, 0])}
+        assert s.host_bytes_per_frame == 4 * c.n * c.n * sum(hi[sy] - lo[sy] + 1 for sy in lo)
+        assert s.host_bytes_per_frame < 0.82 * 4 * c.N * c.N
+        dev = s.measure(torch.from_numpy(ph).cuda()).cpu().numpy()
+        keep = np.zeros((c.N, c.N), bool)
+        for sy in lo:                                          # the bounding extent of each lenslet row
+            keep[sy * c.n:(sy + 1) * c.n, lo[sy] * c.n:(hi[sy] + 1) * c.n] = True
+        poisoned = ph.copy()
+        poisoned[:, ~keep] = np.nan
+        if pinned:
+            src = torch.from_numpy(poisoned).pin_memory()
+            got = s.measure_host(src).numpy()
+        else:
+            got = s.measure_host(poisoned)
+        np.testing.assert_array_equal(got, dev)
+    c1 = W.CONFIGS[1]
+    with B.from_config(c1, 0) as s:                            # 80 of 100 subapertures: still worth it
+        assert s.host_bytes_per_frame == 4 * 80 * c1.n * c1.n    # no obstruction: the row extents hold valid patches only
+        ph1 = W.phase_frames(c1, 0, range(4))
+        np.testing.assert_array_equal(s.measure_host(ph1), s.measure(torch.from_numpy(ph1).cuda()).cpu().numpy())
