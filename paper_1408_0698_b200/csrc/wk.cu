@@ -114,10 +114,24 @@ struct WkCfg {
     static constexpr int SG = THREADS / NP;                 /* spot groups in phase 0: 4 / 3 / 2         */
     static constexpr int ITEMS = (SPOTS + SG - 1) / SG;     /* spots per phase-0 thread: 8 / 11 / 16     */
     static constexpr int ES = (((2 * n * n) / 4) | 1) * 4;  /* floats per spot; /4 odd => LDS.128 conflict-free */
-    static constexpr int HS = (((n * 32) / 4) | 1) * 4;
-    static constexpr size_t SMEM = sizeof(float) * (size_t)(SPOTS * ES + SPOTS * HS) + sizeof(int4) * SPOTS;
-    static constexpr int MIN_CTAS = (int)((227 * 1024) / (SMEM + 1024)) < 1 ? 1 : (int)((227 * 1024) / (SMEM + 1024));
+    static constexpr int HS = (((n * 32) / 4) | 1) * 4;     /* all n rows of H per spot (EXT instances)        */
+    static constexpr int HA = (((NW * 32) / 4) | 1) * 4;    /* the NW rows of the first pass only (plain ones) */
     static_assert(n % 2 == 0 && n <= 16, "n must be even and <= 16");
+    static_assert(NW * 32 <= ES, "the second-pass rows of H must fit in the field buffer they replace");
+};
+
+/* Shared memory of one CTA.  Plain instances (SPLIT): the rows of H produced by the second pass overwrite the
+ * field buffer once every warp is done reading it, so only the first-pass rows need room of their own --
+ * 47 KB instead of 68 KB at n = 10, a fourth CTA per SM.  EXT instances accumulate H across sub-layers while
+ * the field buffer is rewritten, and keep the two apart.                                                  */
+template <int n, bool SPLIT>
+struct WkSmem {
+    using Cfg = WkCfg<n>;
+    static constexpr int HSTRIDE = SPLIT ? Cfg::HA : Cfg::HS;
+    static constexpr size_t BYTES = sizeof(float) * (size_t)(Cfg::SPOTS * Cfg::ES + Cfg::SPOTS * HSTRIDE) + sizeof(int4) * Cfg::SPOTS;
+    static constexpr int BY_SMEM = (int)((227 * 1024) / (BYTES + 1024));
+    /* the plain n = 16 instance needs 196 registers x 256 threads: one CTA per SM whatever the memory says */
+    static constexpr int MIN_CTAS = n == 16 ? 1 : (BY_SMEM < 1 ? 1 : BY_SMEM);
 };
 
 struct WkArgs {
@@ -269,13 +283,15 @@ __device__ __forceinline__ void finish_row(const float2 (&acc)[2 * n - 1], const
 }
 
 template <int n, int MODE, bool EXT>
-__global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_measure_kernel(const WkArgs A)
+__global__ void __launch_bounds__(WkCfg<n>::THREADS, WkSmem<n, !EXT>::MIN_CTAS) wk_measure_kernel(const WkArgs A)
 {
     using Cfg = WkCfg<n>;
+    constexpr bool SPLIT = !EXT;
+    constexpr int HSTRIDE = WkSmem<n, SPLIT>::HSTRIDE;
     extern __shared__ __align__(16) float smem[];
     float *ebuf = smem;
     float *hbuf = smem + Cfg::SPOTS * Cfg::ES;
-    int4 *s_info = reinterpret_cast<int4 *>(hbuf + Cfg::SPOTS * Cfg::HS);   /* {patch offset, t, i, -} */
+    int4 *s_info = reinterpret_cast<int4 *>(hbuf + Cfg::SPOTS * HSTRIDE);   /* {patch offset, t, i, -} */
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g0 = blockIdx.x * Cfg::SPOTS;
@@ -372,7 +388,7 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
     /* ---- phase 1: autocorrelation rows, table product, x-transform ---- */
     {
         const float *eb = ebuf + lane * Cfg::ES;
-        float *hb = hbuf + lane * Cfg::HS;
+        float *hb = hbuf + lane * HSTRIDE;
         const int i = max(s_info[lane].z, 0);
         const float2 *Mi = A.M + (size_t)i * A.mstride;
 #pragma unroll 1
@@ -400,7 +416,14 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
 #pragma unroll
                 for (int a = 0; a < Cfg::LX; ++a) acc[a] = L.lag_value(a);
             }
-            finish_row<n>(acc, Mi + ly * Cfg::LX, hb + ly * 32, EXT && layer > 0);
+            if (SPLIT) {
+                /* first pass: row slot = warp in the H buffer; second pass: same slot in the field buffer,
+                 * once every warp has finished reading the field */
+                if (pass == 1) __syncthreads();
+                finish_row<n>(acc, Mi + ly * Cfg::LX, (pass == 0 ? hb : ebuf + lane * Cfg::ES) + warp * 32, false);
+            } else {
+                finish_row<n>(acc, Mi + ly * Cfg::LX, hb + ly * 32, EXT && layer > 0);
+            }
         }
     }
     }   /* sub-layers */
@@ -410,12 +433,16 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkCfg<n>::MIN_CTAS) wk_meas
     {
         const int half = lane >> 4, C = lane & 15;
         for (int s = warp * 2 + half; s < Cfg::SPOTS; s += 2 * Cfg::NW) {
-            const float *hb = hbuf + s * Cfg::HS + 2 * C;
+            const float *hb = hbuf + s * HSTRIDE + 2 * C;
+            const float *hb2 = ebuf + s * Cfg::ES + 2 * C;       /* SPLIT: second-pass rows */
             float yr[16], yi[16];
 #pragma unroll
             for (int m = 0; m < 16; ++m) {
                 if (m < n) {
-                    const float2 v = *reinterpret_cast<const float2 *>(hb + m * 32);
+                    /* lag row m sits in slot m (first pass), 0 (m = n/2) or n - m (second pass) */
+                    const float *src = !SPLIT ? hb + m * 32
+                                     : m < n / 2 ? hb + m * 32 : hb2 + (m == n / 2 ? 0 : n - m) * 32;
+                    const float2 v = *reinterpret_cast<const float2 *>(src);
                     yr[m] = v.x; yi[m] = v.y;
                 } else { yr[m] = 0.f; yi[m] = 0.f; }
             }
@@ -582,12 +609,12 @@ cudaError_t launch_special_mode(const WkArgs &A, cudaStream_t st)
     cudaGetDevice(&dev);
     if (dev >= 0 && dev < 64 && !attr_set[dev]) {
         cudaError_t e = cudaFuncSetAttribute(wk_measure_kernel<n, MODE, EXT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)Cfg::SMEM);
+                                             (int)WkSmem<n, !EXT>::BYTES);
         if (e != cudaSuccess) return e;
         attr_set[dev] = true;
     }
     const int grid = (A.total + Cfg::SPOTS - 1) / Cfg::SPOTS;
-    wk_measure_kernel<n, MODE, EXT><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(A);
+    wk_measure_kernel<n, MODE, EXT><<<grid, Cfg::THREADS, WkSmem<n, !EXT>::BYTES, st>>>(A);
     return cudaGetLastError();
 }
 
