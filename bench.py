@@ -39,9 +39,9 @@ F_NOM = {1: 10240, 2: 51200, 3: 153600, 4: 153600, 5: 737280}
 # (profiles/r01_fp32_peak.md).
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/r01_{wk10,wk16}_full_v4.md, r01_pf32_full.md), keyed by config; None where no
+# `ncu --set full` captures (profiles/r01_wk10_full_v5.md, r01_wk16_full_v4.md, r01_pf32_full.md), keyed by config; None where no
 # capture of that config's kernel exists.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: 129117184 + 5640192, 3: 206536448 + 7660288, 4: 206536448 + 7660288,
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: 129117184 + 5640192, 3: 206465280 + 5998336, 4: 206465280 + 5998336,
                                 5: 506635264 + 7373568}
 
 
