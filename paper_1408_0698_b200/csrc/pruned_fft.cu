@@ -58,16 +58,13 @@ __host__ __device__ constexpr int col_pos(int u) { return (u % (P / 16)) * 16 + 
 
 /* H1 of one spot row: the NZ/2 pixel pairs of patch row r of spot g (zeros when the row does not exist) */
 template <int NZ>
-__device__ __forceinline__ void pf_gather(const PfArgs &A, int g, int r, float2 (&ph)[NZ / 2], float2 (&am)[NZ / 2])
+__device__ __forceinline__ void pf_gather(const PfArgs &A, int off, int t, float2 (&ph)[NZ / 2], float2 (&am)[NZ / 2])
 {
 #pragma unroll
     for (int q = 0; q < NZ / 2; ++q) { ph[q] = make_float2(0.f, 0.f); am[q] = make_float2(0.f, 0.f); }
-    if (g < A.total && r < A.n) {
-        const int i = g / A.T, t = g - i * A.T;
-        const int2 yx = A.valid[i];
-        const size_t o = (size_t)(yx.x * A.n + r) * A.N + (size_t)yx.y * A.n;
-        const float2 *pp = reinterpret_cast<const float2 *>(A.phase + (size_t)t * A.frame_stride + o);
-        const float2 *pa = reinterpret_cast<const float2 *>(A.amp + o);
+    if (off >= 0) {                         /* off: pixel offset of this thread's patch row, -1 if there is none */
+        const float2 *pp = reinterpret_cast<const float2 *>(A.phase + (size_t)t * A.frame_stride + off);
+        const float2 *pa = reinterpret_cast<const float2 *>(A.amp + off);
 #pragma unroll
         for (int q = 0; q < NZ / 2; ++q)
             if (2 * q < A.n) { ph[q] = __ldg(pp + q); am[q] = __ldg(pa + q); }
@@ -85,8 +82,22 @@ __global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel
     const int tid = threadIdx.x, sp = tid >> 4, r = tid & 15;
     float *tile = pf_smem + sp * Cfg::TILE;
 
+    /* patch-row offsets of all the CTA's tiles first: the valid-list lookups (the only dependent loads of the
+     * gather) are issued together, so that the prefetch below never waits on one in program order */
+    int offs[PF_TILES], tts[PF_TILES];
+#pragma unroll
+    for (int it = 0; it < PF_TILES; ++it) {
+        const int g = (blockIdx.x * PF_TILES + it) * PF_SPOTS + sp;
+        offs[it] = -1; tts[it] = 0;
+        if (g < A.total && r < A.n) {
+            const int i = g / A.T;
+            const int2 yx = __ldg(A.valid + i);
+            tts[it] = g - i * A.T;
+            offs[it] = (yx.x * A.n + r) * A.N + yx.y * A.n;
+        }
+    }
     float2 ph[NZ / 2], am[NZ / 2];
-    pf_gather<NZ>(A, (blockIdx.x * PF_TILES) * PF_SPOTS + sp, r, ph, am);
+    pf_gather<NZ>(A, offs[0], tts[0], ph, am);
 
 #pragma unroll 1
     for (int it = 0; it < PF_TILES; ++it) {
@@ -127,7 +138,9 @@ __global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel
         }
         __syncwarp();
         /* H1 of the next tile: in flight during the column pass */
-        if (it + 1 < PF_TILES) pf_gather<NZ>(A, g + PF_SPOTS, r, ph, am);
+        if (it + 1 < PF_TILES) pf_gather<NZ>(A, offs[1], tts[1], ph, am);
+#pragma unroll
+        for (int q = 0; q + 1 < PF_TILES; ++q) { offs[q] = offs[q + 1]; tts[q] = tts[q + 1]; }   /* rotate */
 
         /* ---- column pass: b columns per thread, |.|^2 and the row half of the bin in registers ---- */
         float acc[16];
