@@ -287,3 +287,31 @@ def test_host_pipeline_copies_only_valid_runs(gpu, oracle, pinned):
         assert s.host_bytes_per_frame == 4 * 80 * c1.n * c1.n    # no obstruction: the row extents hold valid patches only
         ph1 = W.phase_frames(c1, 0, range(4))
         np.testing.assert_array_equal(s.measure_host(ph1), s.measure(torch.from_numpy(ph1).cuda()).cpu().numpy())
+
+
+@pytest.mark.parametrize("cfg_id", [2, 5])
+def test_full_batch_sampled_spots_other_configs(gpu, oracle, cfg_id):
+    """Configs 2 (pruned-FFT path, no elongation) and 5 (n = 16, pad 64, 4x4 binning, elongation <= 6 arcsec) at
+    BASELINE.json's full batch size, in the one-launch configuration bench.py --config uses: 1500 sampled
+    (frame, subaperture) outputs recomputed one by one by the oracle."""
+    torch, B = gpu
+    c = W.CONFIGS[cfg_id]
+    amp = W.pupil_mask(c)
+    dev = torch.device("cuda")
+    phd = W.phase_frames_device(c, 0, range(c.batch), dev)
+    with B.from_config(c, 0) as s:
+        yx = s.valid_yx
+        got = s.measure(phd)
+        assert s.launch_count == 1
+        torch.cuda.synchronize()
+        got = got.cpu().numpy()
+    assert np.isfinite(got).all()
+    rng = np.random.default_rng(77 + cfg_id)
+    for t in (0, int(rng.integers(1, c.batch - 1)), c.batch - 1):
+        idx = np.sort(rng.choice(len(yx), size=500, replace=False))
+        idx[0], idx[-1] = 0, len(yx) - 1
+        K = W.elongation_kernels(c, 0, yx, subset=idx)
+        frame = phd[int(t)].cpu().numpy()[None]
+        want = oracle.measure(frame, amp, yx[idx], c.n, c.P, c.b, tau=c.tau, kernels=K)
+        err = np.abs(got[t, idx] - want[0]).max()
+        assert err <= SLOPE_TOL, (cfg_id, int(t), err)
