@@ -41,6 +41,8 @@ void free_handle(shwfs_handle *h)
     cudaFree(h->d_sod_g);
     cudaFree(h->d_dm_modes);
     cudaFree(h->d_dm_patch);
+    cudaFree(h->d_um_modes);
+    cudaFree(h->d_um_coef);
     for (int k = 0; k < 2; ++k) {
         if (h->h_pin[k]) cudaFreeHost(h->h_pin[k]);
         cudaFree(h->d_phase[k]);
@@ -363,6 +365,8 @@ int shwfs_set_dm(shwfs_handle *h, const float *modes_dev, int32_t M)
     cudaDeviceSynchronize();                     /* nothing in flight may still read the old tables */
     cudaFree(h->d_dm_modes); h->d_dm_modes = nullptr;
     cudaFree(h->d_dm_patch); h->d_dm_patch = nullptr; h->dm_patch_cap = 0;
+    cudaFree(h->d_um_modes); h->d_um_modes = nullptr;
+    cudaFree(h->d_um_coef); h->d_um_coef = nullptr; h->um_coef_cap = 0;
     h->dm_M = 0;
     if (M > 0 && modes_dev) {
         if (!shwfs_wk_supported(h, 0) && !shwfs_wk_supported(h, 1)) { rc = SHWFS_EUNSUPPORTED; goto done; }
@@ -370,8 +374,18 @@ int shwfs_set_dm(shwfs_handle *h, const float *modes_dev, int32_t M)
         h->dm_patch_cap = (size_t)h->nsub * h->n * h->n;          /* one frame: enough for the loop */
         CU_TRY(cudaMalloc(&h->d_dm_patch, sizeof(float) * h->dm_patch_cap), "cudaMalloc(dm patch)");
         CU_TRY(shwfs_loop_relayout_modes(h, modes_dev, M, 0), "relayout_modes");
-        CU_TRY(cudaStreamSynchronize(0), "set_dm sync");
         h->dm_M = M;
+        if (shwfs_umma_np(h) > 0) {
+            /* tensor-core operand tiles (hi|lo split, canonical layout); best effort: without them the FP32
+             * SIMT GEMM of loop.cu serves every batch size */
+            if (cudaMalloc(&h->d_um_modes, sizeof(float) * shwfs_umma_modes_floats(h, M)) == cudaSuccess) {
+                CU_TRY(shwfs_umma_build_modes(h, 0), "umma_build_modes");
+            } else {
+                h->d_um_modes = nullptr;
+                cudaGetLastError();
+            }
+        }
+        CU_TRY(cudaStreamSynchronize(0), "set_dm sync");
     }
     goto done;
 fail:
@@ -445,9 +459,19 @@ int shwfs_measure_residual(shwfs_handle *h, const float *phase_dev, const float 
         if (e != cudaSuccess) { shwfs_note_cuda_error(e, "cudaMalloc(dm patch)"); return SHWFS_ENOMEM; }
         h->dm_patch_cap = need;
     }
+    if (h->d_um_modes && T > 8) {
+        const size_t cneed = shwfs_umma_coef_floats(T, h->dm_M);
+        if (h->um_coef_cap < cneed) {
+            cudaStreamSynchronize(st);
+            cudaFree(h->d_um_coef); h->d_um_coef = nullptr; h->um_coef_cap = 0;
+            cudaError_t e2 = cudaMalloc(&h->d_um_coef, sizeof(float) * cneed);
+            if (e2 != cudaSuccess) { shwfs_note_cuda_error(e2, "cudaMalloc(um coef)"); return SHWFS_ENOMEM; }
+            h->um_coef_cap = cneed;
+        }
+    }
     cudaError_t e = shwfs_loop_dm_phase(h, coef_dev, h->dm_M, T, h->d_dm_patch, st);
     if (e != cudaSuccess) { shwfs_note_cuda_error(e, "dm_phase"); return SHWFS_ECUDA; }
-    h->launches += 1;
+    h->launches += (h->d_um_modes && T > 8 && h->d_um_coef) ? 2 : 1;
     return run_path(h, phase_dev, T, slopes_dev, -1, nullptr, 0u, st, h->d_dm_patch);
 }
 

@@ -44,6 +44,10 @@ struct shwfs_handle {
     /* closed-loop neighbours (shwfs_set_dm ...): modes re-laid per subaperture, padded coefficient buffers */
     float  *d_dm_modes;                 /* [nsub][M][n*n] modes re-laid per subaperture */
     int     dm_M;
+    float  *d_um_modes;                 /* tensor-core operand B: split (hi|lo) canonical tiles, dm_umma.cu; or null */
+    float  *d_um_coef;                  /* tensor-core operand A of the current call (split coefficient tiles)       */
+    size_t  um_coef_cap;                /* floats */
+    int     um_nkb;                     /* k-blocks of 16 modes */
     float  *d_dm_patch;                 /* [cap_T][nsub][n*n] DM phase of the current call, patch layout */
     size_t  dm_patch_cap;               /* floats */
 
@@ -80,6 +84,13 @@ cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *s
 
 /* loop.cu: closed-loop neighbours */
 cudaError_t shwfs_loop_relayout_modes(shwfs_handle *h, const float *modes_dev, int M, cudaStream_t st);
+/* dm_umma.cu: the DM-phase GEMM on tcgen05 (3xTF32) */
+int shwfs_umma_np(const shwfs_handle *h);                         /* padded n*n, 0 if the size has no instance */
+size_t shwfs_umma_modes_floats(const shwfs_handle *h, int M);
+size_t shwfs_umma_coef_floats(int T, int M);
+cudaError_t shwfs_umma_build_modes(shwfs_handle *h, cudaStream_t st);
+cudaError_t shwfs_umma_dm_phase(shwfs_handle *h, const float *coef, int ldc, int T, float *out, cudaStream_t st);
+
 cudaError_t shwfs_loop_dm_phase(shwfs_handle *h, const float *coef, int ldc, int T, float *out, cudaStream_t st);
 cudaError_t shwfs_loop_reconstruct(const float *R, const float *slopes, int T, int K, int M, float gain,
                                    float *coef, int ldc, float *hist_or_null, cudaStream_t st);

@@ -17,6 +17,7 @@
  * shwfs_closed_loop chains the two, frame after frame, on the caller's stream (readings C1..C4 of DESIGN.md).
  */
 #include <cuda_pipeline.h>
+#include <stdlib.h>
 
 #include "internal.h"
 
@@ -281,6 +282,11 @@ cudaError_t shwfs_loop_relayout_modes(shwfs_handle *h, const float *modes_dev, i
 cudaError_t shwfs_loop_dm_phase(shwfs_handle *h, const float *coef, int ldc, int T, float *out, cudaStream_t st)
 {
     const int nn = h->n * h->n, M = h->dm_M;
+    /* batches go to the tensor cores (dm_umma.cu) when the split operand tiles exist; SHWFS_DM_FP32=1 keeps the
+     * FP32 SIMT GEMM below (A/B comparisons) */
+    if (T > 8 && h->d_um_modes && h->d_um_coef && h->um_coef_cap >= shwfs_umma_coef_floats(T, M) &&
+        !getenv("SHWFS_DM_FP32"))
+        return shwfs_umma_dm_phase(h, coef, ldc, T, out, st);
     if (h->nsub <= 65535 && (nn == 64 || nn == 100 || nn == 256)) {
         switch (nn) {
         case 64: launch_dm_phase_n<64>(h, coef, ldc, T, out, st); break;

@@ -151,3 +151,38 @@ def test_residual_with_sublayers(gpu, oracle):
         for a in _wk_algos(s, B):
             got = s.measure_residual(torch.from_numpy(ph).cuda(), torch.from_numpy(coef).cuda()).cpu().numpy()
             assert np.abs(got - want).max() <= SLOPE_TOL, a
+
+
+@pytest.mark.parametrize("cfg_id,M,T", [(3, 37, 20), (1, 50, 150), (5, 21, 12)])
+def test_residual_batches_on_the_tensor_cores(gpu, oracle, loop, cfg_id, M, T):
+    """Batches (T > 8) take the tcgen05 3xTF32 GEMM of dm_umma.cu (n*n = 100 -> N = 112, 64, 256; M not a
+    multiple of the 16-mode stage; T = 150: two frame tiles, the second ragged): slopes against the oracle on a
+    sample of subapertures, and against the FP32 SIMT GEMM (SHWFS_DM_FP32=1) on every spot."""
+    import os
+    torch, B = gpu
+    c = W.CONFIGS[cfg_id]
+    amp = W.pupil_mask(c)
+    yx = oracle.valid_list(amp, c.n, c.min_illum)
+    modes = W.dm_modes(c, M)
+    rng = np.random.default_rng(100 + cfg_id)
+    ph = W.phase_frames(c, 0, [t % 2 for t in range(T)])
+    coef = rng.normal(0, 0.5, (T, M)).astype(np.float32)
+    coef[:, :2] *= 0.3
+    with B.from_config(c, 0) as s:
+        s.set_dm(torch.from_numpy(modes).cuda())
+        phd, cd = torch.from_numpy(ph).cuda(), torch.from_numpy(coef).cuda()
+        l0 = s.launch_count
+        got = s.measure_residual(phd, cd).cpu().numpy()
+        assert s.launch_count - l0 == 3                     # split coefficients, tensor-core GEMM, sensor
+        os.environ["SHWFS_DM_FP32"] = "1"
+        try:
+            ref = s.measure_residual(phd, cd).cpu().numpy()
+        finally:
+            del os.environ["SHWFS_DM_FP32"]
+        assert np.abs(got - ref).max() <= 2e-5              # 3xTF32 is fp32-like: far inside the 1e-3 tolerance
+        K = W.elongation_kernels(c, 0, yx)
+        sel = np.sort(rng.choice(len(yx), size=min(len(yx), 60), replace=False))
+        ts = [0, T // 2, T - 1]
+        want = loop.measure_residual(ph[ts], modes, coef[ts], amp, yx[sel], c.n, c.P, c.b, tau=c.tau,
+                                     kernels=None if K is None else K[sel])
+        assert np.abs(got[ts][:, sel] - want).max() <= SLOPE_TOL
