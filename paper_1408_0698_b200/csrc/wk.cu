@@ -282,11 +282,15 @@ __device__ __forceinline__ void finish_row(const float2 (&acc)[2 * n - 1], const
     }
 }
 
-template <int n, int MODE, bool EXT>
-__global__ void __launch_bounds__(WkCfg<n>::THREADS, WkSmem<n, !EXT>::MIN_CTAS) wk_measure_kernel(const WkArgs A)
+/* EXTK: 0 = plain sensor; 1 = extensions on one (sub-)layer (noise, DM residual, a single sodium layer): same
+ * shared-memory layout and occupancy as the plain instance; 2 = several sodium sub-layers: H accumulates over
+ * the layers in a buffer of its own.                                                                     */
+template <int n, int MODE, int EXTK>
+__global__ void __launch_bounds__(WkCfg<n>::THREADS, WkSmem<n, (EXTK < 2)>::MIN_CTAS) wk_measure_kernel(const WkArgs A)
 {
+    constexpr bool EXT = EXTK > 0;
     using Cfg = WkCfg<n>;
-    constexpr bool SPLIT = !EXT;
+    constexpr bool SPLIT = EXTK < 2;
     constexpr int HSTRIDE = WkSmem<n, SPLIT>::HSTRIDE;
     extern __shared__ __align__(16) float smem[];
     float *ebuf = smem;
@@ -309,7 +313,7 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkSmem<n, !EXT>::MIN_CTAS) 
     }
     __syncthreads();
 
-    const int n_layers = EXT && A.L > 0 ? A.L : 1;      /* A.L == 0: single-layer sensor (noise only) */
+    const int n_layers = EXTK == 2 && A.L > 0 ? A.L : 1;      /* A.L == 0: single-layer sensor (noise only) */
     const bool sodium = EXT && A.L > 0;
 #pragma unroll 1
     for (int layer = 0; layer < n_layers; ++layer) {
@@ -600,7 +604,7 @@ __global__ void __launch_bounds__(GEN_THREADS) wk_generic_kernel(const WkArgs A,
     }
 }
 
-template <int n, int MODE, bool EXT>
+template <int n, int MODE, int EXTK>
 cudaError_t launch_special_mode(const WkArgs &A, cudaStream_t st)
 {
     using Cfg = WkCfg<n>;
@@ -608,22 +612,24 @@ cudaError_t launch_special_mode(const WkArgs &A, cudaStream_t st)
     int dev = 0;
     cudaGetDevice(&dev);
     if (dev >= 0 && dev < 64 && !attr_set[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(wk_measure_kernel<n, MODE, EXT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)WkSmem<n, !EXT>::BYTES);
+        cudaError_t e = cudaFuncSetAttribute(wk_measure_kernel<n, MODE, EXTK>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)WkSmem<n, (EXTK < 2)>::BYTES);
         if (e != cudaSuccess) return e;
         attr_set[dev] = true;
     }
     const int grid = (A.total + Cfg::SPOTS - 1) / Cfg::SPOTS;
-    wk_measure_kernel<n, MODE, EXT><<<grid, Cfg::THREADS, WkSmem<n, !EXT>::BYTES, st>>>(A);
+    wk_measure_kernel<n, MODE, EXTK><<<grid, Cfg::THREADS, WkSmem<n, (EXTK < 2)>::BYTES, st>>>(A);
     return cudaGetLastError();
 }
 
 template <int n>
 cudaError_t launch_special(const WkArgs &A, cudaStream_t st)
 {
+    if (A.L > 1)
+        return A.mode == 0 ? launch_special_mode<n, 0, 2>(A, st) : launch_special_mode<n, 1, 2>(A, st);
     if (A.L > 0 || A.flux > 0.f || A.dm_patch != nullptr)
-        return A.mode == 0 ? launch_special_mode<n, 0, true>(A, st) : launch_special_mode<n, 1, true>(A, st);
-    return A.mode == 0 ? launch_special_mode<n, 0, false>(A, st) : launch_special_mode<n, 1, false>(A, st);
+        return A.mode == 0 ? launch_special_mode<n, 0, 1>(A, st) : launch_special_mode<n, 1, 1>(A, st);
+    return A.mode == 0 ? launch_special_mode<n, 0, 0>(A, st) : launch_special_mode<n, 1, 0>(A, st);
 }
 
 }  // namespace
