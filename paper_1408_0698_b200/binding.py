@@ -314,8 +314,9 @@ class Shwfs:
         import torch
         L = getattr(self, "_layers", 1)
         shape = (self.N, self.N) if L == 1 else (L, self.N, self.N)
+        ok_shape = tuple(phase.shape[1:]) == shape or (L == 1 and tuple(phase.shape[1:]) == (1, self.N, self.N))
         if not (isinstance(phase, torch.Tensor) and phase.is_cuda and phase.dtype == torch.float32
-                and phase.is_contiguous() and tuple(phase.shape[1:]) == shape):
+                and phase.is_contiguous() and ok_shape):
             raise ValueError(f"phase must be a contiguous float32 CUDA tensor [T,{','.join(map(str, shape))}]")
 
     def measure(self, phase, out=None, stream=None):
