@@ -216,3 +216,16 @@ def test_measure_host_matches_device_path(gpu, pinned):
         np.testing.assert_array_equal(got_np, want.numpy())
         got2 = s.measure_host(host[:3].contiguous())      # smaller call after a larger one
         assert torch.equal(got2, want[:3])
+
+
+def test_library_carries_blackwell_tensor_core_code(libshwfs):
+    """The DM-phase GEMM is tcgen05 code: the SASS of the built library holds UTCHMMA (tcgen05.mma), LDTM
+    (tcgen05.ld) and UBLKCP (cp.async.bulk) -- the mnemonics of B200_PROFILING.md -- and no legacy HMMA path."""
+    import shutil
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not Path(cuobjdump).exists():
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([cuobjdump, "-sass", str(libshwfs)], capture_output=True, text=True, check=True).stdout
+    assert "UTCHMMA" in sass and "LDTM" in sass and "UBLKCP" in sass
+    assert "HGMMA" not in sass and " HMMA" not in sass
+    assert "sm_100a" in sass
