@@ -38,6 +38,8 @@ F_NOM = {1: 10240, 2: 51200, 3: 153600, 4: 153600, 5: 737280}
 # lanes per SM, FMA = 2 flop): 148 * 128 * 2 * 1.965e9.  Measured FFMA chain on this pool: 72.4 TFLOP/s
 # (profiles/r01_fp32_peak.md).
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+# sm__pipe_fma_cycles_active (fraction of peak) of the dominant kernel in the committed ncu --set full captures
+NCU_FMA_PIPE_ACTIVE = {2: 0.503, 3: 0.636, 4: 0.636, 5: 0.640}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/r01_wk10_full_v5.md, r01_wk16_full_v4.md, r01_pf32_full.md), keyed by config; None where no
 # capture of that config's kernel exists.
@@ -309,6 +311,7 @@ def run_ours(args):
                     "frac_nominal_fft_flops": (F_NOM[c.cfg] * spots_per_launch / (kern_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS
                                                if L <= 0 else None),
                     "peak_basis": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (measured FFMA chain 72.4)",
+                    "fma_pipe_active_ncu": NCU_FMA_PIPE_ACTIVE.get(c.cfg) if L <= 0 and args.noise_flux <= 0 else None,
                     "hbm_frac": (in_bytes + out_bytes) / c.W / (kern_ms * 1e-3) / 1e9 / _hbm_peak()}
         cpu = None if args.no_cpu_baseline else cpu_baseline(c, args, phase, sensors[0].valid_yx)
         out = {
