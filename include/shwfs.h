@@ -99,6 +99,12 @@ int shwfs_measure(shwfs_handle *h, const float *phase_dev, int32_t T, float *slo
  * slopes have landed in slopes_host.  This is the end-to-end entry point timed as "e2e" by bench.py.   */
 int shwfs_measure_host(shwfs_handle *h, const float *phase_host, int32_t T, float *slopes_host);
 
+/* The same, returning once everything is enqueued on the handle's own streams: both buffers must be pinned host
+ * memory (EINVAL otherwise) and stay untouched until shwfs_host_wait(h) returns.  Several handles (the six LGS
+ * sensors of a system) can so keep the bus busy back to back.  One call in flight per handle.            */
+int shwfs_measure_host_async(shwfs_handle *h, const float *phase_host, int32_t T, float *slopes_host);
+int shwfs_host_wait(shwfs_handle *h);
+
 /* Bytes of one N x N wavefront that shwfs_measure_host actually moves to the device: only the bounding column
  * extent of the valid subapertures of each lenslet row is copied (strided 3-D copies, rows of equal extent
  * merged) when that saves at least a tenth of the frame; the rest is never read by H1.                  */

@@ -26,7 +26,8 @@ EXPORTS = ["shwfs_create", "shwfs_measure", "shwfs_measure_host", "shwfs_destroy
            "shwfs_valid_list", "shwfs_pixel_scale", "shwfs_set_algorithm", "shwfs_get_algorithm",
            "shwfs_launch_count", "shwfs_debug_spots", "shwfs_strerror", "shwfs_last_cuda_error",
            "shwfs_version", "shwfs_set_sodium", "shwfs_set_noise", "shwfs_set_dm",
-           "shwfs_measure_residual", "shwfs_reconstruct", "shwfs_closed_loop", "shwfs_host_bytes_per_frame"]
+           "shwfs_measure_residual", "shwfs_reconstruct", "shwfs_closed_loop", "shwfs_host_bytes_per_frame",
+           "shwfs_measure_host_async", "shwfs_host_wait"]
 SHWFS_MAX_LAYERS = 8
 
 
@@ -89,6 +90,8 @@ def load():
     L.shwfs_set_noise.argtypes = [vp, C.POINTER(ShwfsNoise)]
     L.shwfs_set_dm.argtypes = [vp, vp, i32]
     L.shwfs_host_bytes_per_frame.argtypes = [vp, C.POINTER(i64)]
+    L.shwfs_measure_host_async.argtypes = [vp, vp, i32, vp]
+    L.shwfs_host_wait.argtypes = [vp]
     L.shwfs_measure_residual.argtypes = [vp, vp, vp, i32, vp, vp]
     L.shwfs_reconstruct.argtypes = [vp, vp, vp, i32, C.c_float, vp, vp]
     L.shwfs_closed_loop.argtypes = [vp, vp, vp, C.c_float, vp, i32, vp, vp, vp]
@@ -355,6 +358,17 @@ class Shwfs:
             raise ValueError(f"phase_host must be [T,{','.join(map(str, shape))}]")
         shwfs_measure_host(self._h, ptr, T, optr)
         return out
+
+    def measure_host_async(self, phase_host, out):
+        """Enqueue measure_host on the handle's own streams (pinned CPU torch tensors only); host_wait() ends it."""
+        if not (phase_host.is_pinned() and out.is_pinned() and phase_host.is_contiguous() and out.is_contiguous()):
+            raise ValueError("measure_host_async needs contiguous pinned CPU tensors")
+        _check(load().shwfs_measure_host_async(self._h, phase_host.data_ptr(), int(phase_host.shape[0]),
+                                               out.data_ptr()), "shwfs_measure_host_async")
+        return out
+
+    def host_wait(self):
+        _check(load().shwfs_host_wait(self._h), "shwfs_host_wait")
 
     def debug_spots(self, phase, stage: int, stream=None):
         """Images of stage 0 / 1 ([T,nsub,P,P]) or 2 / 3 ([T,nsub,D,D]; 3 = after the detector noise) as a

@@ -575,7 +575,7 @@ bool is_pinned(const void *p)
 
 }  // namespace
 
-extern "C" int shwfs_measure_host(shwfs_handle *h, const float *phase_host, int32_t T, float *slopes_host)
+static int measure_host_impl(shwfs_handle *h, const float *phase_host, int32_t T, float *slopes_host, bool wait)
 {
     if (!h || T < 0) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
@@ -599,6 +599,7 @@ extern "C" int shwfs_measure_host(shwfs_handle *h, const float *phase_host, int3
             h->d_slopes_cap = n_slopes;
         }
         const bool pinned_in = is_pinned(phase_host);
+        if (!wait && !(pinned_in && is_pinned(slopes_host))) { rc = SHWFS_EINVAL; goto fail; }   /* async: pinned only */
         if (!pinned_in)
             for (int k = 0; k < 2; ++k)
                 if (!h->h_pin[k]) CU_TRY(cudaHostAlloc(&h->h_pin[k], sizeof(float) * (size_t)h->N * h->N * h->chunk_frames, cudaHostAllocDefault), "cudaHostAlloc");
@@ -638,10 +639,29 @@ extern "C" int shwfs_measure_host(shwfs_handle *h, const float *phase_host, int3
             CU_TRY(cudaEventRecord(h->ev_done[k], h->st_comp), "cudaEventRecord");
         }
         CU_TRY(cudaMemcpyAsync(slopes_host, h->d_slopes, sizeof(float) * n_slopes, cudaMemcpyDeviceToHost, h->st_comp), "cudaMemcpyAsync(D2H)");
-        CU_TRY(cudaStreamSynchronize(h->st_comp), "cudaStreamSynchronize");
+        if (wait) CU_TRY(cudaStreamSynchronize(h->st_comp), "cudaStreamSynchronize");
     }
 fail:
     if (rc && h->st_comp) { cudaStreamSynchronize(h->st_comp); cudaStreamSynchronize(h->st_copy); }
     if (prev >= 0 && prev != h->device) cudaSetDevice(prev);
     return rc;
+}
+
+extern "C" int shwfs_measure_host(shwfs_handle *h, const float *phase_host, int32_t T, float *slopes_host)
+{
+    return measure_host_impl(h, phase_host, T, slopes_host, true);
+}
+
+extern "C" int shwfs_measure_host_async(shwfs_handle *h, const float *phase_host, int32_t T, float *slopes_host)
+{
+    return measure_host_impl(h, phase_host, T, slopes_host, false);
+}
+
+extern "C" int shwfs_host_wait(shwfs_handle *h)
+{
+    if (!h) return SHWFS_EINVAL;
+    if (!h->st_comp) return SHWFS_OK;
+    cudaError_t e = cudaStreamSynchronize(h->st_comp);
+    if (e != cudaSuccess) { shwfs_note_cuda_error(e, "shwfs_host_wait"); return SHWFS_ECUDA; }
+    return SHWFS_OK;
 }

@@ -229,3 +229,21 @@ def test_library_carries_blackwell_tensor_core_code(libshwfs):
     assert "UTCHMMA" in sass and "LDTM" in sass and "UBLKCP" in sass
     assert "HGMMA" not in sass and " HMMA" not in sass
     assert "sm_100a" in sass
+
+
+@pytest.mark.gpu
+def test_measure_host_async_matches_the_blocking_call(gpu):
+    torch, B = gpu
+    from paper_1408_0698_b200 import workloads as W
+    c = W.CONFIGS[1]
+    host = torch.from_numpy(W.phase_frames(c, 0, range(4))).pin_memory()
+    with B.from_config(c, 0) as s1, B.from_config(c, 0) as s2:
+        want = s1.measure_host(host).clone()
+        o1 = torch.empty((4, s1.nsub, 2), dtype=torch.float32).pin_memory()
+        o2 = torch.empty((4, s2.nsub, 2), dtype=torch.float32).pin_memory()
+        s1.measure_host_async(host, o1)
+        s2.measure_host_async(host, o2)               # two handles in flight
+        s1.host_wait(); s2.host_wait()
+        assert torch.equal(o1, want) and torch.equal(o2, want)
+        rc = B.load().shwfs_measure_host_async(s1._h, host.numpy().copy().ctypes.data, 4, o1.data_ptr())
+        assert rc == B.SHWFS_EINVAL                   # pageable input is refused
