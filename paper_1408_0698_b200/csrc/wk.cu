@@ -114,7 +114,11 @@ struct WkCfg {
     static constexpr int SG = THREADS / NP;                 /* spot groups in phase 0: 4 / 3 / 2         */
     static constexpr int ITEMS = (SPOTS + SG - 1) / SG;     /* spots per phase-0 thread: 8 / 11 / 16     */
     static constexpr int ES = (((2 * n * n) / 4) | 1) * 4;  /* floats per spot; /4 odd => LDS.128 conflict-free */
-    static constexpr int HS = (((n * 32) / 4) | 1) * 4;     /* all n rows of H per spot (EXT instances)        */
+    /* multi-layer instances: the raw lag rows G pile up over the sub-layers in shared memory, one row of RS floats
+     * per lag row (2n-1 complex lags, and room for the 16 complex values of H that replace them after the last
+     * sub-layer); GS/2 odd => the lane-strided 8-byte accesses are conflict-free                              */
+    static constexpr int RS = 2 * LX > 32 ? 2 * LX : 32;
+    static constexpr int GS = n * RS + (((n * RS / 2) & 1) ? 0 : 2);
     static constexpr int HA = (((NW * 32) / 4) | 1) * 4;    /* the NW rows of the first pass only (plain ones) */
     static_assert(n % 2 == 0 && n <= 16, "n must be even and <= 16");
     static_assert(NW * 32 <= ES, "the second-pass rows of H must fit in the field buffer they replace");
@@ -127,7 +131,7 @@ struct WkCfg {
 template <int n, bool SPLIT>
 struct WkSmem {
     using Cfg = WkCfg<n>;
-    static constexpr int HSTRIDE = SPLIT ? Cfg::HA : Cfg::HS;
+    static constexpr int HSTRIDE = SPLIT ? Cfg::HA : Cfg::GS;
     static constexpr size_t BYTES = sizeof(float) * (size_t)(Cfg::SPOTS * Cfg::ES + Cfg::SPOTS * HSTRIDE) + sizeof(int4) * Cfg::SPOTS;
     static constexpr int BY_SMEM = (int)((227 * 1024) / (BYTES + 1024));
     /* the plain n = 16 instance needs 196 registers x 256 threads: one CTA per SM whatever the memory says */
@@ -243,9 +247,9 @@ __device__ __forceinline__ void rowself_acc(const float *__restrict__ p, LagAcc<
 }
 
 /* S = G * M aliased onto lx mod 16, 16-point x-transform, H[ly][0..15] -> shared memory */
-template <int n>
+template <int n, bool F2 = false>
 __device__ __forceinline__ void finish_row(const float2 (&acc)[2 * n - 1], const float2 *__restrict__ Mrow,
-                                           float *__restrict__ hrow, bool accumulate = false)
+                                           float *__restrict__ hrow)
 {
     float sr[16], si[16];
 #pragma unroll
@@ -273,12 +277,12 @@ __device__ __forceinline__ void finish_row(const float2 (&acc)[2 * n - 1], const
 #pragma unroll
     for (int C = 0; C < 16; C += 2) {
         const int p0 = fft_out_index<16>(C), p1 = fft_out_index<16>(C + 1);
-        float4 v = make_float4(sr[p0], si[p0], sr[p1], si[p1]);
-        if (accumulate) {                        /* sub-layer arrays are piled up (linear up to H) */
-            const float4 o = reinterpret_cast<float4 *>(hrow)[C / 2];
-            v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w;
+        if (F2) {                                /* 8-byte aligned row (multi-layer instances) */
+            reinterpret_cast<float2 *>(hrow)[C] = make_float2(sr[p0], si[p0]);
+            reinterpret_cast<float2 *>(hrow)[C + 1] = make_float2(sr[p1], si[p1]);
+        } else {
+            reinterpret_cast<float4 *>(hrow)[C / 2] = make_float4(sr[p0], si[p0], sr[p1], si[p1]);
         }
-        reinterpret_cast<float4 *>(hrow)[C / 2] = v;
     }
 }
 
@@ -424,9 +428,22 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkSmem<n, (EXTK < 2)>::MIN_
                 /* first pass: row slot = warp in the H buffer; second pass: same slot in the field buffer,
                  * once every warp has finished reading the field */
                 if (pass == 1) __syncthreads();
-                finish_row<n>(acc, Mi + ly * Cfg::LX, (pass == 0 ? hb : ebuf + lane * Cfg::ES) + warp * 32, false);
+                finish_row<n>(acc, Mi + ly * Cfg::LX, (pass == 0 ? hb : ebuf + lane * Cfg::ES) + warp * 32);
             } else {
-                finish_row<n>(acc, Mi + ly * Cfg::LX, hb + ly * 32, EXT && layer > 0);
+                /* several sub-layers: everything up to the table product is linear in the intensity, so the raw
+                 * lag row piles up in shared memory and only the last sub-layer pays the table product and
+                 * the x-transform (whose 16 complex values then take the row's place) */
+                float2 *grow = reinterpret_cast<float2 *>(hb + ly * Cfg::RS);
+                if (layer > 0) {
+#pragma unroll
+                    for (int a = 0; a < Cfg::LX; ++a) { const float2 g = grow[a]; acc[a].x += g.x; acc[a].y += g.y; }
+                }
+                if (layer + 1 < n_layers) {
+#pragma unroll
+                    for (int a = 0; a < Cfg::LX; ++a) grow[a] = acc[a];
+                } else {
+                    finish_row<n, true>(acc, Mi + ly * Cfg::LX, hb + ly * Cfg::RS);
+                }
             }
         }
     }
@@ -444,7 +461,7 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkSmem<n, (EXTK < 2)>::MIN_
             for (int m = 0; m < 16; ++m) {
                 if (m < n) {
                     /* lag row m sits in slot m (first pass), 0 (m = n/2) or n - m (second pass) */
-                    const float *src = !SPLIT ? hb + m * 32
+                    const float *src = !SPLIT ? hb + m * Cfg::RS
                                      : m < n / 2 ? hb + m * 32 : hb2 + (m == n / 2 ? 0 : n - m) * 32;
                     const float2 v = *reinterpret_cast<const float2 *>(src);
                     yr[m] = v.x; yi[m] = v.y;
