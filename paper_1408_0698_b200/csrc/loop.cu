@@ -140,16 +140,27 @@ void launch_dm_phase(shwfs_handle *h, const float *coef, int ldc, int T, float *
         coef, ldc, h->d_dm_modes, T, h->nsub, h->dm_M, out);
 }
 
-template <int NN>
+template <int NN, int FMAX>
 __global__ void dm_phase_gemv_kernel(const float *__restrict__ coef, int ldc, const float *__restrict__ modes_sub,
                                      int T, int nsub, int M, float *__restrict__ out);
+
+template <int NN, int FMAX>
+void launch_dm_gemv(shwfs_handle *h, const float *coef, int ldc, int T, float *out, cudaStream_t st)
+{
+    dm_phase_gemv_kernel<NN, FMAX><<<(unsigned)((h->nsub + 7) / 8), 256, sizeof(float) * FMAX * (size_t)h->dm_M, st>>>(
+        coef, ldc, h->d_dm_modes, T, h->nsub, h->dm_M, out);
+}
 
 template <int NN>
 void launch_dm_phase_n(shwfs_handle *h, const float *coef, int ldc, int T, float *out, cudaStream_t st)
 {
     if (T <= 8 && (size_t)h->dm_M * 8 * sizeof(float) <= 48 * 1024) {
-        dm_phase_gemv_kernel<NN><<<(unsigned)((h->nsub + 7) / 8), 256, sizeof(float) * 8 * (size_t)h->dm_M, st>>>(
-            coef, ldc, h->d_dm_modes, T, h->nsub, h->dm_M, out);
+        /* accumulators for exactly as many frames as needed: the T = 1 loop step keeps 1 + 8 float4 live and
+         * fits five CTAs per SM, i.e. the whole table in one wave */
+        if (T == 1) launch_dm_gemv<NN, 1>(h, coef, ldc, T, out, st);
+        else if (T == 2) launch_dm_gemv<NN, 2>(h, coef, ldc, T, out, st);
+        else if (T <= 4) launch_dm_gemv<NN, 4>(h, coef, ldc, T, out, st);
+        else launch_dm_gemv<NN, 8>(h, coef, ldc, T, out, st);
     } else if (T <= 8) launch_dm_phase<1, NN>(h, coef, ldc, T, out, st);
     else if (T <= 32) launch_dm_phase<4, NN>(h, coef, ldc, T, out, st);
     else launch_dm_phase<8, NN>(h, coef, ldc, T, out, st);
@@ -171,12 +182,12 @@ __global__ void dm_phase_simple_kernel(const float *__restrict__ coef, int ldc, 
 /* Few frames (the T = 1 loop step): the product is a matrix-vector one, bound by streaming the mode table
  * once.  One warp per subaperture, lane = float4 column, eight independent 16-byte loads in flight per lane,
  * the coefficients of the <= 8 frames broadcast from shared memory.                                      */
-template <int NN>
+template <int NN, int FMAX>
 __global__ void __launch_bounds__(256) dm_phase_gemv_kernel(const float *__restrict__ coef, int ldc,
                                                             const float *__restrict__ modes_sub, int T, int nsub,
                                                             int M, float *__restrict__ out)
 {
-    constexpr int NQ = NN / 4, MAXQ = (NQ + 31) / 32, FMAX = 8, UN = 8;
+    constexpr int NQ = NN / 4, MAXQ = (NQ + 31) / 32, UN = 8;
     extern __shared__ float gv_coef[];                       /* [M][FMAX] */
     for (int q = threadIdx.x; q < M * FMAX; q += 256) {
         const int m = q / FMAX, f = q - m * FMAX;
