@@ -177,13 +177,16 @@ int shwfs_set_noise(shwfs_handle *h, const shwfs_noise *nz);
  * Requires the lag-domain algorithm (EUNSUPPORTED otherwise), like shwfs_set_sodium; with sub-layers the
  * same DM phase is subtracted from every sub-layer's wavefront.
  *
- * shwfs_set_dm: modes_dev DEVICE [M*N*N] fp32; the library keeps its own per-subaperture re-layout
- * (nsub * M * n*n floats) and does not reference modes_dev after the call returns (it synchronises).
+ * shwfs_set_dm: modes_dev DEVICE [M*N*N] fp32; the library keeps its own per-subaperture re-layouts (nsub * M *
+ * n*n floats for the frame-by-frame loop, and -- for n*n in {64, 100, 256} -- about 2.3x that as hi|lo TF32
+ * operand tiles of the tcgen05 GEMM that serves batches of more than 8 frames) and does not reference modes_dev
+ * after the call returns (it synchronises).
  * M == 0 or modes_dev == NULL drops the DM.  Errors: EINVAL, EUNSUPPORTED, ENOMEM, ECUDA.               */
 int shwfs_set_dm(shwfs_handle *h, const float *modes_dev, int32_t M);
 
 /* shwfs_measure on the residual phase: coef_dev DEVICE [T*M].  Two kernels: the DM phase on the valid
- * subapertures (a batched GEMM into a T*nsub*n*n scratch in patch layout), then the sensor kernel, whose
+ * subapertures (a batched GEMM into a T*nsub*n*n scratch in patch layout: tensor cores with a 3-term TF32 split,
+ * fp32-like accuracy, for T > 8; an fp32 matrix-vector kernel below), then the sensor kernel, whose
  * gather subtracts it: the full-frame residual is never written to memory.  Enqueues on cuda_stream; may
  * (re)allocate the scratch the first time a larger T is seen (that call synchronises the stream once).
  * Errors: EINVAL (no DM set, null pointers, T < 0), ENOMEM, ECUDA.                                      */
