@@ -398,7 +398,7 @@ int pyrwfs_create(const pyrwfs_config *c, pyrwfs_handle **out)
         PY_TRY(cudaGetDevice(&h->device), "cudaGetDevice");
         const size_t per_frame = sizeof(float2) * (size_t)h->Kp * ((size_t)Np * N + (size_t)2 * N * Np) +
                                  sizeof(float) * ((size_t)4 * N * N + (size_t)4 * Sp * Sp);
-        size_t chunk = ((size_t)768 << 20) / per_frame;
+        size_t chunk = ((size_t)1536 << 20) / per_frame;
         if (chunk < 1) chunk = 1;
         if (chunk > 64) chunk = 64;
         h->chunk = (int)chunk;
