@@ -13,8 +13,9 @@
  * (LBO = bytes between the two 16-byte K chunks of one MMA, SBO = 128 bytes between 8-row groups):
  *     B = modes: [nsub][k-block][hi|lo][KB/4][NP/8][8][4]   built once per shwfs_set_dm (umma_split_modes_kernel)
  *     A = coef : [frame tile][k-block][hi|lo][KB/4][16][8][4] built per call              (umma_split_coef_kernel)
- * CTA = (subaperture, tile of 128 frames), 128 threads: thread 0 issues the bulk copies (3-stage ring) and the
- * MMAs (six per stage: two K steps x three split terms, M = 128, N = NP, K = 8), tcgen05.commit frees a stage /
+ * CTA = (subaperture, tile of 128 frames), 128 threads: thread 0 issues the bulk copies (3-stage ring of 8-mode
+ * stages: 46 KB, four CTAs and 4 x 128 TMEM columns per SM) and the MMAs (three per stage: the split terms,
+ * M = 128, N = NP, K = 8), tcgen05.commit frees a stage /
  * signals the epilogue; then every warp reads its 32 TMEM lanes (= frames) with tcgen05.ld and writes 16-byte
  * rows of the patch-layout output.  Used for T > 8; the T <= 8 loop step is the bandwidth-bound GEMV of loop.cu.
  */
@@ -22,7 +23,7 @@
 
 namespace {
 
-constexpr int UM_KB = 16;                  /* modes per stage */
+constexpr int UM_KB = 8;                   /* modes per stage */
 constexpr int UM_STAGES = 3;
 constexpr int UM_MT = 128;                 /* frames per CTA = UMMA M */
 
@@ -167,11 +168,11 @@ __global__ void __launch_bounds__(128) dm_umma_kernel(const float *__restrict__ 
                              ::"r"(tmem), "l"(dah), "l"(dbh), "r"(idesc), "r"(1u) : "memory");
             }
             asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&empty_bar[s])) : "memory");
-            /* refill the stage of the PREVIOUS k-block (its MMAs are done or about to be) with k-block kb+2 */
-            if (kb >= 1 && kb + 2 < nkb) {
+            /* refill the stage of the PREVIOUS k-block (its MMAs are done or about to be) with the k-block that comes UM_STAGES after it */
+            if (kb >= 1 && kb - 1 + UM_STAGES < nkb) {
                 const int sp = (kb - 1) % UM_STAGES;
                 mbar_wait(smem_u32(&empty_bar[sp]), (uint32_t)(((kb - 1) / UM_STAGES) & 1));
-                load(kb + 2);
+                load(kb - 1 + UM_STAGES);
             }
         }
         asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&done_bar)) : "memory");
