@@ -186,3 +186,28 @@ def test_residual_batches_on_the_tensor_cores(gpu, oracle, loop, cfg_id, M, T):
         want = loop.measure_residual(ph[ts], modes, coef[ts], amp, yx[sel], c.n, c.P, c.b, tau=c.tau,
                                      kernels=None if K is None else K[sel])
         assert np.abs(got[ts][:, sel] - want).max() <= SLOPE_TOL
+
+
+@pytest.mark.parametrize("n,P,b,T", [(5, 8, 1, 3), (12, 32, 2, 11), (6, 16, 1, 20)])
+def test_residual_on_sizes_without_a_templated_gemm(gpu, oracle, loop, n, P, b, T):
+    """Odd n (generic sensor kernel) and n*n outside {64, 100, 256}: the DM phase falls back to the
+    one-thread-per-output kernel, for the loop step (T <= 8) and for batches alike."""
+    torch, B = gpu
+    S, N, M = 3, 3 * n, 7
+    rng = np.random.default_rng(n * 10 + T)
+    amp = (rng.random((N, N)) > 0.15).astype(np.float32)
+    yx = np.array([[sy, sx] for sy in range(S) for sx in range(S)], dtype=np.int32)
+    ph = rng.normal(0, 1.5, (T, N, N)).astype(np.float32)
+    modes = rng.normal(0, 1.0, (M, N, N)).astype(np.float32)
+    coef = rng.normal(0, 0.4, (T, M)).astype(np.float32)
+    want = loop.measure_residual(ph, modes, coef, amp, yx, n, P, b, tau=0.1)
+    with B.Shwfs(amp, S, n, 0.05, W.LAMBDA_M, P, b, valid_yx=yx, threshold_frac=0.1) as s:
+        s.set_dm(torch.from_numpy(modes).cuda())
+        got = s.measure_residual(torch.from_numpy(ph).cuda(), torch.from_numpy(coef).cuda()).cpu().numpy()
+        assert np.abs(got - want).max() <= SLOPE_TOL
+        R = rng.normal(0, 1, (M, 2 * len(yx))).astype(np.float32) / len(yx)
+        ws, wh, wc = loop.closed_loop(ph[:4], modes, R, 0.4, np.zeros(M), amp, yx, n, P, b, tau=0.1)
+        c0 = torch.zeros(M, device="cuda")
+        gs, gh = s.closed_loop(torch.from_numpy(ph[:4]).cuda(), torch.from_numpy(R).cuda(), 0.4, c0)
+        assert np.abs(gs.cpu().numpy() - ws).max() <= SLOPE_TOL
+        np.testing.assert_allclose(c0.cpu().numpy(), wc, rtol=0, atol=2e-4 * max(np.abs(wc).max(), 1e-3))
