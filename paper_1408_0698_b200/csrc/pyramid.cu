@@ -70,7 +70,7 @@ __device__ __forceinline__ void unscramble(float (&re)[R], float (&im)[R])
 /* One L = R*R point transform of the line owned by the R threads j = 0..R-1 (all in one warp).
  * In : re/im[m] = x[j + R m] (natural order; entries m >= NZ are zero).
  * Out: re/im[q] = X[p + R q], p = this thread's index (natural order).
- * X[k] = sum_x x[x] exp(SIGN 2 pi i x k / L).  `line` is this line's R*(R+1) float2 of shared memory.      */
+ * X[k] = sum_x x[x] exp(SIGN 2 pi i x k / L).  `line` is this line's R*(R+2) float2 of shared memory.      */
 template <int R, int SIGN, int NZ>
 __device__ __forceinline__ void line_fft(float (&re)[R], float (&im)[R], int j, float2 *__restrict__ line,
                                          const float2 *__restrict__ tw)
@@ -88,13 +88,13 @@ __device__ __forceinline__ void line_fft(float (&re)[R], float (&im)[R], int j, 
             b = a * ws + b * w.x;
             a = t;
         }
-        line[p * (R + 1) + j] = make_float2(a, b);
+        line[p * (R + 2) + j] = make_float2(a, b);
     }
     __syncwarp();
 #pragma unroll
-    for (int jj = 0; jj < R; ++jj) {
-        const float2 v = line[j * (R + 1) + jj];                        /* this thread is now p = j */
-        re[jj] = v.x; im[jj] = v.y;
+    for (int jj = 0; jj < R; jj += 2) {                                 /* this thread is now p = j */
+        const float4 v = *reinterpret_cast<const float4 *>(line + j * (R + 2) + jj);   /* row stride R+2: 16-byte rows */
+        re[jj] = v.x; im[jj] = v.y; re[jj + 1] = v.z; im[jj + 1] = v.w;
     }
     __syncwarp();
     fft_dif<R, SIGN, R>(re, im);
@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(PY_LINES * R) pyr_rows_kernel(const PyArgs A)
             }
         }
     }
-    line_fft<R, -1, NZ>(re, im, j, py_smem + b * R * (R + 1), A.tw);
+    line_fft<R, -1, NZ>(re, im, j, py_smem + b * R * (R + 2), A.tw);
     __syncthreads();
     /* transposed hand-over: stage[u][b] (row padded to 9), then 64-byte segments of A1[tk][u][y0..y0+7] */
     float2 *stage = py_smem;
@@ -181,7 +181,7 @@ __global__ void __launch_bounds__(PY_LINES * R, 2) pyr_cols_kernel(const PyArgs 
         const int y = j + R * m;
         if (y < A.N) { const float2 v = __ldg(src + y); re[m] = v.x; im[m] = v.y; }
     }
-    float2 *line = py_smem + b * R * (R + 1);
+    float2 *line = py_smem + b * R * (R + 2);
     line_fft<R, -1, NZ>(re, im, j, line, A.tw);
     /* Q3: exp(-2 pi i s (|u~| + |v~|) / Np) at v = j + R q */
     const int ua = u < L / 2 ? u : L - u;
@@ -219,7 +219,7 @@ __global__ void __launch_bounds__(PY_LINES * R, 2) pyr_final_kernel(const PyArgs
     float acc[R];
 #pragma unroll
     for (int q = 0; q < R; ++q) acc[q] = 0.f;
-    float2 *line = py_smem + b * R * (R + 1);
+    float2 *line = py_smem + b * R * (R + 2);
     for (int k = 0; k < A.Kp; ++k) {
         float re[R], im[R];
         const float2 *src = A.A2 + (((size_t)t * A.Kp + k) * rows + (live ? r : 0)) * L;
@@ -295,8 +295,8 @@ cudaError_t run_chunk(pyrwfs_handle *h, const float *phase, int Tc, float *signa
     A.N = h->N; A.Np = h->Np; A.s = h->s; A.Kp = h->Kp; A.Tc = Tc;
     A.turns = (float)((double)h->c_phi / 6.283185307179586476925286766559);
     A.scale = (float)(1.0 / ((double)h->Kp * pow((double)h->Np, 4.0)));
-    const size_t smem = sizeof(float2) * (size_t)(L * (PY_LINES + 1) > PY_LINES * R * (R + 1) ? L * (PY_LINES + 1)
-                                                                                              : PY_LINES * R * (R + 1));
+    const size_t smem = sizeof(float2) * (size_t)(L * (PY_LINES + 1) > PY_LINES * R * (R + 2) ? L * (PY_LINES + 1)
+                                                                                              : PY_LINES * R * (R + 2));
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(pyr_rows_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
