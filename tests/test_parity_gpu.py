@@ -315,3 +315,26 @@ def test_full_batch_sampled_spots_other_configs(gpu, oracle, cfg_id):
         want = oracle.measure(frame, amp, yx[idx], c.n, c.P, c.b, tau=c.tau, kernels=K)
         err = np.abs(got[t, idx] - want[0]).max()
         assert err <= SLOPE_TOL, (cfg_id, int(t), err)
+
+
+@pytest.mark.parametrize("cfg_id", [4, 5])
+def test_all_six_wfs_frames_0_1_499_999_in_full(gpu, oracle, cfg_id):
+    """SURVEY.md 8(d) parity subset for configs 4-5: all six WFS (six launch points, independent seeded
+    screens), frames {0, 1, 499, 999} of the 1000-frame stream, EVERY spot (6 x 4 x 4632 = 111 168 per config)
+    against the oracle on the numpy-recipe frames."""
+    torch, B = gpu
+    c = W.CONFIGS[cfg_id]
+    amp = W.pupil_mask(c)
+    yx = oracle.valid_list(amp, c.n, c.min_illum)
+    frames = [0, 1, 499, 999]
+    worst = 0.0
+    for w in range(c.W):
+        ph = W.phase_frames(c, w, frames)
+        K = W.elongation_kernels(c, w, yx, device=torch.device("cuda")).cpu().numpy()
+        want = oracle.measure(ph, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K)
+        with B.Shwfs(amp, c.S, c.n, c.dx, W.LAMBDA_M, c.P, c.b, valid_yx=yx, threshold_frac=c.tau, elong_kernels=K) as s:
+            got = s.measure(torch.from_numpy(ph).cuda()).cpu().numpy()
+        err = float(np.abs(got - want).max())
+        worst = max(worst, err)
+        assert err <= SLOPE_TOL, (cfg_id, w, err)
+    assert worst <= 1e-4          # measured margin: two orders below the tolerance
