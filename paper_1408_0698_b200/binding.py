@@ -20,7 +20,7 @@ _PKG = Path(__file__).resolve().parent
 LIB_PATH = _PKG / "libshwfs.so"
 
 SHWFS_OK, SHWFS_EINVAL, SHWFS_EUNSUPPORTED, SHWFS_ENOMEM, SHWFS_ECUDA = 0, -1, -2, -3, -4
-ALGO_AUTO, ALGO_LITERAL, ALGO_WK, ALGO_WK_GENERIC, ALGO_PRUNED_FFT = 0, 1, 2, 3, 4
+ALGO_AUTO, ALGO_LITERAL, ALGO_WK, ALGO_WK_GENERIC, ALGO_PRUNED_FFT, ALGO_WK_FFT = 0, 1, 2, 3, 4, 5
 
 EXPORTS = ["shwfs_create", "shwfs_measure", "shwfs_measure_host", "shwfs_destroy", "shwfs_num_subaps",
            "shwfs_valid_list", "shwfs_pixel_scale", "shwfs_set_algorithm", "shwfs_get_algorithm",

@@ -14,7 +14,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libshwfs.so"
-SOURCES = ["api.cu", "wk.cu", "literal.cu", "pruned_fft.cu", "loop.cu", "pyramid.cu", "dm_umma.cu"]
+SOURCES = ["api.cu", "wk.cu", "wk_fft.cu", "literal.cu", "pruned_fft.cu", "loop.cu", "pyramid.cu", "dm_umma.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

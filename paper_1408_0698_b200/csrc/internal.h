@@ -95,6 +95,7 @@ cudaError_t shwfs_loop_dm_phase(shwfs_handle *h, const float *coef, int ldc, int
 cudaError_t shwfs_loop_reconstruct(const float *R, const float *slopes, int T, int K, int M, float gain,
                                    float *coef, int ldc, float *hist_or_null, cudaStream_t st);
 int shwfs_wk_supported(const shwfs_handle *h, int generic);
+int shwfs_wk_fft_supported(const shwfs_handle *h);   /* wk_fft.cu: autocorrelation by FFT (n = 16) */
 
 /* Literal chain: P x P FFT(s) in shared memory/registers.  stage < 0: slopes only.
  * stage 0/1/2 also writes that image to `img`.                                              */

@@ -24,6 +24,7 @@
 #include "field.cuh"
 #include "cog.cuh"
 #include "noise.cuh"
+#include "wk_common.cuh"
 
 namespace {
 
@@ -138,31 +139,6 @@ struct WkSmem {
     static constexpr int MIN_CTAS = n == 16 ? 1 : (BY_SMEM < 1 ? 1 : BY_SMEM);
 };
 
-struct WkArgs {
-    const float *phase;
-    const float *amp;
-    const int2 *valid;
-    const float2 *M;
-    float *slopes;
-    float *binned;
-    long long frame_stride;
-    int T, N, nsub, mstride, total, mode;
-    float tau, turns, ramp_unit;
-    /* paper's full LGS model (EXT instances only): sodium sub-layers and detector noise */
-    const float2 *sod_g;         /* [L][nsub] local gradient of the sub-layer's analytic phase, turns/pixel */
-    float *noisy;                /* stage-3 debug image (binned, after noise) or null                       */
-    long long layer_stride;      /* elements between sub-layers of one frame (0: shared wavefront)          */
-    int L;
-    float sod_q[SHWFS_MAX_LAYERS];   /* curvature a_l dx^2 / 2pi, turns/pixel^2                             */
-    float sod_sw[SHWFS_MAX_LAYERS];  /* sqrt(w_l): folded into the amplitude                                */
-    float flux, ron2;
-    uint2 key;
-    unsigned t0;
-    /* closed-loop neighbour (EXT instances only): residual = wavefront - DM phase.  The DM
-     * phase sum_m coef[t][m] * mode[m] arrives in patch layout from dm_phase_kernel (loop.cu).          */
-    const float *dm_patch;       /* [T][nsub][n*n] or null */
-};
-
 template <int n>
 __device__ __forceinline__ void load_row(const float *__restrict__ p, float (&r)[2 * n])
 {
@@ -242,46 +218,6 @@ __device__ __forceinline__ void rowself_acc(const float *__restrict__ p, LagAcc<
             const int a = k2 - k + n - 1;
             A.xy[a] = __ffma2_rn(e[k], e[k2], A.xy[a]);
             if (k2 > k) A.z[a] = fmaf(s[k], t[k2], A.z[a]);
-        }
-    }
-}
-
-/* S = G * M aliased onto lx mod 16, 16-point x-transform, H[ly][0..15] -> shared memory */
-template <int n, bool F2 = false>
-__device__ __forceinline__ void finish_row(const float2 (&acc)[2 * n - 1], const float2 *__restrict__ Mrow,
-                                           float *__restrict__ hrow)
-{
-    float sr[16], si[16];
-#pragma unroll
-    for (int m = 0; m < 16; ++m) {
-        bool first = true;
-        sr[m] = 0.f; si[m] = 0.f;
-#pragma unroll
-        for (int pass = 0; pass < 2; ++pass) {
-            const int lx = pass == 0 ? m : m - 16;
-            if (lx > n - 1 || lx < -(n - 1)) continue;
-            const int a = lx + n - 1;
-            const float2 mv = __ldg(Mrow + a);
-            const float gr = acc[a].x, gi = acc[a].y;
-            if (first) {
-                sr[m] = fmaf(gr, mv.x, -gi * mv.y);
-                si[m] = fmaf(gr, mv.y, gi * mv.x);
-                first = false;
-            } else {
-                sr[m] = fmaf(gr, mv.x, fmaf(-gi, mv.y, sr[m]));
-                si[m] = fmaf(gr, mv.y, fmaf(gi, mv.x, si[m]));
-            }
-        }
-    }
-    fft_dif<16, +1>(sr, si);                     /* H[C] = sum_m s'[m] w_16^(C m) */
-#pragma unroll
-    for (int C = 0; C < 16; C += 2) {
-        const int p0 = fft_out_index<16>(C), p1 = fft_out_index<16>(C + 1);
-        if (F2) {                                /* 8-byte aligned row (multi-layer instances) */
-            reinterpret_cast<float2 *>(hrow)[C] = make_float2(sr[p0], si[p0]);
-            reinterpret_cast<float2 *>(hrow)[C + 1] = make_float2(sr[p1], si[p1]);
-        } else {
-            reinterpret_cast<float4 *>(hrow)[C / 2] = make_float4(sr[p0], si[p0], sr[p1], si[p1]);
         }
     }
 }
@@ -691,6 +627,8 @@ cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *s
     A.ramp_unit = 0.5f / (float)h->P;
     if (A.total == 0) return cudaSuccess;
     h->launches += 1;
+    if (h->algo != SHWFS_ALGO_WK && !generic && shwfs_wk_fft_supported(h) && A.L <= 1)   /* explicit WK: direct sums */
+        return shwfs_wk_fft_launch(A, st);
     if (!generic) {
         switch (h->n) {
         case 8: return launch_special<8>(A, st);

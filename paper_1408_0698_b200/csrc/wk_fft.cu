@@ -1,0 +1,241 @@
+/*
+ * wk_fft.cu -- the lag-domain (Wiener-Khinchin) form of the Shack-Hartmann hot path for n = 16, with the
+ * autocorrelation of the field computed by FFT instead of by direct sums, sm_100a.
+ *
+ * Same operation as wk.cu (H1..H8 of include/shwfs.h; "the spot computed by FFT for each sensor
+ * sub-aperture ... a convolution for a gaussian ... the centroid computed on the final image"), same table M,
+ * same result to fp32 rounding.  What differs is how G[ly,lx] = sum_{j,k} e[j,k] conj(e[j+ly,k+lx]) is
+ * obtained: the direct sums cost n^2 (n+1)/2 * n = 32.9 k complex MACs per spot at n = 16 (92 k instructions,
+ * profiles/r01_wk16_full_v4.md); on a Q x Q grid with Q = 2n = 32 >= 2n-1 the aperiodic autocorrelation is
+ * the periodic one, G = DFT_Q(|DFT_Q(e)|^2) / Q^2, i.e. 80 line transforms of 32 points (~50 k instructions
+ * with everything around them).  The grid size is independent of the sensor's padding P: the identity of
+ * wk.cu's header holds for any P, and P enters only through the table M.
+ *
+ * Thread mapping: a half-warp per spot, 8 spots per CTA, no CTA-wide barrier; one 16 x 32 complex tile of
+ * shared memory per spot is reused by every exchange.
+ *   A  thread r owns patch row r: H1 gather (16-byte loads), H2 field (scaled by 2^-5.5 so that the
+ *      unnormalised transforms below need no further factor), 32-point FFT of the row (inputs >= 16 are zero)
+ *      -> tile[r][u]
+ *   B  thread c owns columns c and c + 16: 32-point FFT down each (16 non-zero inputs), S[v][u] = |.|^2; the
+ *      two columns run through one copy of the code (a rolled loop): the kernel is straight-line code of
+ *      ~3 k instructions per thread and stalls on instruction fetch (ncu: no_instructions first), so code
+ *      size counts -- rolling the two columns is worth 4 %, rolling A with B or C with D costs spills
+ *   C  the two real columns go through ONE complex transform z = S[.][c] + i S[.][c+16]; the transforms
+ *      g_u[ly] of the two columns are separated by the Hermitian symmetry of each (ly = 0..15 is all that
+ *      is needed: G[-l] = conj G[l] is folded into M) -> tile[ly][u]
+ *   D  thread ly owns lag row ly: 32-point FFT over u -> G[ly][lx], lx = -15..15
+ *   E  table product with M_i[ly][.], alias lx mod 16, 16-point x-transform (finish_row of wk_common.cuh)
+ *      -> tile[ly][0..15]
+ *   F  thread C owns detector column C: 16-point y-transform (real part), optional detector noise, H7 + H8
+ *      (cog16) with half-warp shuffles; lane 0 writes the two slopes.
+ * Extensions of the single-layer instance of wk.cu (detector noise, DM residual, one sodium sub-layer) are
+ * carried; several sub-layers stay with wk.cu's multi-layer instance.
+ */
+#include "wk_common.cuh"
+#include "field.cuh"
+#include "cog.cuh"
+#include "noise.cuh"
+
+namespace {
+
+using namespace shwfs;
+
+constexpr int WF_N = 16;                       /* subaperture side                                   */
+constexpr int WF_Q = 32;                       /* transform grid side                                */
+constexpr int WF_THREADS = 128;
+constexpr int WF_SPOTS = WF_THREADS / 16;
+constexpr int WF_LD = 2 * WF_Q + 4;            /* floats per tile row; LD/4 odd => 16-byte row accesses conflict-free */
+constexpr int WF_TILE = WF_N * WF_LD;
+constexpr size_t WF_SMEM = sizeof(float) * (size_t)WF_SPOTS * WF_TILE;
+constexpr int WF_LX = 2 * WF_N - 1;
+
+__device__ __forceinline__ constexpr int xq(int k) { return fft_out_index<WF_Q>(k & (WF_Q - 1)); }
+
+template <int MODE, bool EXT>
+__global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
+{
+    constexpr int n = WF_N, Q = WF_Q, LD = WF_LD;
+    extern __shared__ __align__(16) float wf_smem[];
+    const int tid = threadIdx.x, sp = tid >> 4, r = tid & 15;
+    float *tile = wf_smem + sp * WF_TILE;
+
+    const int g = blockIdx.x * WF_SPOTS + sp;
+    const bool live = g < A.total;
+    int i = 0, t = 0;
+    if (live) { i = g / A.T; t = g - i * A.T; }
+
+    float re[Q], im[Q];
+
+    /* ---- A: gather, field, row transform ---- */
+    {
+        float4 ph[n / 4], am[n / 4];
+#pragma unroll
+        for (int q = 0; q < n / 4; ++q) { ph[q] = make_float4(0.f, 0.f, 0.f, 0.f); am[q] = ph[q]; }
+        if (live) {
+            const int2 yx = __ldg(A.valid + i);
+            const int off = (yx.x * n + r) * A.N + yx.y * n;
+            const float4 *pp = reinterpret_cast<const float4 *>(A.phase + (size_t)t * A.frame_stride + off);
+            const float4 *pa = reinterpret_cast<const float4 *>(A.amp + off);
+#pragma unroll
+            for (int q = 0; q < n / 4; ++q) { ph[q] = __ldg(pp + q); am[q] = __ldg(pa + q); }
+            if (EXT && A.dm_patch != nullptr) {
+                /* PAPER.md:76 "the residual phase (the open loop wavefront subtracted by the DM)" */
+                const float4 *pd = reinterpret_cast<const float4 *>(A.dm_patch + ((size_t)t * A.nsub + i) * (n * n) + r * n);
+#pragma unroll
+                for (int q = 0; q < n / 4; ++q) {
+                    const float4 d = __ldg(pd + q);
+                    ph[q].x -= d.x; ph[q].y -= d.y; ph[q].z -= d.z; ph[q].w -= d.w;
+                }
+            }
+        }
+        /* 2^-5.5 on the field = 1/2048 on the intensity: 1/Q^2 of the two unnormalised transforms of S and the
+         * 1/2 of the real-pair separation of step C */
+        float sc = 0.02209708691207961f;
+        float lin0 = 0.f, gx = 0.f, lq = 0.f, dj2 = 0.f;
+        const bool sodium = EXT && A.L > 0;
+        if (sodium) {
+            /* the sub-layer's analytic phase in turns (reading B1): g . d + q |d|^2, d from the patch centre */
+            const float2 gr = __ldg(A.sod_g + i);
+            const float dj = (float)r - 0.5f * (float)(n - 1);
+            lq = A.sod_q[0];
+            gx = gr.x;
+            lin0 = fmaf(gr.y, dj, gr.x * (-0.5f * (float)(n - 1)));
+            dj2 = dj * dj;
+            sc *= A.sod_sw[0];
+        }
+        const float pv[n] = {ph[0].x, ph[0].y, ph[0].z, ph[0].w, ph[1].x, ph[1].y, ph[1].z, ph[1].w,
+                             ph[2].x, ph[2].y, ph[2].z, ph[2].w, ph[3].x, ph[3].y, ph[3].z, ph[3].w};
+        const float av[n] = {am[0].x, am[0].y, am[0].z, am[0].w, am[1].x, am[1].y, am[1].z, am[1].w,
+                             am[2].x, am[2].y, am[2].z, am[2].w, am[3].x, am[3].y, am[3].z, am[3].w};
+#pragma unroll
+        for (int k = 0; k < n; ++k) {
+            float ramp = (float)(r + k) * A.ramp_unit;
+            if (sodium) {
+                const float dk = (float)k - 0.5f * (float)(n - 1);
+                ramp -= fmaf(gx, (float)k, lin0) + lq * (dj2 + dk * dk);
+            }
+            const float2 e = field_value(pv[k], av[k] * sc, A.turns, ramp);
+            re[k] = e.x; im[k] = e.y;
+        }
+#pragma unroll
+        for (int k = n; k < Q; ++k) { re[k] = 0.f; im[k] = 0.f; }
+        fft_dif<Q, -1, n>(re, im);
+        float4 *row = reinterpret_cast<float4 *>(tile + r * LD);
+#pragma unroll
+        for (int q = 0; q < Q / 2; ++q)
+            row[q] = make_float4(re[xq(2 * q)], im[xq(2 * q)], re[xq(2 * q + 1)], im[xq(2 * q + 1)]);
+    }
+    __syncwarp();
+
+    /* ---- B: column transforms of columns r and r + 16, intensity ---- */
+    float zr[Q], zi[Q];
+#pragma unroll 1                                 /* one copy of the transform's code: the kernel is instruction-fetch bound */
+    for (int col = 0; col < 2; ++col) {
+        const float2 *colp = reinterpret_cast<const float2 *>(tile) + r + 16 * col;
+#pragma unroll
+        for (int v = 0; v < n; ++v) {
+            const float2 f = colp[v * (LD / 2)];
+            re[v] = f.x; im[v] = f.y;
+        }
+#pragma unroll
+        for (int v = n; v < Q; ++v) { re[v] = 0.f; im[v] = 0.f; }
+        fft_dif<Q, -1, n>(re, im);
+#pragma unroll
+        for (int v = 0; v < Q; ++v) {
+            const float s = fmaf(re[xq(v)], re[xq(v)], im[xq(v)] * im[xq(v)]);
+            zi[v] = s;
+        }
+        if (col == 0) {
+#pragma unroll
+            for (int v = 0; v < Q; ++v) zr[v] = zi[v];
+        }
+    }
+    __syncwarp();                                /* every thread has read its columns: the tile can be rewritten */
+
+    /* ---- C: both real columns in one complex transform over v, separated by symmetry ---- */
+    fft_dif<Q, -1>(zr, zi);
+    {
+        float2 *colp = reinterpret_cast<float2 *>(tile) + r;
+#pragma unroll
+        for (int ly = 0; ly < n; ++ly) {
+            const int a = xq(ly), b = xq(Q - ly);
+            /* Z[ly] = g1[ly] + i g2[ly], conj Z[-ly] = g1[ly] - i g2[ly]  (the 1/2 is in the field's scale) */
+            colp[ly * (LD / 2)] = make_float2(zr[a] + zr[b], zi[a] - zi[b]);
+            colp[ly * (LD / 2) + 16] = make_float2(zi[a] + zi[b], zr[b] - zr[a]);
+        }
+    }
+    __syncwarp();
+
+    /* ---- D: lag row r: transform over u ---- */
+    {
+        const float4 *row = reinterpret_cast<const float4 *>(tile + r * LD);
+#pragma unroll
+        for (int q = 0; q < Q / 2; ++q) {
+            const float4 f = row[q];
+            re[2 * q] = f.x; im[2 * q] = f.y; re[2 * q + 1] = f.z; im[2 * q + 1] = f.w;
+        }
+        fft_dif<Q, -1>(re, im);
+    }
+    /* ---- E: table product, alias, x-transform; H[r][0..15] takes the place of the row this thread read ---- */
+    {
+        float2 acc[WF_LX];
+#pragma unroll
+        for (int a = 0; a < WF_LX; ++a) acc[a] = make_float2(re[xq(a - (n - 1))], im[xq(a - (n - 1))]);
+        const float2 *Mi = A.M + (size_t)i * A.mstride;
+        finish_row<n>(acc, Mi + r * WF_LX, tile + r * LD);
+    }
+    __syncwarp();
+
+    /* ---- F: y-transform (real part), noise, threshold, centre of gravity ---- */
+    {
+        const int C = r;
+        float yr[16], yi[16];
+#pragma unroll
+        for (int m = 0; m < 16; ++m) {
+            const float2 v = *reinterpret_cast<const float2 *>(tile + m * LD + 2 * C);
+            yr[m] = v.x; yi[m] = v.y;
+        }
+        fft_dif<16, +1>(yr, yi);                 /* B[R,C] = Re sum_m H[m][C] w_16^(R m) */
+        float bcol[16];
+#pragma unroll
+        for (int R = 0; R < 16; ++R) bcol[R] = yr[fft_out_index<16>(R)];
+        const size_t o = (size_t)t * A.nsub + i;
+        if (live && A.binned) {
+#pragma unroll
+            for (int R = 0; R < 16; ++R) A.binned[(o * 16 + R) * 16 + C] = bcol[R];
+        }
+        if (EXT && A.flux > 0.f) {
+            add_noise_col16(bcol, C, A.key, A.t0 + (unsigned)t, (unsigned)i, A.flux, A.ron2);
+            if (live && A.noisy) {
+#pragma unroll
+                for (int R = 0; R < 16; ++R) A.noisy[(o * 16 + R) * 16 + C] = bcol[R];
+            }
+        }
+        const float2 sl = cog16<MODE>(bcol, C, A.tau);
+        if (live && C == 0) reinterpret_cast<float2 *>(A.slopes)[o] = sl;
+    }
+}
+
+template <int MODE, bool EXT>
+cudaError_t launch_wkf(const WkArgs &A, cudaStream_t st)
+{
+    const int grid = (A.total + WF_SPOTS - 1) / WF_SPOTS;
+    wkf16_kernel<MODE, EXT><<<grid, WF_THREADS, WF_SMEM, st>>>(A);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+int shwfs_wk_fft_supported(const shwfs_handle *h)
+{
+    return h->D == 16 && h->n == 16 && h->N % 4 == 0;
+}
+
+/* A.L <= 1 (several sub-layers: wk.cu's multi-layer instance) */
+cudaError_t shwfs_wk_fft_launch(const shwfs::WkArgs &A, cudaStream_t st)
+{
+    static_assert(WF_SMEM <= 48 * 1024, "static limit of dynamic shared memory");
+    const bool ext = A.L > 0 || A.flux > 0.f || A.dm_patch != nullptr;
+    if (ext) return A.mode == 0 ? launch_wkf<0, true>(A, st) : launch_wkf<1, true>(A, st);
+    return A.mode == 0 ? launch_wkf<0, false>(A, st) : launch_wkf<1, false>(A, st);
+}

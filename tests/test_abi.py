@@ -164,7 +164,7 @@ def test_measure_rejects_bad_arguments_and_queries(gpu):
         assert L.shwfs_num_subaps(s._h, None) == B.SHWFS_EINVAL
         assert s.nsub == 80
         assert abs(s.pixel_scale - c.b * W.LAMBDA_M / (c.P * c.dx)) < 1e-12   # float dx, lambda
-        assert s.algorithm in (B.ALGO_LITERAL, B.ALGO_WK, B.ALGO_WK_GENERIC, B.ALGO_PRUNED_FFT)
+        assert s.algorithm in (B.ALGO_LITERAL, B.ALGO_WK, B.ALGO_WK_GENERIC, B.ALGO_PRUNED_FFT, B.ALGO_WK_FFT)
         yx = s.valid_yx
         assert yx.shape == (80, 2) and (np.diff(yx[:, 0] * c.S + yx[:, 1]) > 0).all()   # row-major order
 

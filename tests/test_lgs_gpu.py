@@ -20,7 +20,7 @@ def _img_err(got, want):
 
 def _wk_algos(s, B):
     out = []
-    for a in (B.ALGO_WK, B.ALGO_WK_GENERIC):
+    for a in (B.ALGO_WK, B.ALGO_WK_GENERIC, B.ALGO_WK_FFT):
         try:
             s.algorithm = a
             out.append(a)
@@ -53,6 +53,7 @@ def test_config3_sublayers_match_oracle(gpu, oracle, L, shared):
                      shared_phase=shared)
         phd = torch.from_numpy(ph).cuda()
         for a in _wk_algos(s, B):
+            s.algorithm = a
             l0 = s.launch_count
             got = s.measure(phd).cpu().numpy()
             assert s.launch_count == l0 + 1                     # all sub-layers in ONE launch
@@ -89,6 +90,7 @@ def test_config3_noise_matches_oracle(gpu, oracle):
         s.set_noise(F, ron, seed)
         phd = torch.from_numpy(ph).cuda()
         for a in _wk_algos(s, B):
+            s.algorithm = a
             got = s.measure(phd).cpu().numpy()
             img = s.debug_spots(phd, 3).cpu().numpy()
             assert _img_err(img, wimg) <= IMAGE_TOL, (a, _img_err(img, wimg))
@@ -98,6 +100,7 @@ def test_config3_noise_matches_oracle(gpu, oracle):
         w1, i1 = oracle.measure_lgs(ph, amp, yx, c.n, c.P, c.b, c.dx, weight=[1.0], defocus=[0.0], tau=c.tau,
                                     kernels=K, flux=F, ron=ron, seed=seed, stage=3)
         for a in _wk_algos(s, B):
+            s.algorithm = a
             got = s.measure(phd).cpu().numpy()
             img = s.debug_spots(phd, 3).cpu().numpy()
             assert _img_err(img, i1) <= IMAGE_TOL, (a, _img_err(img, i1))
@@ -132,7 +135,7 @@ def test_small_grids_sublayers_and_noise(gpu, oracle, n, P, b):
     K = rng.random((len(yx), P, P)).astype(np.float32)
     T = 5
     for L, shared, tau, mode, F in ((1, True, 0.0, 0, 0.0), (2, False, 0.1, 0, 0.0), (4, False, 0.1, 0, 30.0),
-                                    (3, True, 0.2, 1, 0.0)):
+                                    (3, True, 0.2, 1, 0.0), (1, False, 0.1, 0, 30.0)):
         ph = rng.normal(0, 2.0, (T, N, N) if shared else (T, L, N, N)).astype(np.float32)
         w = rng.uniform(0.1, 1.0, L)
         de = rng.normal(0, 40.0, L)                      # rad/m^2: up to ~20 rad across the 3n-pixel pupil
@@ -149,6 +152,7 @@ def test_small_grids_sublayers_and_noise(gpu, oracle, n, P, b):
             algos = _wk_algos(s, B)
             assert B.ALGO_WK_GENERIC in algos
             for a in algos:
+                s.algorithm = a
                 got = s.measure(phd).cpu().numpy()
                 img = s.debug_spots(phd, 3).cpu().numpy()
                 lit = wimg.max(axis=(2, 3)) > 0

@@ -18,7 +18,7 @@ def loop():
 
 def _wk_algos(s, B):
     out = []
-    for a in (B.ALGO_WK, B.ALGO_WK_GENERIC):
+    for a in (B.ALGO_WK, B.ALGO_WK_GENERIC, B.ALGO_WK_FFT):
         try:
             s.algorithm = a
             out.append(a)
@@ -46,6 +46,7 @@ def test_residual_slopes_match_oracle(gpu, oracle, loop, cfg_id, M, T):
         s.set_dm(torch.from_numpy(modes).cuda())
         phd, cd = torch.from_numpy(ph).cuda(), torch.from_numpy(coef).cuda()
         for a in _wk_algos(s, B):
+            s.algorithm = a
             got = s.measure_residual(phd, cd).cpu().numpy()
             assert np.abs(got - want).max() <= SLOPE_TOL, (a, np.abs(got - want).max())
         # zero coefficients: the plain sensor
@@ -149,6 +150,7 @@ def test_residual_with_sublayers(gpu, oracle):
         s.set_sodium(w, de, None, None, (4.0, 0.0))
         s.set_dm(torch.from_numpy(modes).cuda())
         for a in _wk_algos(s, B):
+            s.algorithm = a
             got = s.measure_residual(torch.from_numpy(ph).cuda(), torch.from_numpy(coef).cuda()).cpu().numpy()
             assert np.abs(got - want).max() <= SLOPE_TOL, a
 

@@ -17,7 +17,7 @@ IMAGE_TOL = 1e-4      # fraction of the spot peak      (north_star)
 
 def _algos(sensor, B):
     out = []
-    for a in (B.ALGO_WK, B.ALGO_WK_GENERIC, B.ALGO_LITERAL, B.ALGO_PRUNED_FFT):
+    for a in (B.ALGO_WK, B.ALGO_WK_GENERIC, B.ALGO_LITERAL, B.ALGO_PRUNED_FFT, B.ALGO_WK_FFT):
         try:
             sensor.algorithm = a
             out.append(a)
