@@ -2,7 +2,7 @@
  * fft_regs.cuh -- register-resident power-of-two complex FFTs with compile-time twiddles.
  *
  * Every index is a compile-time constant after unrolling, so the arrays live in registers, the
- * bit-reversal is free (renaming) and multiplications by 1, +-i and (1+-i)/sqrt(2) are special-cased.
+ * bit-reversal is free (renaming) and multiplications by 1 and +-i are special-cased.
  * Used by the lag-domain D-point transforms (H6 of include/shwfs.h in Fourier form) and by the
  * literal P x P chain (H3, H5).  X[k] = sum_m x[m] exp(SIGN * 2*pi*i * m*k / L).
  */
@@ -37,83 +37,70 @@ __host__ __device__ constexpr int bitrev(int v, int bits)
     return r;
 }
 
-/* (re,im) *= exp(2*pi*i*K64/64), K64 compile-time */
-template <int K64>
-__device__ __forceinline__ void twiddle(float &re, float &im)
-{
-    constexpr int k = K64 & 63;
-    if constexpr (k == 0) {
-    } else if constexpr (k == 16) { float t = re; re = -im; im = t; }
-    else if constexpr (k == 32) { re = -re; im = -im; }
-    else if constexpr (k == 48) { float t = re; re = im; im = -t; }
-    else if constexpr (k == 8)  { float a = re, b = im; re = (a - b) * 0.70710678118654752f; im = (a + b) * 0.70710678118654752f; }
-    else if constexpr (k == 24) { float a = re, b = im; re = (a + b) * -0.70710678118654752f; im = (a - b) * 0.70710678118654752f; }
-    else if constexpr (k == 40) { float a = re, b = im; re = (b - a) * 0.70710678118654752f; im = (a + b) * -0.70710678118654752f; }
-    else if constexpr (k == 56) { float a = re, b = im; re = (a + b) * 0.70710678118654752f; im = (b - a) * 0.70710678118654752f; }
-    else {
-        constexpr float c = cos64(k), s = sin64(k);
-        float a = re, b = im;
-        re = fmaf(a, c, -b * s);
-        im = fmaf(a, s, b * c);
-    }
-}
-
-/* One decimation-in-frequency stage over blocks of LEN inside an L-point array.
- * NZ: inputs with index >= NZ are known to be zero (only honoured when LEN == L). */
-template <int L, int LEN, int SIGN, int NZ>
-__device__ __forceinline__ void dif_stage(float (&re)[L], float (&im)[L])
-{
-    constexpr int half = LEN / 2;
-#pragma unroll
-    for (int base = 0; base < L; base += LEN) {
-#pragma unroll
-        for (int q = 0; q < half; ++q) {
-            const int i0 = base + q, i1 = base + q + half;
-            float dr, di;
-            if (LEN == L && i1 >= NZ) {          /* second operand is zero: u+0, (u-0)*w */
-                if (LEN == L && i0 >= NZ) { re[i0] = 0.f; im[i0] = 0.f; re[i1] = 0.f; im[i1] = 0.f; continue; }
-                dr = re[i0]; di = im[i0];
+/* ---------------------------------------------------------------------------------------------------------
+ * Radix-2 decimation in time with fused multiply-adds.  A butterfly (a + w b, a - w b) with w = c + i s costs
+ * six FFMA when the twiddle is taken in tangent form, w b = c ((br - t bi) + i (bi + t br)), t = s / c
+ * (cotangent form when |c| < |s|), against four operations for the product and four for the sums: 388
+ * floating-point instructions at L = 32 (the decimation-in-frequency form this replaced compiled to ~440).
+ * The array is addressed through the bit reversal (element i of the decimated order lives in register
+ * bitrev(i)): natural-order input, output k at position fft_out_index<L>(k).  Inputs with index >= NZ are
+ * known zeros and are never read: a block whose inputs are all zero is skipped, a butterfly whose second
+ * operand is zero is a copy -- with NZ <= L/2 the whole first stage costs nothing.
+ * ------------------------------------------------------------------------------------------------------- */
+template <int L, int SIGN, int NZ, int S, int I>
+struct DitBf {
+    __device__ __forceinline__ static void run(float (&re)[L], float (&im)[L])
+    {
+        constexpr int bits = ilog2(L);
+        constexpr int h = 1 << (S - 1);
+        constexpr int j = I % h;
+        constexpr int i0 = (I / h) * 2 * h + j, i1 = i0 + h;
+        constexpr int p0 = bitrev(i0, bits), p1 = bitrev(i1, bits);
+        /* the block of h elements around i holds a partial transform of the inputs bitrev(block): all zero
+         * iff the smallest of them is >= NZ */
+        constexpr bool az = bitrev((i0 / h) * h, bits) >= NZ;
+        constexpr bool bz = bitrev((i1 / h) * h, bits) >= NZ;
+        constexpr int k64 = ((SIGN > 0 ? j : -j) * (64 / (2 * h))) & 63;
+        if constexpr (az) {
+            static_assert(!az || bz, "prefix of non-zero inputs");
+        } else if constexpr (bz) {
+            re[p1] = re[p0]; im[p1] = im[p0];
+        } else {
+            const float ar = re[p0], ai = im[p0], br = re[p1], bi = im[p1];
+            if constexpr (k64 == 0) {
+                re[p0] = ar + br; im[p0] = ai + bi; re[p1] = ar - br; im[p1] = ai - bi;
+            } else if constexpr (k64 == 16) {           /* w = +i: w b = (-bi, br) */
+                re[p0] = ar - bi; im[p0] = ai + br; re[p1] = ar + bi; im[p1] = ai - br;
+            } else if constexpr (k64 == 48) {           /* w = -i: w b = (bi, -br) */
+                re[p0] = ar + bi; im[p0] = ai - br; re[p1] = ar - bi; im[p1] = ai + br;
             } else {
-                float ur = re[i0], ui = im[i0], vr = re[i1], vi = im[i1];
-                re[i0] = ur + vr; im[i0] = ui + vi;
-                dr = ur - vr; di = ui - vi;
+                constexpr float c = cos64(k64), s = sin64(k64);
+                constexpr bool tanform = (c < 0 ? -c : c) >= (s < 0 ? -s : s);
+                if constexpr (tanform) {
+                    constexpr float t = (float)((double)s / (double)c);
+                    const float p = fmaf(-t, bi, br), q = fmaf(t, br, bi);
+                    re[p0] = fmaf(c, p, ar); im[p0] = fmaf(c, q, ai);
+                    re[p1] = fmaf(-c, p, ar); im[p1] = fmaf(-c, q, ai);
+                } else {
+                    constexpr float ct = (float)((double)c / (double)s);
+                    const float p = fmaf(ct, br, -bi), q = fmaf(ct, bi, br);
+                    re[p0] = fmaf(s, p, ar); im[p0] = fmaf(s, q, ai);
+                    re[p1] = fmaf(-s, p, ar); im[p1] = fmaf(-s, q, ai);
+                }
             }
-            re[i1] = dr; im[i1] = di;
         }
-    }
-}
-
-/* helper to apply the stage twiddles with compile-time indices */
-template <int L, int LEN, int SIGN, int BASE, int Q>
-struct TwApply {
-    __device__ __forceinline__ static void run(float (&re)[L], float (&im)[L])
-    {
-        constexpr int half = LEN / 2;
-        constexpr int k64 = ((SIGN > 0 ? Q : -Q) * (64 / LEN)) & 63;
-        twiddle<k64>(re[BASE + Q + half], im[BASE + Q + half]);
-        if constexpr (Q + 1 < half) TwApply<L, LEN, SIGN, BASE, Q + 1>::run(re, im);
-        else if constexpr (BASE + LEN < L) TwApply<L, LEN, SIGN, BASE + LEN, 0>::run(re, im);
+        if constexpr (I + 1 < L / 2) DitBf<L, SIGN, NZ, S, I + 1>::run(re, im);
+        else if constexpr ((1 << S) < L) DitBf<L, SIGN, NZ, S + 1, 0>::run(re, im);
     }
 };
 
-template <int L, int LEN, int SIGN, int NZ>
-struct DifRec {
-    __device__ __forceinline__ static void run(float (&re)[L], float (&im)[L])
-    {
-        dif_stage<L, LEN, SIGN, NZ>(re, im);
-        if constexpr (LEN > 2) {
-            TwApply<L, LEN, SIGN, 0, 0>::run(re, im);
-            DifRec<L, LEN / 2, SIGN, L>::run(re, im);
-        }
-    }
-};
-
-/* In-place L-point DIF FFT.  Output element k is left at position bitrev(k): use fft_out_index<L>(k). */
+/* In-place L-point FFT: X[k] = sum_m x[m] exp(SIGN 2 pi i m k / L) is left at position fft_out_index<L>(k). */
 template <int L, int SIGN, int NZ = L>
-__device__ __forceinline__ void fft_dif(float (&re)[L], float (&im)[L])
+__device__ __forceinline__ void fft_fma(float (&re)[L], float (&im)[L])
 {
     static_assert(L >= 2 && L <= 64 && (L & (L - 1)) == 0, "L must be a power of two <= 64");
-    DifRec<L, L, SIGN, NZ>::run(re, im);
+    static_assert(NZ >= 1 && NZ <= L, "at least one non-zero input");
+    DitBf<L, SIGN, NZ, 1, 0>::run(re, im);
 }
 
 template <int L>

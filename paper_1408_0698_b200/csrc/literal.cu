@@ -43,7 +43,7 @@ struct LitArgs {
 template <int L, int SIGN, int NZ = L>
 __device__ __forceinline__ void fft_nat(float (&re)[L], float (&im)[L])
 {
-    fft_dif<L, SIGN, NZ>(re, im);
+    fft_fma<L, SIGN, NZ>(re, im);
 #pragma unroll
     for (int k = 0; k < L; ++k) {
         const int q = fft_out_index<L>(k);

@@ -6,8 +6,8 @@
  * Steps H1 gather, H2 field, H3 zero-padded P x P DFT, H4 |.|^2/P^2, H6 centre + b x b bin, H7 threshold,
  * H8 centre of gravity of include/shwfs.h, D = P/b = 16 detector pixels per side.
  *
- * Thread mapping: 16 threads (a half-warp) per spot, 8 spots per tile, 4 tiles per CTA (the gather of the next
- * tile is issued before the column pass of the current one), no CTA-wide barrier.
+ * Thread mapping: 16 threads (a half-warp) per spot, 8 spots per tile, persistent CTAs striding over the tiles
+ * (the gather of the next tile is issued before the column pass of the current one), no CTA-wide barrier.
  *   row pass     thread r < n owns patch row r: 8-byte gathers, sincos, one P-point DIF FFT in registers
  *                whose inputs >= NZ are known zeros (first stage free); the n x P result goes to shared
  *                memory with the columns permuted (u -> (u mod b) * 16 + u / b) so that the column pass
@@ -71,7 +71,6 @@ __device__ __forceinline__ void pf_gather(const PfArgs &A, int off, int t, float
     }
 }
 
-constexpr int PF_TILES = 4;     /* tiles of 8 spots per CTA: the gather of tile k+1 flies during the column pass of k */
 
 template <int P, int NZ, int MODE>
 __global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel(const PfArgs A)
@@ -82,26 +81,28 @@ __global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel
     const int tid = threadIdx.x, sp = tid >> 4, r = tid & 15;
     float *tile = pf_smem + sp * Cfg::TILE;
 
-    /* patch-row offsets of all the CTA's tiles first: the valid-list lookups (the only dependent loads of the
-     * gather) are issued together, so that the prefetch below never waits on one in program order */
-    int offs[PF_TILES], tts[PF_TILES];
-#pragma unroll
-    for (int it = 0; it < PF_TILES; ++it) {
-        const int g = (blockIdx.x * PF_TILES + it) * PF_SPOTS + sp;
-        offs[it] = -1; tts[it] = 0;
-        if (g < A.total && r < A.n) {
-            const int i = g / A.T;
-            const int2 yx = __ldg(A.valid + i);
-            tts[it] = g - i * A.T;
-            offs[it] = (yx.x * A.n + r) * A.N + yx.y * A.n;
-        }
-    }
+    /* persistent CTAs: CTA b takes tiles b, b + gridDim.x, ... (the host sizes the grid to the resident CTAs of
+     * the device, so a launch has no ragged last wave).  Two tiles of look-ahead: the valid-list lookup (the
+     * only dependent load of the gather) of tile k+2 and the gather of tile k+1 fly during tile k. */
+    const int ntiles = (A.total + PF_SPOTS - 1) / PF_SPOTS;
+    auto row_offset = [&](int tile_id, int &tt) {
+        const int g = tile_id * PF_SPOTS + sp;
+        tt = 0;
+        if (tile_id >= ntiles || g >= A.total || r >= A.n) return -1;
+        const int i = g / A.T;
+        const int2 yx = __ldg(A.valid + i);
+        tt = g - i * A.T;
+        return (yx.x * A.n + r) * A.N + yx.y * A.n;
+    };
+    int tt0, tt1;
+    int off0 = row_offset(blockIdx.x, tt0);
+    int off1 = row_offset(blockIdx.x + gridDim.x, tt1);
     float2 ph[NZ / 2], am[NZ / 2];
-    pf_gather<NZ>(A, offs[0], tts[0], ph, am);
+    pf_gather<NZ>(A, off0, tt0, ph, am);
 
 #pragma unroll 1
-    for (int it = 0; it < PF_TILES; ++it) {
-        const int g = (blockIdx.x * PF_TILES + it) * PF_SPOTS + sp;
+    for (int tile_id = blockIdx.x; tile_id < ntiles; tile_id += gridDim.x) {
+        const int g = tile_id * PF_SPOTS + sp;
         const bool live = g < A.total;
         int i = 0, t = 0;
         if (live) { i = g / A.T; t = g - i * A.T; }
@@ -121,7 +122,7 @@ __global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel
                 }
 #pragma unroll
                 for (int k = NZ; k < P; ++k) { re[k] = 0.f; im[k] = 0.f; }
-                fft_dif<P, -1, NZ>(re, im);
+                fft_fma<P, -1, NZ>(re, im);
             } else {
 #pragma unroll
                 for (int k = 0; k < P; ++k) { re[k] = 0.f; im[k] = 0.f; }
@@ -138,9 +139,8 @@ __global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel
         }
         __syncwarp();
         /* H1 of the next tile: in flight during the column pass */
-        if (it + 1 < PF_TILES) pf_gather<NZ>(A, offs[1], tts[1], ph, am);
-#pragma unroll
-        for (int q = 0; q + 1 < PF_TILES; ++q) { offs[q] = offs[q + 1]; tts[q] = tts[q + 1]; }   /* rotate */
+        pf_gather<NZ>(A, off1, tt1, ph, am);
+        off1 = row_offset(tile_id + 2 * gridDim.x, tt1);
 
         /* ---- column pass: b columns per thread, |.|^2 and the row half of the bin in registers ---- */
         float acc[16];
@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel
             }
 #pragma unroll
             for (int v = NZ; v < P; ++v) { re[v] = 0.f; im[v] = 0.f; }
-            fft_dif<P, -1, NZ>(re, im);
+            fft_fma<P, -1, NZ>(re, im);
 #pragma unroll
             for (int R = 0; R < 16; ++R) {
 #pragma unroll
@@ -194,7 +194,16 @@ cudaError_t launch_pf_mode(const PfArgs &A, cudaStream_t st)
                                              (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
     }
-    const int grid = (A.total + PF_SPOTS * PF_TILES - 1) / (PF_SPOTS * PF_TILES);
+    const int ntiles = (A.total + PF_SPOTS - 1) / PF_SPOTS;
+    static int resident = 0;                       /* CTAs the device holds at once */
+    if (resident == 0) {
+        int dev = 0, sms = 0, per_sm = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pruned_fft_kernel<P, NZ, MODE>, PF_THREADS, Cfg::SMEM);
+        resident = sms * (per_sm > 0 ? per_sm : 1);
+    }
+    const int grid = ntiles < resident ? ntiles : resident;
     pruned_fft_kernel<P, NZ, MODE><<<grid, PF_THREADS, Cfg::SMEM, st>>>(A);
     return cudaGetLastError();
 }

@@ -76,7 +76,7 @@ __device__ __forceinline__ void line_fft(float (&re)[R], float (&im)[R], int j, 
                                          const float2 *__restrict__ tw)
 {
     constexpr int L = R * R;
-    fft_dif<R, SIGN, NZ>(re, im);
+    fft_fma<R, SIGN, NZ>(re, im);
 #pragma unroll
     for (int p = 0; p < R; ++p) {
         const int x = fft_out_index<R>(p);
@@ -97,7 +97,7 @@ __device__ __forceinline__ void line_fft(float (&re)[R], float (&im)[R], int j, 
         re[jj] = v.x; im[jj] = v.y; re[jj + 1] = v.z; im[jj + 1] = v.w;
     }
     __syncwarp();
-    fft_dif<R, SIGN, R>(re, im);
+    fft_fma<R, SIGN, R>(re, im);
     unscramble<R>(re, im);
 }
 

@@ -403,7 +403,7 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkSmem<n, (EXTK < 2)>::MIN_
                     yr[m] = v.x; yi[m] = v.y;
                 } else { yr[m] = 0.f; yi[m] = 0.f; }
             }
-            fft_dif<16, +1, n>(yr, yi);          /* B[R,C] = Re sum_m H[m][C] w_16^(R m) */
+            fft_fma<16, +1, n>(yr, yi);          /* B[R,C] = Re sum_m H[m][C] w_16^(R m) */
             float bcol[16];
 #pragma unroll
             for (int R = 0; R < 16; ++R) bcol[R] = yr[fft_out_index<16>(R)];

@@ -63,7 +63,7 @@ __device__ __forceinline__ void finish_row(const float2 (&acc)[2 * n - 1], const
             }
         }
     }
-    fft_dif<16, +1>(sr, si);                     /* H[C] = sum_m s'[m] w_16^(C m) */
+    fft_fma<16, +1>(sr, si);                     /* H[C] = sum_m s'[m] w_16^(C m) */
 #pragma unroll
     for (int C = 0; C < 16; C += 2) {
         const int p0 = fft_out_index<16>(C), p1 = fft_out_index<16>(C + 1);

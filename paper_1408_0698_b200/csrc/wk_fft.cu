@@ -119,7 +119,7 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
         }
 #pragma unroll
         for (int k = n; k < Q; ++k) { re[k] = 0.f; im[k] = 0.f; }
-        fft_dif<Q, -1, n>(re, im);
+        fft_fma<Q, -1, n>(re, im);
         float4 *row = reinterpret_cast<float4 *>(tile + r * LD);
 #pragma unroll
         for (int q = 0; q < Q / 2; ++q)
@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
         }
 #pragma unroll
         for (int v = n; v < Q; ++v) { re[v] = 0.f; im[v] = 0.f; }
-        fft_dif<Q, -1, n>(re, im);
+        fft_fma<Q, -1, n>(re, im);
 #pragma unroll
         for (int v = 0; v < Q; ++v) {
             const float s = fmaf(re[xq(v)], re[xq(v)], im[xq(v)] * im[xq(v)]);
@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
     __syncwarp();                                /* every thread has read its columns: the tile can be rewritten */
 
     /* ---- C: both real columns in one complex transform over v, separated by symmetry ---- */
-    fft_dif<Q, -1>(zr, zi);
+    fft_fma<Q, -1>(zr, zi);
     {
         float2 *colp = reinterpret_cast<float2 *>(tile) + r;
 #pragma unroll
@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
             const float4 f = row[q];
             re[2 * q] = f.x; im[2 * q] = f.y; re[2 * q + 1] = f.z; im[2 * q + 1] = f.w;
         }
-        fft_dif<Q, -1>(re, im);
+        fft_fma<Q, -1>(re, im);
     }
     /* ---- E: table product, alias, x-transform; H[r][0..15] takes the place of the row this thread read ---- */
     {
@@ -195,7 +195,7 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
             const float2 v = *reinterpret_cast<const float2 *>(tile + m * LD + 2 * C);
             yr[m] = v.x; yi[m] = v.y;
         }
-        fft_dif<16, +1>(yr, yi);                 /* B[R,C] = Re sum_m H[m][C] w_16^(R m) */
+        fft_fma<16, +1>(yr, yi);                 /* B[R,C] = Re sum_m H[m][C] w_16^(R m) */
         float bcol[16];
 #pragma unroll
         for (int R = 0; R < 16; ++R) bcol[R] = yr[fft_out_index<16>(R)];
