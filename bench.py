@@ -39,12 +39,12 @@ F_NOM = {1: 10240, 2: 51200, 3: 153600, 4: 153600, 5: 737280}
 # (profiles/r01_fp32_peak.md).
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 # sm__pipe_fma_cycles_active (fraction of peak) of the dominant kernel in the committed ncu --set full captures
-NCU_FMA_PIPE_ACTIVE = {2: 0.503, 3: 0.636, 4: 0.636, 5: 0.640}
+NCU_FMA_PIPE_ACTIVE = {2: 0.472, 3: 0.636, 4: 0.636, 5: 0.618}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/r01_wk10_full_v5.md, r01_wk16_full_v4.md, r01_pf32_full.md), keyed by config; None where no
+# `ncu --set full` captures (profiles/r01_wk10_full_v5.md, r01_wkf16_full.md, r01_pf32_full.md), keyed by config; None where no
 # capture of that config's kernel exists.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: 129117184 + 5640192, 3: 206465280 + 5998336, 4: 206465280 + 5998336,
-                                5: 506635264 + 7373568}
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: 129117696 + 4491776, 3: 206465280 + 5998336, 4: 206465280 + 5998336,
+                                5: 506622720 + 6679808}
 
 
 def _dist_env():
@@ -305,7 +305,7 @@ def run_ours(args):
         ach = fa * spots_per_launch / (kern_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                     "frac": ach / FP32_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(c.cfg) if L <= 0 and args.noise_flux <= 0 else None,
-                    "kernel": {B.ALGO_WK: f"wk_measure_kernel<{c.n}>", B.ALGO_PRUNED_FFT: f"pruned_fft_kernel<{c.P}>",
+                    "kernel": {B.ALGO_WK: f"wk_measure_kernel<{c.n}>", B.ALGO_WK_FFT: "wkf16_kernel", B.ALGO_PRUNED_FFT: f"pruned_fft_kernel<{c.P}>",
                                B.ALGO_LITERAL: f"literal_kernel<{c.P}>"}.get(sensors[0].algorithm, f"algo{sensors[0].algorithm}"),
                     "kernel_ms": kern_ms, "spots_per_launch": spots_per_launch,
                     "flops_per_spot": fa, "flops_basis": "F_alg (SURVEY.md 8(d))" if L <= 0 else
