@@ -305,7 +305,7 @@ def run_ours(args):
         ach = fa * spots_per_launch / (kern_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                     "frac": ach / FP32_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(c.cfg) if L <= 0 and args.noise_flux <= 0 else None,
-                    "kernel": {B.ALGO_WK: f"wk_measure_kernel<{c.n}>", B.ALGO_WK_FFT: "wkf16_kernel", B.ALGO_PRUNED_FFT: f"pruned_fft_kernel<{c.P}>",
+                    "kernel": {B.ALGO_WK: f"wk_measure_kernel<{c.n}>", B.ALGO_WK_FFT: f"wkf_kernel<{c.n}>", B.ALGO_PRUNED_FFT: f"pruned_fft_kernel<{c.P}>",
                                B.ALGO_LITERAL: f"literal_kernel<{c.P}>"}.get(sensors[0].algorithm, f"algo{sensors[0].algorithm}"),
                     "kernel_ms": kern_ms, "spots_per_launch": spots_per_launch,
                     "flops_per_spot": fa, "flops_basis": "F_alg (SURVEY.md 8(d))" if L <= 0 else

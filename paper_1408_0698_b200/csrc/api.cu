@@ -67,7 +67,7 @@ int pick_auto(const shwfs_handle *h)
     const bool wk = shwfs_wk_supported(h, 0), lit = shwfs_literal_supported(h);
     if (shwfs_pruned_fft_supported(h) && (h->n >= 16 || !wk)) return SHWFS_ALGO_PRUNED_FFT;
     if (!h->has_kernels && lit && (h->n >= 16 || !wk)) return SHWFS_ALGO_LITERAL;
-    if (wk && shwfs_wk_fft_supported(h)) return SHWFS_ALGO_WK_FFT;     /* n = 16: 80 line FFTs beat 33 k complex MACs */
+    if (shwfs_wk_fft_supported(h)) return SHWFS_ALGO_WK_FFT;           /* n >= 12: 80 line FFTs beat n^4 complex MACs */
     if (wk) return SHWFS_ALGO_WK;
     if (shwfs_wk_supported(h, 1)) return SHWFS_ALGO_WK_GENERIC;
     if (lit) return SHWFS_ALGO_LITERAL;
@@ -261,7 +261,7 @@ int shwfs_set_algorithm(shwfs_handle *h, int32_t algo)
         break;
     case SHWFS_ALGO_WK: if (!shwfs_wk_supported(h, 0)) return SHWFS_EUNSUPPORTED; break;
     case SHWFS_ALGO_WK_GENERIC: if (!shwfs_wk_supported(h, 1)) return SHWFS_EUNSUPPORTED; break;
-    case SHWFS_ALGO_WK_FFT: if (!shwfs_wk_supported(h, 0) || !shwfs_wk_fft_supported(h)) return SHWFS_EUNSUPPORTED; break;
+    case SHWFS_ALGO_WK_FFT: if (!shwfs_wk_fft_supported(h)) return SHWFS_EUNSUPPORTED; break;
     case SHWFS_ALGO_PRUNED_FFT: if (!shwfs_pruned_fft_supported(h)) return SHWFS_EUNSUPPORTED; break;
     default: return SHWFS_EINVAL;
     }
@@ -413,7 +413,7 @@ static int run_path(shwfs_handle *h, const float *phase_dev, int T, float *slope
     if (ext_on(h) || dm_patch) {
         /* sub-layers / noise / DM live in the lag-domain kernels only (shwfs_set_sodium made sure one exists) */
         if (stage == 0 || stage == 1) return SHWFS_EUNSUPPORTED;
-        const int generic = (h->algo == SHWFS_ALGO_WK_GENERIC) || !shwfs_wk_supported(h, 0);
+        const int generic = (h->algo == SHWFS_ALGO_WK_GENERIC) || !(shwfs_wk_supported(h, 0) || shwfs_wk_fft_supported(h));
         e = shwfs_wk_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr, stage == 3 ? img : nullptr,
                             t_base, dm_patch, generic, st);
     } else if (stage == 0 || stage == 1) {

@@ -628,8 +628,8 @@ cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *s
     if (A.total == 0) return cudaSuccess;
     h->launches += 1;
     if (h->algo != SHWFS_ALGO_WK && !generic && shwfs_wk_fft_supported(h) && A.L <= 1)   /* explicit WK: direct sums */
-        return shwfs_wk_fft_launch(A, st);
-    if (!generic) {
+        return shwfs_wk_fft_launch(A, h->n, st);
+    if (!generic && shwfs_wk_supported(h, 0)) {
         switch (h->n) {
         case 8: return launch_special<8>(A, st);
         case 10: return launch_special<10>(A, st);

@@ -1,5 +1,5 @@
 /*
- * wk_fft.cu -- the lag-domain (Wiener-Khinchin) form of the Shack-Hartmann hot path for n = 16, with the
+ * wk_fft.cu -- the lag-domain (Wiener-Khinchin) form of the Shack-Hartmann hot path for n = 12, 14, 16, with the
  * autocorrelation of the field computed by FFT instead of by direct sums, sm_100a.
  *
  * Same operation as wk.cu (H1..H8 of include/shwfs.h; "the spot computed by FFT for each sensor
@@ -9,7 +9,9 @@
  * profiles/r01_wk16_full_v4.md); on a Q x Q grid with Q = 2n = 32 >= 2n-1 the aperiodic autocorrelation is
  * the periodic one, G = DFT_Q(|DFT_Q(e)|^2) / Q^2, i.e. 80 line transforms of 32 points (~50 k instructions
  * with everything around them).  The grid size is independent of the sensor's padding P: the identity of
- * wk.cu's header holds for any P, and P enters only through the table M.
+ * wk.cu's header holds for any P, and P enters only through the table M.  n = 12 and 14, which have no
+ * direct-sum instance, run the same code with the rows, lag rows and table width of their size (threads
+ * r >= n idle in steps A, D, E).
  *
  * Thread mapping: a half-warp per spot, 8 spots per CTA, no CTA-wide barrier; one 16 x 32 complex tile of
  * shared memory per spot is reused by every exchange.
@@ -40,21 +42,21 @@ namespace {
 
 using namespace shwfs;
 
-constexpr int WF_N = 16;                       /* subaperture side                                   */
+constexpr int WF_ROWS = 16;                    /* tile rows (threads per spot): n <= 16              */
 constexpr int WF_Q = 32;                       /* transform grid side                                */
 constexpr int WF_THREADS = 128;
 constexpr int WF_SPOTS = WF_THREADS / 16;
 constexpr int WF_LD = 2 * WF_Q + 4;            /* floats per tile row; LD/4 odd => 16-byte row accesses conflict-free */
-constexpr int WF_TILE = WF_N * WF_LD;
+constexpr int WF_TILE = WF_ROWS * WF_LD;
 constexpr size_t WF_SMEM = sizeof(float) * (size_t)WF_SPOTS * WF_TILE;
-constexpr int WF_LX = 2 * WF_N - 1;
 
 __device__ __forceinline__ constexpr int xq(int k) { return fft_out_index<WF_Q>(k & (WF_Q - 1)); }
 
-template <int MODE, bool EXT>
-__global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
+template <int n, int MODE, bool EXT>
+__global__ void __launch_bounds__(WF_THREADS, 4) wkf_kernel(const WkArgs A)
 {
-    constexpr int n = WF_N, Q = WF_Q, LD = WF_LD;
+    static_assert(n % 2 == 0 && n <= WF_ROWS && 2 * n - 1 <= WF_Q, "even n <= 16: one thread per patch row, grid 32 >= 2n-1");
+    constexpr int Q = WF_Q, LD = WF_LD, LX = 2 * n - 1;
     extern __shared__ __align__(16) float wf_smem[];
     const int tid = threadIdx.x, sp = tid >> 4, r = tid & 15;
     float *tile = wf_smem + sp * WF_TILE;
@@ -66,25 +68,46 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
 
     float re[Q], im[Q];
 
-    /* ---- A: gather, field, row transform ---- */
-    {
-        float4 ph[n / 4], am[n / 4];
+    /* ---- A: gather, field, row transform (threads r < n) ---- */
+    if (r < n) {
+        float pv[n], av[n];
 #pragma unroll
-        for (int q = 0; q < n / 4; ++q) { ph[q] = make_float4(0.f, 0.f, 0.f, 0.f); am[q] = ph[q]; }
+        for (int k = 0; k < n; ++k) { pv[k] = 0.f; av[k] = 0.f; }
         if (live) {
             const int2 yx = __ldg(A.valid + i);
             const int off = (yx.x * n + r) * A.N + yx.y * n;
-            const float4 *pp = reinterpret_cast<const float4 *>(A.phase + (size_t)t * A.frame_stride + off);
-            const float4 *pa = reinterpret_cast<const float4 *>(A.amp + off);
-#pragma unroll
-            for (int q = 0; q < n / 4; ++q) { ph[q] = __ldg(pp + q); am[q] = __ldg(pa + q); }
-            if (EXT && A.dm_patch != nullptr) {
-                /* PAPER.md:76 "the residual phase (the open loop wavefront subtracted by the DM)" */
-                const float4 *pd = reinterpret_cast<const float4 *>(A.dm_patch + ((size_t)t * A.nsub + i) * (n * n) + r * n);
+            const float *pp = A.phase + (size_t)t * A.frame_stride + off;
+            const float *pa = A.amp + off;
+            /* PAPER.md:76 "the residual phase (the open loop wavefront subtracted by the DM)" */
+            const float *pd = EXT && A.dm_patch != nullptr ? A.dm_patch + ((size_t)t * A.nsub + i) * (n * n) + r * n : nullptr;
+            if constexpr (n % 4 == 0) {          /* rows start on 16 bytes */
 #pragma unroll
                 for (int q = 0; q < n / 4; ++q) {
-                    const float4 d = __ldg(pd + q);
-                    ph[q].x -= d.x; ph[q].y -= d.y; ph[q].z -= d.z; ph[q].w -= d.w;
+                    const float4 v = __ldg(reinterpret_cast<const float4 *>(pp) + q);
+                    const float4 w = __ldg(reinterpret_cast<const float4 *>(pa) + q);
+                    pv[4 * q] = v.x; pv[4 * q + 1] = v.y; pv[4 * q + 2] = v.z; pv[4 * q + 3] = v.w;
+                    av[4 * q] = w.x; av[4 * q + 1] = w.y; av[4 * q + 2] = w.z; av[4 * q + 3] = w.w;
+                }
+                if (EXT && pd != nullptr) {
+#pragma unroll
+                    for (int q = 0; q < n / 4; ++q) {
+                        const float4 d = __ldg(reinterpret_cast<const float4 *>(pd) + q);
+                        pv[4 * q] -= d.x; pv[4 * q + 1] -= d.y; pv[4 * q + 2] -= d.z; pv[4 * q + 3] -= d.w;
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int q = 0; q < n / 2; ++q) {
+                    const float2 v = __ldg(reinterpret_cast<const float2 *>(pp) + q);
+                    const float2 w = __ldg(reinterpret_cast<const float2 *>(pa) + q);
+                    pv[2 * q] = v.x; pv[2 * q + 1] = v.y; av[2 * q] = w.x; av[2 * q + 1] = w.y;
+                }
+                if (EXT && pd != nullptr) {
+#pragma unroll
+                    for (int q = 0; q < n / 2; ++q) {
+                        const float2 d = __ldg(reinterpret_cast<const float2 *>(pd) + q);
+                        pv[2 * q] -= d.x; pv[2 * q + 1] -= d.y;
+                    }
                 }
             }
         }
@@ -103,10 +126,6 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
             dj2 = dj * dj;
             sc *= A.sod_sw[0];
         }
-        const float pv[n] = {ph[0].x, ph[0].y, ph[0].z, ph[0].w, ph[1].x, ph[1].y, ph[1].z, ph[1].w,
-                             ph[2].x, ph[2].y, ph[2].z, ph[2].w, ph[3].x, ph[3].y, ph[3].z, ph[3].w};
-        const float av[n] = {am[0].x, am[0].y, am[0].z, am[0].w, am[1].x, am[1].y, am[1].z, am[1].w,
-                             am[2].x, am[2].y, am[2].z, am[2].w, am[3].x, am[3].y, am[3].z, am[3].w};
 #pragma unroll
         for (int k = 0; k < n; ++k) {
             float ramp = (float)(r + k) * A.ramp_unit;
@@ -166,8 +185,8 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
     }
     __syncwarp();
 
-    /* ---- D: lag row r: transform over u ---- */
-    {
+    /* ---- D: lag row r < n: transform over u ---- */
+    if (r < n) {
         const float4 *row = reinterpret_cast<const float4 *>(tile + r * LD);
 #pragma unroll
         for (int q = 0; q < Q / 2; ++q) {
@@ -175,14 +194,12 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
             re[2 * q] = f.x; im[2 * q] = f.y; re[2 * q + 1] = f.z; im[2 * q + 1] = f.w;
         }
         fft_fma<Q, -1>(re, im);
-    }
-    /* ---- E: table product, alias, x-transform; H[r][0..15] takes the place of the row this thread read ---- */
-    {
-        float2 acc[WF_LX];
+        /* ---- E: table product, alias, x-transform; H[r][0..15] takes the place of the row this thread read ---- */
+        float2 acc[LX];
 #pragma unroll
-        for (int a = 0; a < WF_LX; ++a) acc[a] = make_float2(re[xq(a - (n - 1))], im[xq(a - (n - 1))]);
+        for (int a = 0; a < LX; ++a) acc[a] = make_float2(re[xq(a - (n - 1))], im[xq(a - (n - 1))]);
         const float2 *Mi = A.M + (size_t)i * A.mstride;
-        finish_row<n>(acc, Mi + r * WF_LX, tile + r * LD);
+        finish_row<n>(acc, Mi + r * LX, tile + r * LD);
     }
     __syncwarp();
 
@@ -192,10 +209,12 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
         float yr[16], yi[16];
 #pragma unroll
         for (int m = 0; m < 16; ++m) {
-            const float2 v = *reinterpret_cast<const float2 *>(tile + m * LD + 2 * C);
-            yr[m] = v.x; yi[m] = v.y;
+            if (m < n) {
+                const float2 v = *reinterpret_cast<const float2 *>(tile + m * LD + 2 * C);
+                yr[m] = v.x; yi[m] = v.y;
+            } else { yr[m] = 0.f; yi[m] = 0.f; }
         }
-        fft_fma<16, +1>(yr, yi);                 /* B[R,C] = Re sum_m H[m][C] w_16^(R m) */
+        fft_fma<16, +1, n>(yr, yi);               /* B[R,C] = Re sum_m H[m][C] w_16^(R m) */
         float bcol[16];
 #pragma unroll
         for (int R = 0; R < 16; ++R) bcol[R] = yr[fft_out_index<16>(R)];
@@ -216,26 +235,37 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf16_kernel(const WkArgs A)
     }
 }
 
-template <int MODE, bool EXT>
-cudaError_t launch_wkf(const WkArgs &A, cudaStream_t st)
+template <int n, int MODE, bool EXT>
+cudaError_t launch_wkf_mode(const WkArgs &A, cudaStream_t st)
 {
     const int grid = (A.total + WF_SPOTS - 1) / WF_SPOTS;
-    wkf16_kernel<MODE, EXT><<<grid, WF_THREADS, WF_SMEM, st>>>(A);
+    wkf_kernel<n, MODE, EXT><<<grid, WF_THREADS, WF_SMEM, st>>>(A);
     return cudaGetLastError();
+}
+
+template <int n>
+cudaError_t launch_wkf(const WkArgs &A, cudaStream_t st)
+{
+    const bool ext = A.L > 0 || A.flux > 0.f || A.dm_patch != nullptr;
+    if (ext) return A.mode == 0 ? launch_wkf_mode<n, 0, true>(A, st) : launch_wkf_mode<n, 1, true>(A, st);
+    return A.mode == 0 ? launch_wkf_mode<n, 0, false>(A, st) : launch_wkf_mode<n, 1, false>(A, st);
 }
 
 }  // namespace
 
 int shwfs_wk_fft_supported(const shwfs_handle *h)
 {
-    return h->D == 16 && h->n == 16 && h->N % 4 == 0;
+    return h->D == 16 && (h->n == 12 || h->n == 14 || h->n == 16);
 }
 
-/* A.L <= 1 (several sub-layers: wk.cu's multi-layer instance) */
-cudaError_t shwfs_wk_fft_launch(const shwfs::WkArgs &A, cudaStream_t st)
+/* A.L <= 1 (several sub-layers: wk.cu's multi-layer or generic instance) */
+cudaError_t shwfs_wk_fft_launch(const shwfs::WkArgs &A, int n, cudaStream_t st)
 {
     static_assert(WF_SMEM <= 48 * 1024, "static limit of dynamic shared memory");
-    const bool ext = A.L > 0 || A.flux > 0.f || A.dm_patch != nullptr;
-    if (ext) return A.mode == 0 ? launch_wkf<0, true>(A, st) : launch_wkf<1, true>(A, st);
-    return A.mode == 0 ? launch_wkf<0, false>(A, st) : launch_wkf<1, false>(A, st);
+    switch (n) {
+    case 12: return launch_wkf<12>(A, st);
+    case 14: return launch_wkf<14>(A, st);
+    case 16: return launch_wkf<16>(A, st);
+    default: return cudaErrorInvalidValue;
+    }
 }

@@ -121,7 +121,8 @@ def test_config3_noise_matches_oracle(gpu, oracle):
         assert np.abs(off - clean).max() <= SLOPE_TOL
 
 
-@pytest.mark.parametrize("n,P,b", [(8, 16, 1), (10, 32, 2), (16, 64, 4), (16, 32, 2), (6, 16, 1), (12, 32, 2)])
+@pytest.mark.parametrize("n,P,b", [(8, 16, 1), (10, 32, 2), (16, 64, 4), (16, 32, 2), (6, 16, 1), (12, 32, 2),
+                                   (14, 32, 2)])
 def test_small_grids_sublayers_and_noise(gpu, oracle, n, P, b):
     """3x3 subapertures, partially lit mask with a dark subaperture, random kernels, 1..4 sub-layers with
     large random defocus / tilts (several wraps per patch), own or shared wavefronts, with and without

@@ -190,7 +190,7 @@ def test_residual_batches_on_the_tensor_cores(gpu, oracle, loop, cfg_id, M, T):
         assert np.abs(got[ts][:, sel] - want).max() <= SLOPE_TOL
 
 
-@pytest.mark.parametrize("n,P,b,T", [(5, 8, 1, 3), (12, 32, 2, 11), (6, 16, 1, 20)])
+@pytest.mark.parametrize("n,P,b,T", [(5, 8, 1, 3), (12, 32, 2, 11), (6, 16, 1, 20), (14, 32, 2, 9)])
 def test_residual_on_sizes_without_a_templated_gemm(gpu, oracle, loop, n, P, b, T):
     """Odd n (generic sensor kernel) and n*n outside {64, 100, 256}: the DM phase falls back to the
     one-thread-per-output kernel, for the loop step (T <= 8) and for batches alike."""

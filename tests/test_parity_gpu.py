@@ -160,7 +160,8 @@ def test_t_zero_is_a_noop(gpu):
 
 
 @pytest.mark.parametrize("n,P,b", [(8, 16, 1), (10, 32, 2), (16, 32, 2), (16, 64, 4), (8, 32, 2), (10, 16, 1),
-                                   (6, 16, 2), (12, 32, 1), (5, 8, 1)])
+                                   (6, 16, 2), (12, 32, 1), (5, 8, 1), (12, 32, 2), (14, 32, 2), (14, 64, 4),
+                                   (12, 16, 1)])
 def test_small_grids_all_sizes(gpu, oracle, n, P, b):
     """3x3 subapertures with a partially lit mask, explicit valid list (including a dark subaperture), random
     phases of several radians, with and without kernels, tau 0 and 0.1, both threshold modes."""
