@@ -58,8 +58,7 @@ extern "C" {
 #define SHWFS_ALGO_PRUNED_FFT 4  /* no elongation kernels, D = 16: one input-pruned P x P FFT per spot,   */
                                  /* half-warp per spot, bin + threshold + CoG in registers             */
 #define SHWFS_ALGO_WK_FFT   5    /* the lag-domain form with the field's autocorrelation taken by FFT on  */
-                                 /* a 32 x 32 grid instead of by direct sums (n = 12, 14, 16; D = 16);   */
-                                 /* several sodium sub-layers fall through to the direct-sum instances    */
+                                 /* a 32 x 32 grid instead of by direct sums (n = 12, 14, 16; D = 16)    */
 
 #define SHWFS_MAX_LAYERS 8        /* sodium sub-layers per LGS ("1 to 5 typically")            */
 

@@ -627,7 +627,7 @@ cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *s
     A.ramp_unit = 0.5f / (float)h->P;
     if (A.total == 0) return cudaSuccess;
     h->launches += 1;
-    if (h->algo != SHWFS_ALGO_WK && !generic && shwfs_wk_fft_supported(h) && A.L <= 1)   /* explicit WK: direct sums */
+    if (h->algo != SHWFS_ALGO_WK && !generic && shwfs_wk_fft_supported(h))   /* explicit WK: direct sums */
         return shwfs_wk_fft_launch(A, h->n, st);
     if (!generic && shwfs_wk_supported(h, 0)) {
         switch (h->n) {

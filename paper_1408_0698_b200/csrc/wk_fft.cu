@@ -30,8 +30,8 @@
  *      -> tile[ly][0..15]
  *   F  thread C owns detector column C: 16-point y-transform (real part), optional detector noise, H7 + H8
  *      (cog16) with half-warp shuffles; lane 0 writes the two slopes.
- * Extensions of the single-layer instance of wk.cu (detector noise, DM residual, one sodium sub-layer) are
- * carried; several sub-layers stay with wk.cu's multi-layer instance.
+ * The extensions of wk.cu are carried: detector noise, DM residual, sodium sub-layers (several: steps A-C per
+ * sub-layer, the separated transforms of S pile up in a second tile per spot, D-F once).
  */
 #include "wk_common.cuh"
 #include "field.cuh"
@@ -52,14 +52,19 @@ constexpr size_t WF_SMEM = sizeof(float) * (size_t)WF_SPOTS * WF_TILE;
 
 __device__ __forceinline__ constexpr int xq(int k) { return fft_out_index<WF_Q>(k & (WF_Q - 1)); }
 
-template <int n, int MODE, bool EXT>
-__global__ void __launch_bounds__(WF_THREADS, 4) wkf_kernel(const WkArgs A)
+/* EXTK as in wk.cu: 0 plain sensor, 1 extensions on one (sub-)layer, 2 several sodium sub-layers (S is linear in the
+ * sub-layer intensities: steps A-C run per sub-layer and the separated column transforms pile up in a second
+ * tile per spot, each element owned by one thread; D-F run once) */
+template <int n, int MODE, int EXTK>
+__global__ void __launch_bounds__(WF_THREADS, EXTK == 2 ? 3 : 4) wkf_kernel(const WkArgs A)
 {
+    constexpr bool EXT = EXTK > 0, ML = EXTK == 2;
     static_assert(n % 2 == 0 && n <= WF_ROWS && 2 * n - 1 <= WF_Q, "even n <= 16: one thread per patch row, grid 32 >= 2n-1");
     constexpr int Q = WF_Q, LD = WF_LD, LX = 2 * n - 1;
     extern __shared__ __align__(16) float wf_smem[];
     const int tid = threadIdx.x, sp = tid >> 4, r = tid & 15;
     float *tile = wf_smem + sp * WF_TILE;
+    float *gtile = ML ? wf_smem + (WF_SPOTS + sp) * WF_TILE : tile;      /* where step C leaves g_u[ly] */
 
     const int g = blockIdx.x * WF_SPOTS + sp;
     const bool live = g < A.total;
@@ -68,6 +73,9 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf_kernel(const WkArgs A)
 
     float re[Q], im[Q];
 
+    const int n_layers = ML ? A.L : 1;
+#pragma unroll 1
+    for (int layer = 0; layer < n_layers; ++layer) {
     /* ---- A: gather, field, row transform (threads r < n) ---- */
     if (r < n) {
         float pv[n], av[n];
@@ -76,7 +84,7 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf_kernel(const WkArgs A)
         if (live) {
             const int2 yx = __ldg(A.valid + i);
             const int off = (yx.x * n + r) * A.N + yx.y * n;
-            const float *pp = A.phase + (size_t)t * A.frame_stride + off;
+            const float *pp = A.phase + (size_t)t * A.frame_stride + (ML ? (size_t)layer * A.layer_stride : 0) + off;
             const float *pa = A.amp + off;
             /* PAPER.md:76 "the residual phase (the open loop wavefront subtracted by the DM)" */
             const float *pd = EXT && A.dm_patch != nullptr ? A.dm_patch + ((size_t)t * A.nsub + i) * (n * n) + r * n : nullptr;
@@ -118,13 +126,13 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf_kernel(const WkArgs A)
         const bool sodium = EXT && A.L > 0;
         if (sodium) {
             /* the sub-layer's analytic phase in turns (reading B1): g . d + q |d|^2, d from the patch centre */
-            const float2 gr = __ldg(A.sod_g + i);
+            const float2 gr = __ldg(A.sod_g + (size_t)layer * A.nsub + i);
             const float dj = (float)r - 0.5f * (float)(n - 1);
-            lq = A.sod_q[0];
+            lq = A.sod_q[layer];
             gx = gr.x;
             lin0 = fmaf(gr.y, dj, gr.x * (-0.5f * (float)(n - 1)));
             dj2 = dj * dj;
-            sc *= A.sod_sw[0];
+            sc *= A.sod_sw[layer];
         }
 #pragma unroll
         for (int k = 0; k < n; ++k) {
@@ -174,20 +182,27 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf_kernel(const WkArgs A)
     /* ---- C: both real columns in one complex transform over v, separated by symmetry ---- */
     fft_fma<Q, -1>(zr, zi);
     {
-        float2 *colp = reinterpret_cast<float2 *>(tile) + r;
+        float2 *colp = reinterpret_cast<float2 *>(gtile) + r;
 #pragma unroll
         for (int ly = 0; ly < n; ++ly) {
             const int a = xq(ly), b = xq(Q - ly);
             /* Z[ly] = g1[ly] + i g2[ly], conj Z[-ly] = g1[ly] - i g2[ly]  (the 1/2 is in the field's scale) */
-            colp[ly * (LD / 2)] = make_float2(zr[a] + zr[b], zi[a] - zi[b]);
-            colp[ly * (LD / 2) + 16] = make_float2(zi[a] + zi[b], zr[b] - zr[a]);
+            float2 g1 = make_float2(zr[a] + zr[b], zi[a] - zi[b]);
+            float2 g2 = make_float2(zi[a] + zi[b], zr[b] - zr[a]);
+            if (ML && layer > 0) {
+                const float2 p1 = colp[ly * (LD / 2)], p2 = colp[ly * (LD / 2) + 16];
+                g1.x += p1.x; g1.y += p1.y; g2.x += p2.x; g2.y += p2.y;
+            }
+            colp[ly * (LD / 2)] = g1;
+            colp[ly * (LD / 2) + 16] = g2;
         }
     }
+    }   /* sub-layers */
     __syncwarp();
 
     /* ---- D: lag row r < n: transform over u ---- */
     if (r < n) {
-        const float4 *row = reinterpret_cast<const float4 *>(tile + r * LD);
+        const float4 *row = reinterpret_cast<const float4 *>(gtile + r * LD);
 #pragma unroll
         for (int q = 0; q < Q / 2; ++q) {
             const float4 f = row[q];
@@ -235,20 +250,26 @@ __global__ void __launch_bounds__(WF_THREADS, 4) wkf_kernel(const WkArgs A)
     }
 }
 
-template <int n, int MODE, bool EXT>
+template <int n, int MODE, int EXTK>
 cudaError_t launch_wkf_mode(const WkArgs &A, cudaStream_t st)
 {
+    constexpr size_t smem = EXTK == 2 ? 2 * WF_SMEM : WF_SMEM;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(wkf_kernel<n, MODE, EXTK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
     const int grid = (A.total + WF_SPOTS - 1) / WF_SPOTS;
-    wkf_kernel<n, MODE, EXT><<<grid, WF_THREADS, WF_SMEM, st>>>(A);
+    wkf_kernel<n, MODE, EXTK><<<grid, WF_THREADS, smem, st>>>(A);
     return cudaGetLastError();
 }
 
 template <int n>
 cudaError_t launch_wkf(const WkArgs &A, cudaStream_t st)
 {
-    const bool ext = A.L > 0 || A.flux > 0.f || A.dm_patch != nullptr;
-    if (ext) return A.mode == 0 ? launch_wkf_mode<n, 0, true>(A, st) : launch_wkf_mode<n, 1, true>(A, st);
-    return A.mode == 0 ? launch_wkf_mode<n, 0, false>(A, st) : launch_wkf_mode<n, 1, false>(A, st);
+    if (A.L > 1) return A.mode == 0 ? launch_wkf_mode<n, 0, 2>(A, st) : launch_wkf_mode<n, 1, 2>(A, st);
+    if (A.L > 0 || A.flux > 0.f || A.dm_patch != nullptr)
+        return A.mode == 0 ? launch_wkf_mode<n, 0, 1>(A, st) : launch_wkf_mode<n, 1, 1>(A, st);
+    return A.mode == 0 ? launch_wkf_mode<n, 0, 0>(A, st) : launch_wkf_mode<n, 1, 0>(A, st);
 }
 
 }  // namespace
@@ -258,7 +279,6 @@ int shwfs_wk_fft_supported(const shwfs_handle *h)
     return h->D == 16 && (h->n == 12 || h->n == 14 || h->n == 16);
 }
 
-/* A.L <= 1 (several sub-layers: wk.cu's multi-layer or generic instance) */
 cudaError_t shwfs_wk_fft_launch(const shwfs::WkArgs &A, int n, cudaStream_t st)
 {
     static_assert(WF_SMEM <= 48 * 1024, "static limit of dynamic shared memory");
