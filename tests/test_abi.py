@@ -31,6 +31,19 @@ def test_library_exports_every_declared_symbol(libshwfs):
     assert b"invalid" in L.shwfs_strerror(-1)
 
 
+def test_binding_constants_match_the_header():
+    """Every #define of include/shwfs.h with an integer value (error codes, SHWFS_ALGO_*, SHWFS_MAX_LAYERS) has
+    the same value in the binding (ALGO_* drop the SHWFS_ prefix there)."""
+    from paper_1408_0698_b200 import binding
+    defs = dict(re.findall(r"^#define\s+(SHWFS_[A-Z_]+)\s+\(?(-?\d+)\)?", HEADER.read_text(), flags=re.M))
+    assert {"SHWFS_OK", "SHWFS_ECUDA", "SHWFS_ALGO_AUTO", "SHWFS_ALGO_WK_FFT", "SHWFS_MAX_LAYERS"} <= set(defs)
+    for name, value in defs.items():
+        py = name[len("SHWFS_"):] if name.startswith("SHWFS_ALGO_") else name
+        assert getattr(binding, py) == int(value), name
+    algos = sorted(int(v) for k, v in defs.items() if k.startswith("SHWFS_ALGO_"))
+    assert algos == list(range(len(algos)))                 # dense, no two algorithms share a number
+
+
 @pytest.mark.parametrize("cname,pyname", [("shwfs_geometry", "ShwfsGeometry"), ("shwfs_sodium", "ShwfsSodium"),
                                           ("shwfs_noise", "ShwfsNoise"), ("pyrwfs_config", "PyrwfsConfig")])
 def test_ctypes_struct_matches_the_header(tmp_path, cname, pyname):
