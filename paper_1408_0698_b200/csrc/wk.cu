@@ -311,12 +311,15 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkSmem<n, (EXTK < 2)>::MIN_
                             am = __ldg(reinterpret_cast<const float2 *>(A.amp + acur));
                         }
                         float2 e0, e1;
-                        if (EXT) {
-                            /* ONE pair of field evaluations whatever the run-time flags: with two calls under
-                             * if (sodium) / else the compiler evaluates both and selects (twice the sincos).
-                             * Without sodium lq = 0, lsw = 1, g = 0: the arguments are the plain ones exactly. */
-                            float2 g = make_float2(0.f, 0.f);
-                            if (sodium) g = __ldg(A.sod_g + (size_t)layer * A.nsub + s_info[s].z);
+                        if (EXTK == 2) {
+                            /* several sub-layers: sodium is on by construction.  (Written as if (sodium) .. else ..
+                             * this compiled to BOTH field evaluations per pixel: twice the sincos.) */
+                            const float2 g = __ldg(A.sod_g + (size_t)layer * A.nsub + s_info[s].z);
+                            const float lin = fmaf(g.x, dk0, g.y * dj);
+                            e0 = field_value(ph[r].x, am.x * lsw, A.turns, ramp0 - (lin + quad0));
+                            e1 = field_value(ph[r].y, am.y * lsw, A.turns, ramp1 - (lin + g.x + quad1));
+                        } else if (sodium) {
+                            const float2 g = __ldg(A.sod_g + (size_t)layer * A.nsub + s_info[s].z);
                             const float lin = fmaf(g.x, dk0, g.y * dj);
                             e0 = field_value(ph[r].x, am.x * lsw, A.turns, ramp0 - (lin + quad0));
                             e1 = field_value(ph[r].y, am.y * lsw, A.turns, ramp1 - (lin + g.x + quad1));
