@@ -254,9 +254,13 @@ template <int n, int MODE, int EXTK>
 cudaError_t launch_wkf_mode(const WkArgs &A, cudaStream_t st)
 {
     constexpr size_t smem = EXTK == 2 ? 2 * WF_SMEM : WF_SMEM;
-    if (smem > 48 * 1024) {
+    static bool attr_set[64] = {false};             /* per device, as in wk.cu */
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (smem > 48 * 1024 && dev >= 0 && dev < 64 && !attr_set[dev]) {
         cudaError_t e = cudaFuncSetAttribute(wkf_kernel<n, MODE, EXTK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
+        attr_set[dev] = true;
     }
     const int grid = (A.total + WF_SPOTS - 1) / WF_SPOTS;
     wkf_kernel<n, MODE, EXTK><<<grid, WF_THREADS, smem, st>>>(A);
