@@ -51,6 +51,8 @@ extern "C" {
 
 /* Algorithms.  Both give the H1..H8 result to fp32 rounding. */
 #define SHWFS_ALGO_AUTO     0    /* the fastest instance for the handle's sizes (default)              */
+                                 /* (for n = 8, 10 also per call: calls of under ~64 spots per SM, i.e.  */
+                                 /* the one-frame closed-loop step, take the SHWFS_ALGO_WK_FFT instance) */
 #define SHWFS_ALGO_LITERAL  1    /* P x P shared-memory FFT chain, exactly the H3..H6 order             */
 #define SHWFS_ALGO_WK       2    /* Wiener-Khinchin lag-domain form: autocorrelation of the field, x   */
                                  /* precomputed (kernel MTF x bin x centre) table, D x D real transform */

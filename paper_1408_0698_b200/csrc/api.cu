@@ -193,6 +193,8 @@ int shwfs_create(const shwfs_geometry *g, float lambda_m, int32_t pad, int32_t b
     CU_TRY(cudaGetDevice(&h->device), "cudaGetDevice");
     if (!shwfs_wk_supported(h, 0) && !shwfs_wk_supported(h, 1) && !shwfs_literal_supported(h) && !shwfs_pruned_fft_supported(h)) { rc = SHWFS_EUNSUPPORTED; goto fail; }
     h->algo = pick_auto(h);
+    h->algo_explicit = 0;
+    h->call_T = 0;
     if (h->algo < 0) { rc = SHWFS_EUNSUPPORTED; goto fail; }
 
     CU_TRY(cudaMalloc(&h->d_amp, sizeof(float) * (size_t)N * N), "cudaMalloc(amplitude)");
@@ -266,6 +268,7 @@ int shwfs_set_algorithm(shwfs_handle *h, int32_t algo)
     default: return SHWFS_EINVAL;
     }
     h->algo = a;
+    h->algo_explicit = algo != SHWFS_ALGO_AUTO;
     return SHWFS_OK;
 }
 
@@ -606,6 +609,7 @@ static int measure_host_impl(shwfs_handle *h, const float *phase_host, int32_t T
             for (int k = 0; k < 2; ++k)
                 if (!h->h_pin[k]) CU_TRY(cudaHostAlloc(&h->h_pin[k], sizeof(float) * (size_t)h->N * h->N * h->chunk_frames, cudaHostAllocDefault), "cudaHostAlloc");
         int c = 0;
+        h->call_T = T;                          /* the chunks are parts of one call: same kernel instance for all */
         for (int t0 = 0; t0 < T; t0 += chunk_steps, ++c) {
             const int k = c & 1;
             const int tc = (T - t0 < chunk_steps) ? T - t0 : chunk_steps;
@@ -637,13 +641,15 @@ static int measure_host_impl(shwfs_handle *h, const float *phase_host, int32_t T
             CU_TRY(cudaEventRecord(h->ev_h2d[k], h->st_copy), "cudaEventRecord");
             CU_TRY(cudaStreamWaitEvent(h->st_comp, h->ev_h2d[k], 0), "cudaStreamWaitEvent");
             rc = run_path(h, h->d_phase[k], tc, h->d_slopes + 2 * (size_t)t0 * h->nsub, -1, nullptr, (unsigned)t0, h->st_comp);
-            if (rc) goto fail;
+            if (rc) { h->call_T = 0; goto fail; }
             CU_TRY(cudaEventRecord(h->ev_done[k], h->st_comp), "cudaEventRecord");
         }
+        h->call_T = 0;
         CU_TRY(cudaMemcpyAsync(slopes_host, h->d_slopes, sizeof(float) * n_slopes, cudaMemcpyDeviceToHost, h->st_comp), "cudaMemcpyAsync(D2H)");
         if (wait) CU_TRY(cudaStreamSynchronize(h->st_comp), "cudaStreamSynchronize");
     }
 fail:
+    h->call_T = 0;
     if (rc && h->st_comp) { cudaStreamSynchronize(h->st_comp); cudaStreamSynchronize(h->st_copy); }
     if (prev >= 0 && prev != h->device) cudaSetDevice(prev);
     return rc;

@@ -22,6 +22,8 @@ struct shwfs_handle {
     int device;
     int has_kernels;
     int algo;              /* resolved SHWFS_ALGO_* used by shwfs_measure */
+    int algo_explicit;     /* 1: chosen by shwfs_set_algorithm (non-AUTO): no per-call choice between instances */
+    int call_T;            /* > 0 while the host pipeline feeds one call in chunks: the size the per-call choice sees */
     int64_t launches;
 
     /* device tables (owned) */

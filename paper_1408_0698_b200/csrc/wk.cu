@@ -634,6 +634,15 @@ cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *s
     A.ramp_unit = 0.5f / (float)h->P;
     if (A.total == 0) return cudaSuccess;
     h->launches += 1;
+    /* n = 8, 10 under SHWFS_ALGO_AUTO: direct sums win on batches (1.0e9 against 0.7e9 spots/s at config 4), but a call of
+     * one or two frames (the closed-loop step) is less than a wave of their 32-spot CTAs and runs at the latency of one
+     * CTA; the half-warp-per-spot FFT instance spreads it over four times as many CTAs without CTA barriers */
+    if (!generic && !h->algo_explicit && h->algo == SHWFS_ALGO_WK && h->D == 16 && (h->n == 8 || h->n == 10)) {
+        static int sms = 0;
+        if (sms == 0) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+        const long long call_spots = (long long)(h->call_T > 0 ? h->call_T : T) * h->nsub;
+        if (call_spots <= 64LL * sms) return shwfs_wk_fft_launch(A, h->n, st);
+    }
     if (h->algo != SHWFS_ALGO_WK && !generic && shwfs_wk_fft_supported(h))   /* explicit WK: direct sums */
         return shwfs_wk_fft_launch(A, h->n, st);
     if (!generic && shwfs_wk_supported(h, 0)) {

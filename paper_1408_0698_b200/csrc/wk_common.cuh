@@ -78,7 +78,7 @@ __device__ __forceinline__ void finish_row(const float2 (&acc)[2 * n - 1], const
 
 }  // namespace shwfs
 
-/* wk_fft.cu: n = 12, 14, 16, D = 16 */
+/* wk_fft.cu: even n = 8 .. 16, D = 16 */
 cudaError_t shwfs_wk_fft_launch(const shwfs::WkArgs &A, int n, cudaStream_t st);
 
 #endif

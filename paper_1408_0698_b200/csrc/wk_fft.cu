@@ -11,7 +11,8 @@
  * with everything around them).  The grid size is independent of the sensor's padding P: the identity of
  * wk.cu's header holds for any P, and P enters only through the table M.  n = 12 and 14, which have no
  * direct-sum instance, run the same code with the rows, lag rows and table width of their size (threads
- * r >= n idle in steps A, D, E).
+ * r >= n idle in steps A, D, E).  n = 8 and 10 are instantiated too: under SHWFS_ALGO_AUTO calls of one or two frames
+ * (the closed-loop step, less than a wave of wk.cu's 32-spot CTAs) come here; on batches the direct sums win.
  *
  * Thread mapping: a half-warp per spot, 8 spots per CTA, no CTA-wide barrier; one 16 x 32 complex tile of
  * shared memory per spot is reused by every exchange.
@@ -287,6 +288,8 @@ cudaError_t shwfs_wk_fft_launch(const shwfs::WkArgs &A, int n, cudaStream_t st)
 {
     static_assert(WF_SMEM <= 48 * 1024, "static limit of dynamic shared memory");
     switch (n) {
+    case 8: return launch_wkf<8>(A, st);
+    case 10: return launch_wkf<10>(A, st);
     case 12: return launch_wkf<12>(A, st);
     case 14: return launch_wkf<14>(A, st);
     case 16: return launch_wkf<16>(A, st);
