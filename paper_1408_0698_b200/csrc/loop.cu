@@ -232,9 +232,9 @@ __global__ void __launch_bounds__(256) dm_phase_gemv_kernel(const float *__restr
 /* coef[t][m] += gain * sum_k R[m][k] * s[t][k].  One CTA per mode m, its 256 threads split the row of R
  * (8-byte loads, frames in register tiles of RC_TT so that the row is read once per tile), warp-shuffle then
  * shared-memory reduction.  hist (optional): hist[t][m] = coef[t][m] BEFORE the update (reading C4).     */
-constexpr int RC_THREADS = 256;
 constexpr int RC_TT = 8;
 
+template <int RC_THREADS>
 __global__ void __launch_bounds__(RC_THREADS) recon_kernel(const float *__restrict__ R, const float *__restrict__ s,
                                                            int T, int K, int M, float gain,
                                                            float *__restrict__ coef, int ldc, float *__restrict__ hist)
@@ -315,6 +315,9 @@ cudaError_t shwfs_loop_dm_phase(shwfs_handle *h, const float *coef, int ldc, int
 cudaError_t shwfs_loop_reconstruct(const float *R, const float *slopes, int T, int K, int M, float gain,
                                    float *coef, int ldc, float *hist, cudaStream_t st)
 {
-    recon_kernel<<<M, RC_THREADS, 0, st>>>(R, slopes, T, K, M, gain, coef, ldc, hist);
+    /* the loop step (a frame or two): 1024 threads put the whole row of R in flight at once -- the kernel is one
+     * L2 round trip deep instead of five; batches reuse each row element over 8 frames and are fine with 256 */
+    if (T <= 2) recon_kernel<1024><<<M, 1024, 0, st>>>(R, slopes, T, K, M, gain, coef, ldc, hist);
+    else recon_kernel<256><<<M, 256, 0, st>>>(R, slopes, T, K, M, gain, coef, ldc, hist);
     return cudaGetLastError();
 }
