@@ -200,10 +200,12 @@ __global__ void __launch_bounds__(PY_LINES * R, 2) pyr_cols_kernel(const PyArgs 
     for (int q = 0; q < R; ++q) stage[(j + R * q) * (PY_LINES + 1) + b] = make_float2(re[q], im[q]);
     __syncthreads();
     float2 *dst = A.A2 + (size_t)tk * 2 * A.N * L;
-    for (int e = tid; e < L * PY_LINES; e += PY_LINES * R) {
-        const int yy = e / PY_LINES, bb = e - yy * PY_LINES;
-        const int r = kept_index(yy, A.N, L, A.s);
-        if (r >= 0) dst[(size_t)r * L + u0 + bb] = stage[yy * (PY_LINES + 1) + bb];
+    /* only the 2N kept rows are written: row r < N is pupil-plane row r + s, row N + d is row (d - s) mod Np
+     * (the inverse of kept_index; the two ranges are disjoint by the create-time checks on s) */
+    for (int e = tid; e < 2 * A.N * PY_LINES; e += PY_LINES * R) {
+        const int r = e / PY_LINES, bb = e - r * PY_LINES;
+        const int yy = r < A.N ? r + A.s : (r - A.N - A.s) & (L - 1);
+        dst[(size_t)r * L + u0 + bb] = stage[yy * (PY_LINES + 1) + bb];
     }
 }
 
