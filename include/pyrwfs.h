@@ -2,7 +2,8 @@
  * pyrwfs.h -- C ABI of the B200-native pyramid wavefront sensor, exported by the same
  * library as include/shwfs.h (libshwfs.so) with the same conventions: every function returns 0 or a negative
  * SHWFS_E* code (shwfs_strerror / shwfs_last_cuda_error apply), nothing throws or exits, "HOST"/"DEVICE" say
- * where a pointer lives, pyrwfs_measure only enqueues work on the caller's stream.
+ * where a pointer lives, pyrwfs_measure only enqueues work on the caller's stream (and, like shwfs_measure,
+ * must be called with the handle's device current: SHWFS_EINVAL otherwise).
  *
  * The operation is the pyramid sensor module of PAPER.md:92 (section 4): "We follow the scheme presented in
  * (Verinaud 2004) [...] This module makes a large use of the GPU computing power for the whole computation

@@ -29,9 +29,13 @@
  *     output arguments are untouched on failure.
  *   - "HOST" pointers are ordinary host memory, "DEVICE" pointers are CUDA device memory of the
  *     device that was current at shwfs_create.  shwfs_create copies every HOST array it is given.
- *   - shwfs_measure / shwfs_debug_spots only enqueue work on `cuda_stream` (a cudaStream_t passed
- *     as void*, NULL = default stream): no allocation, no synchronisation, no host<->device copy.
- *     Results are valid once the caller has synchronised that stream.
+ *   - shwfs_measure only enqueues work on `cuda_stream` (a cudaStream_t passed as void*, NULL = default
+ *     stream): no allocation, no synchronisation, no host<->device copy.  Results are valid once the
+ *     caller has synchronised that stream.  (shwfs_debug_spots, a test hook, may allocate its scratch and
+ *     synchronise the stream the first time it is called, see there.)
+ *   - The enqueue-only calls (shwfs_measure, _measure_residual, _reconstruct, _closed_loop, _debug_spots)
+ *     must be made with the handle's device current (the one that was current at shwfs_create) and return
+ *     SHWFS_EINVAL otherwise; the other calls switch to it and back themselves.
  *   - A handle is not thread-safe; distinct handles are independent (one handle = one WFS).
  */
 #ifndef SHWFS_H_
@@ -211,7 +215,10 @@ int shwfs_closed_loop(shwfs_handle *h, const float *phase_dev, const float *R_de
                       int32_t T, float *slopes_dev, float *coef_hist_dev, void *cuda_stream);
 
 /* ---- debug (parity on images; not on the timed path) ------------------------------------------- */
-/* stage 0: centred intensity  roll(I)  DEVICE out [T*nsub*P*P]
+/* Enqueues on cuda_stream like shwfs_measure, except that the first call (and a later call with a larger T,
+ * and the first call of stage 0 or 1 on a handle with elongation kernels, which builds the literal chain's
+ * transformed kernels) allocates handle-owned scratch and synchronises the stream once.
+ * stage 0: centred intensity  roll(I)  DEVICE out [T*nsub*P*P]
  * stage 1: centred image after elongation  Sh  [T*nsub*P*P]  (== stage 0 without kernels)
  * stage 2: binned image B  [T*nsub*D*D], D = P/b -- produced by the handle's CURRENT algorithm, so it
  *          is the image the timed path thresholds; stages 0 and 1 exist only in the literal chain
@@ -221,7 +228,7 @@ int shwfs_debug_spots(shwfs_handle *h, const float *phase_dev, int32_t T, int32_
                       float *out_dev, void *cuda_stream);
 
 const char *shwfs_strerror(int code);
-/* Text of the last CUDA error seen by this process's calls into the library ("" if none). */
+/* Text of the last CUDA error seen by the calling thread's calls into the library ("" if none). */
 const char *shwfs_last_cuda_error(void);
 int shwfs_version(void);
 

@@ -10,6 +10,7 @@
 #include <new>
 
 #include "internal.h"
+#include "tma.cuh"
 
 namespace {
 
@@ -35,6 +36,7 @@ void free_handle(shwfs_handle *h)
     if (prev != h->device) cudaSetDevice(h->device);
     cudaFree(h->d_amp);
     cudaFree(h->d_valid);
+    cudaFree(h->d_patch);
     cudaFree(h->d_kernels);
     cudaFree(h->d_wk_table);
     cudaFree(h->d_khat);
@@ -50,7 +52,6 @@ void free_handle(shwfs_handle *h)
         if (h->ev_done[k]) cudaEventDestroy(h->ev_done[k]);
     }
     cudaFree(h->d_slopes);
-    if (h->h_slopes_pin) cudaFreeHost(h->h_slopes_pin);
     if (h->st_copy) cudaStreamDestroy(h->st_copy);
     if (h->st_comp) cudaStreamDestroy(h->st_comp);
     free(h->h_valid);
@@ -90,6 +91,36 @@ int ensure_khat(shwfs_handle *h)
 }
 
 }  // namespace
+
+/* tma.cuh: the driver's encoder is fetched through the runtime, so the library links against cudart only */
+bool shwfs_tma_patch_map(CUtensorMap *out, const float *base, int N, long long frames, int n)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    static bool looked = false;
+    if (!looked) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            encode = (encode_fn)fn;
+        else
+            cudaGetLastError();
+        looked = true;
+    }
+    if (!encode || !base || frames <= 0 || N <= 0 || (N & 3) || (n & 3) || n > 256) return false;
+    if (reinterpret_cast<uintptr_t>(base) & 15) return false;
+    const cuuint64_t dim[3] = {(cuuint64_t)N, (cuuint64_t)N, (cuuint64_t)frames};
+    const cuuint64_t stride[2] = {(cuuint64_t)N * 4, (cuuint64_t)N * (cuuint64_t)N * 4};
+    const cuuint32_t box[3] = {(cuuint32_t)n, (cuuint32_t)n, 1};
+    const cuuint32_t one[3] = {1, 1, 1};
+    const CUtensorMapSwizzle sw = n == 16 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE;
+    return encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float *>(base), dim, stride, box, one,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 
 void shwfs_note_cuda_error(cudaError_t e, const char *where)
 {
@@ -191,16 +222,33 @@ int shwfs_create(const shwfs_geometry *g, float lambda_m, int32_t pad, int32_t b
 
     int rc = SHWFS_OK;
     CU_TRY(cudaGetDevice(&h->device), "cudaGetDevice");
+    CU_TRY(cudaDeviceGetAttribute(&h->sms, cudaDevAttrMultiProcessorCount, h->device), "cudaDeviceGetAttribute");
+    h->no_tma = getenv("SHWFS_NO_TMA") != nullptr;
     if (!shwfs_wk_supported(h, 0) && !shwfs_wk_supported(h, 1) && !shwfs_literal_supported(h) && !shwfs_pruned_fft_supported(h)) { rc = SHWFS_EUNSUPPORTED; goto fail; }
     h->algo = pick_auto(h);
     h->algo_explicit = 0;
-    h->call_T = 0;
     if (h->algo < 0) { rc = SHWFS_EUNSUPPORTED; goto fail; }
 
     CU_TRY(cudaMalloc(&h->d_amp, sizeof(float) * (size_t)N * N), "cudaMalloc(amplitude)");
     CU_TRY(cudaMemcpy(h->d_amp, g->amplitude, sizeof(float) * (size_t)N * N, cudaMemcpyHostToDevice), "cudaMemcpy(amplitude)");
     CU_TRY(cudaMalloc(&h->d_valid, sizeof(int2) * (size_t)nsub), "cudaMalloc(valid)");
     CU_TRY(cudaMemcpy(h->d_valid, valid, sizeof(int2) * (size_t)nsub, cudaMemcpyHostToDevice), "cudaMemcpy(valid)");
+    {   /* patch table: origin of each valid subaperture in pixels, flagged when its amplitudes are all exactly 1 */
+        int2 *patch = (int2 *)malloc(sizeof(int2) * (size_t)nsub);
+        if (!patch) { rc = SHWFS_ENOMEM; goto fail; }
+        for (int i = 0; i < nsub; ++i) {
+            const int y0 = valid[2 * i] * n, x0 = valid[2 * i + 1] * n;
+            bool lit = true;
+            for (int j = 0; j < n && lit; ++j)
+                for (int k = 0; k < n; ++k)
+                    if (g->amplitude[(size_t)(y0 + j) * N + x0 + k] != 1.0f) { lit = false; break; }
+            patch[i] = make_int2(x0 | (lit ? SHWFS_PATCH_LIT : 0), y0);
+        }
+        cudaError_t e1 = cudaMalloc(&h->d_patch, sizeof(int2) * (size_t)nsub);
+        if (e1 == cudaSuccess) e1 = cudaMemcpy(h->d_patch, patch, sizeof(int2) * (size_t)nsub, cudaMemcpyHostToDevice);
+        free(patch);
+        CU_TRY(e1, "patch table");
+    }
     if (h->has_kernels) {
         const size_t kb = sizeof(float) * (size_t)nsub * P * P;
         CU_TRY(cudaMalloc(&h->d_kernels, kb), "cudaMalloc(kernels)");
@@ -380,6 +428,7 @@ int shwfs_set_dm(shwfs_handle *h, const float *modes_dev, int32_t M)
         CU_TRY(cudaMalloc(&h->d_dm_patch, sizeof(float) * h->dm_patch_cap), "cudaMalloc(dm patch)");
         CU_TRY(shwfs_loop_relayout_modes(h, modes_dev, M, 0), "relayout_modes");
         h->dm_M = M;
+        h->dm_fp32 = getenv("SHWFS_DM_FP32") != nullptr;   /* A/B runs: keep the FP32 SIMT GEMM for batches too */
         if (shwfs_umma_np(h) > 0) {
             /* tensor-core operand tiles (hi|lo split, canonical layout); best effort: without them the FP32
              * SIMT GEMM of loop.cu serves every batch size */
@@ -402,12 +451,20 @@ done:
     return rc;
 }
 
+/* the enqueue-only entry points launch on the current device: it has to be the handle's */
+static bool on_device(const shwfs_handle *h)
+{
+    int dev = -1;
+    return cudaGetDevice(&dev) == cudaSuccess && dev == h->device;
+}
+
 static bool ext_on(const shwfs_handle *h) { return h->sod_L > 0 || h->nz_flux > 0.f; }
 
 /* frames of phase per time step t: L when every sub-layer has its own wavefront */
 static int frames_per_step(const shwfs_handle *h) { return (h->sod_L > 0 && !h->sod_shared) ? h->sod_L : 1; }
 
-static int run_path(shwfs_handle *h, const float *phase_dev, int T, float *slopes_dev, int stage, float *img,
+/* call_T: frames of the whole API call (== T unless the host pipeline feeds it in chunks), see shwfs_wk_launch */
+static int run_path(shwfs_handle *h, const float *phase_dev, int T, int call_T, float *slopes_dev, int stage, float *img,
                     unsigned t_base, cudaStream_t st, const float *dm_patch = nullptr)
 {
     if ((long long)T * h->nsub > 0x7fffffffLL / 2) return SHWFS_EINVAL;
@@ -417,7 +474,7 @@ static int run_path(shwfs_handle *h, const float *phase_dev, int T, float *slope
         /* sub-layers / noise / DM live in the lag-domain kernels only (shwfs_set_sodium made sure one exists) */
         if (stage == 0 || stage == 1) return SHWFS_EUNSUPPORTED;
         const int generic = (h->algo == SHWFS_ALGO_WK_GENERIC) || !(shwfs_wk_supported(h, 0) || shwfs_wk_fft_supported(h));
-        e = shwfs_wk_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr, stage == 3 ? img : nullptr,
+        e = shwfs_wk_launch(h, phase_dev, T, call_T, slopes_dev, stage == 2 ? img : nullptr, stage == 3 ? img : nullptr,
                             t_base, dm_patch, generic, st);
     } else if (stage == 0 || stage == 1) {
         int rc = ensure_khat(h);
@@ -430,12 +487,8 @@ static int run_path(shwfs_handle *h, const float *phase_dev, int T, float *slope
         e = shwfs_pruned_fft_launch(h, phase_dev, T, slopes_dev, (stage == 2 || stage == 3) ? img : nullptr, st);
     } else {
         if (stage == 3) stage = 2;
-        if (h->algo == SHWFS_ALGO_PRUNED_FFT) {
-            e = shwfs_pruned_fft_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr, st);
-        } else {
-            e = shwfs_wk_launch(h, phase_dev, T, slopes_dev, stage == 2 ? img : nullptr, nullptr, t_base, nullptr,
-                                h->algo == SHWFS_ALGO_WK_GENERIC, st);
-        }
+        e = shwfs_wk_launch(h, phase_dev, T, call_T, slopes_dev, stage == 2 ? img : nullptr, nullptr, t_base, nullptr,
+                            h->algo == SHWFS_ALGO_WK_GENERIC, st);
     }
     if (e != cudaSuccess) { shwfs_note_cuda_error(e, "kernel launch"); return SHWFS_ECUDA; }
     return SHWFS_OK;
@@ -445,8 +498,8 @@ int shwfs_measure(shwfs_handle *h, const float *phase_dev, int32_t T, float *slo
 {
     if (!h || T < 0) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
-    if (!phase_dev || !slopes_dev) return SHWFS_EINVAL;
-    return run_path(h, phase_dev, T, slopes_dev, -1, nullptr, 0u, (cudaStream_t)cuda_stream);
+    if (!phase_dev || !slopes_dev || !on_device(h)) return SHWFS_EINVAL;
+    return run_path(h, phase_dev, T, T, slopes_dev, -1, nullptr, 0u, (cudaStream_t)cuda_stream);
 }
 
 int shwfs_measure_residual(shwfs_handle *h, const float *phase_dev, const float *coef_dev, int32_t T,
@@ -454,7 +507,7 @@ int shwfs_measure_residual(shwfs_handle *h, const float *phase_dev, const float 
 {
     if (!h || T < 0 || h->dm_M <= 0) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
-    if (!phase_dev || !coef_dev || !slopes_dev) return SHWFS_EINVAL;
+    if (!phase_dev || !coef_dev || !slopes_dev || !on_device(h)) return SHWFS_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t need = (size_t)T * h->nsub * h->n * h->n;
     if (h->dm_patch_cap < need) {
@@ -476,8 +529,8 @@ int shwfs_measure_residual(shwfs_handle *h, const float *phase_dev, const float 
     }
     cudaError_t e = shwfs_loop_dm_phase(h, coef_dev, h->dm_M, T, h->d_dm_patch, st);
     if (e != cudaSuccess) { shwfs_note_cuda_error(e, "dm_phase"); return SHWFS_ECUDA; }
-    h->launches += (h->d_um_modes && T > 8 && h->d_um_coef) ? 2 : 1;
-    return run_path(h, phase_dev, T, slopes_dev, -1, nullptr, 0u, st, h->d_dm_patch);
+    h->launches += (h->d_um_modes && T > 8 && h->d_um_coef && !h->dm_fp32) ? 2 : 1;
+    return run_path(h, phase_dev, T, T, slopes_dev, -1, nullptr, 0u, st, h->d_dm_patch);
 }
 
 int shwfs_reconstruct(shwfs_handle *h, const float *R_dev, const float *slopes_dev, int32_t T, float gain,
@@ -485,7 +538,7 @@ int shwfs_reconstruct(shwfs_handle *h, const float *R_dev, const float *slopes_d
 {
     if (!h || T < 0 || h->dm_M <= 0 || !isfinite(gain)) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
-    if (!R_dev || !slopes_dev || !coef_dev) return SHWFS_EINVAL;
+    if (!R_dev || !slopes_dev || !coef_dev || !on_device(h)) return SHWFS_EINVAL;
     cudaError_t e = shwfs_loop_reconstruct(R_dev, slopes_dev, T, 2 * h->nsub, h->dm_M, gain, coef_dev, h->dm_M,
                                            nullptr, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) { shwfs_note_cuda_error(e, "reconstruct"); return SHWFS_ECUDA; }
@@ -498,7 +551,7 @@ int shwfs_closed_loop(shwfs_handle *h, const float *phase_dev, const float *R_de
 {
     if (!h || T < 0 || h->dm_M <= 0 || !isfinite(gain)) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
-    if (!phase_dev || !R_dev || !coef_dev || !slopes_dev) return SHWFS_EINVAL;
+    if (!phase_dev || !R_dev || !coef_dev || !slopes_dev || !on_device(h)) return SHWFS_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t step = (size_t)h->N * h->N * frames_per_step(h);
     const int K = 2 * h->nsub;
@@ -508,7 +561,7 @@ int shwfs_closed_loop(shwfs_handle *h, const float *phase_dev, const float *R_de
         e = shwfs_loop_dm_phase(h, coef_dev, h->dm_M, 1, h->d_dm_patch, st);
         if (e != cudaSuccess) break;
         h->launches += 1;
-        int rc = run_path(h, phase_dev + (size_t)t * step, 1, slopes_dev + (size_t)t * K, -1, nullptr, (unsigned)t,
+        int rc = run_path(h, phase_dev + (size_t)t * step, 1, 1, slopes_dev + (size_t)t * K, -1, nullptr, (unsigned)t,
                           st, h->d_dm_patch);
         if (rc) return rc;
         e = shwfs_loop_reconstruct(R_dev, slopes_dev + (size_t)t * K, 1, K, h->dm_M, gain, coef_dev, h->dm_M,
@@ -524,7 +577,7 @@ int shwfs_debug_spots(shwfs_handle *h, const float *phase_dev, int32_t T, int32_
 {
     if (!h || T < 0 || stage < 0 || stage > 3) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
-    if (!phase_dev || !out_dev) return SHWFS_EINVAL;
+    if (!phase_dev || !out_dev || !on_device(h)) return SHWFS_EINVAL;
     /* the debug path needs somewhere to put the slopes it also computes */
     const size_t need = 2 * (size_t)T * h->nsub;
     if (h->d_slopes_cap < need) {
@@ -534,7 +587,7 @@ int shwfs_debug_spots(shwfs_handle *h, const float *phase_dev, int32_t T, int32_
         if (e != cudaSuccess) { shwfs_note_cuda_error(e, "cudaMalloc(debug slopes)"); return SHWFS_ENOMEM; }
         h->d_slopes_cap = need;
     }
-    return run_path(h, phase_dev, T, h->d_slopes, stage, out_dev, 0u, (cudaStream_t)cuda_stream);
+    return run_path(h, phase_dev, T, T, h->d_slopes, stage, out_dev, 0u, (cudaStream_t)cuda_stream);
 }
 
 }  // extern "C"
@@ -609,7 +662,6 @@ static int measure_host_impl(shwfs_handle *h, const float *phase_host, int32_t T
             for (int k = 0; k < 2; ++k)
                 if (!h->h_pin[k]) CU_TRY(cudaHostAlloc(&h->h_pin[k], sizeof(float) * (size_t)h->N * h->N * h->chunk_frames, cudaHostAllocDefault), "cudaHostAlloc");
         int c = 0;
-        h->call_T = T;                          /* the chunks are parts of one call: same kernel instance for all */
         for (int t0 = 0; t0 < T; t0 += chunk_steps, ++c) {
             const int k = c & 1;
             const int tc = (T - t0 < chunk_steps) ? T - t0 : chunk_steps;
@@ -640,16 +692,15 @@ static int measure_host_impl(shwfs_handle *h, const float *phase_host, int32_t T
             }
             CU_TRY(cudaEventRecord(h->ev_h2d[k], h->st_copy), "cudaEventRecord");
             CU_TRY(cudaStreamWaitEvent(h->st_comp, h->ev_h2d[k], 0), "cudaStreamWaitEvent");
-            rc = run_path(h, h->d_phase[k], tc, h->d_slopes + 2 * (size_t)t0 * h->nsub, -1, nullptr, (unsigned)t0, h->st_comp);
-            if (rc) { h->call_T = 0; goto fail; }
+            /* the chunks are parts of one call of T frames: same kernel instance for all */
+            rc = run_path(h, h->d_phase[k], tc, T, h->d_slopes + 2 * (size_t)t0 * h->nsub, -1, nullptr, (unsigned)t0, h->st_comp);
+            if (rc) goto fail;
             CU_TRY(cudaEventRecord(h->ev_done[k], h->st_comp), "cudaEventRecord");
         }
-        h->call_T = 0;
         CU_TRY(cudaMemcpyAsync(slopes_host, h->d_slopes, sizeof(float) * n_slopes, cudaMemcpyDeviceToHost, h->st_comp), "cudaMemcpyAsync(D2H)");
         if (wait) CU_TRY(cudaStreamSynchronize(h->st_comp), "cudaStreamSynchronize");
     }
 fail:
-    h->call_T = 0;
     if (rc && h->st_comp) { cudaStreamSynchronize(h->st_comp); cudaStreamSynchronize(h->st_copy); }
     if (prev >= 0 && prev != h->device) cudaSetDevice(prev);
     return rc;

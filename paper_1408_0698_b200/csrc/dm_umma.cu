@@ -207,11 +207,12 @@ template <int NP>
 cudaError_t launch_umma(shwfs_handle *h, int T, float *out, cudaStream_t st)
 {
     using Cfg = UmCfg<NP>;
-    static bool attr_done = false;
-    if (!attr_done) {
+    static shwfs_once_per_device attr;
+    int dev;
+    if (attr.pending(&dev)) {
         cudaError_t e = cudaFuncSetAttribute(dm_umma_kernel<NP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        attr.mark(dev);
     }
     const int nn = h->n * h->n;
     dm_umma_kernel<NP><<<dim3((unsigned)((T + UM_MT - 1) / UM_MT), (unsigned)h->nsub), 128, Cfg::SMEM, st>>>(

@@ -106,5 +106,75 @@ __device__ __forceinline__ void fft_fma(float (&re)[L], float (&im)[L])
 template <int L>
 __host__ __device__ constexpr int fft_out_index(int k) { return bitrev(k, ilog2(L)); }
 
+/* ---------------------------------------------------------------------------------------------------------
+ * The same transform on packed complex registers (float2 = (re, im) in an even register pair), sm_100a.
+ * Blackwell's FP32x2 instructions (FFMA2 / FADD2 / FMUL2) take a 64-bit register pair per operand, a scalar
+ * immediate broadcast to both halves, and a per-operand half swizzle with per-half negation (SASS
+ * `-R8.F32x2.LO_HI.NP`), so multiplication by +-i costs nothing and a complex rotation is ONE instruction:
+ *     w b = c (b + t (-b_i, b_r)),  t = s / c      ->  pq = FFMA2((-b_i, b_r), t, b)
+ *     a +- w b                                      ->  FFMA2(pq, +-c, a)
+ * A general butterfly is 3 instructions instead of 6, a trivial one (w = 1, +-i) 2 FADD2 instead of 4 FADD:
+ * 194 instructions at L = 32 (162 pruned to 16 inputs) against 388 (324).  The FMA pipe does the same work
+ * (an FP32x2 instruction occupies it for two cycles); what is halved is the issue slots, which is what
+ * bounded the line transforms (profiles/r02_pf32_tma.md: issue 76 %, FMA pipe 59 %).  Arithmetic and
+ * rounding are those of fft_fma, element for element.
+ * ------------------------------------------------------------------------------------------------------- */
+__device__ __forceinline__ float2 rot_pi2(float2 b) { return make_float2(-b.y, b.x); }     /* +i b */
+__device__ __forceinline__ float2 rot_mi2(float2 b) { return make_float2(b.y, -b.x); }     /* -i b */
+__device__ __forceinline__ float2 neg2(float2 b) { return make_float2(-b.x, -b.y); }
+__device__ __forceinline__ float2 bc2(float c) { return make_float2(c, c); }
+
+template <int L, int SIGN, int NZ, int S, int I>
+struct DitBf2 {
+    __device__ __forceinline__ static void run(float2 (&z)[L])
+    {
+        constexpr int bits = ilog2(L);
+        constexpr int h = 1 << (S - 1);
+        constexpr int j = I % h;
+        constexpr int i0 = (I / h) * 2 * h + j, i1 = i0 + h;
+        constexpr int p0 = bitrev(i0, bits), p1 = bitrev(i1, bits);
+        constexpr bool az = bitrev((i0 / h) * h, bits) >= NZ;
+        constexpr bool bz = bitrev((i1 / h) * h, bits) >= NZ;
+        constexpr int k64 = ((SIGN > 0 ? j : -j) * (64 / (2 * h))) & 63;
+        if constexpr (az) {
+            static_assert(!az || bz, "prefix of non-zero inputs");
+        } else if constexpr (bz) {
+            z[p1] = z[p0];
+        } else {
+            const float2 a = z[p0], b = z[p1];
+            if constexpr (k64 == 0) {
+                z[p0] = __fadd2_rn(a, b); z[p1] = __fadd2_rn(a, neg2(b));
+            } else if constexpr (k64 == 16) {           /* w = +i */
+                z[p0] = __fadd2_rn(a, rot_pi2(b)); z[p1] = __fadd2_rn(a, rot_mi2(b));
+            } else if constexpr (k64 == 48) {           /* w = -i */
+                z[p0] = __fadd2_rn(a, rot_mi2(b)); z[p1] = __fadd2_rn(a, rot_pi2(b));
+            } else {
+                constexpr float c = cos64(k64), s = sin64(k64);
+                constexpr bool tanform = (c < 0 ? -c : c) >= (s < 0 ? -s : s);
+                if constexpr (tanform) {
+                    constexpr float t = (float)((double)s / (double)c);
+                    const float2 pq = __ffma2_rn(rot_pi2(b), bc2(t), b);          /* (br - t bi, bi + t br) */
+                    z[p0] = __ffma2_rn(pq, bc2(c), a); z[p1] = __ffma2_rn(pq, bc2(-c), a);
+                } else {
+                    constexpr float ct = (float)((double)c / (double)s);
+                    const float2 pq = __ffma2_rn(b, bc2(ct), rot_pi2(b));         /* (ct br - bi, ct bi + br) */
+                    z[p0] = __ffma2_rn(pq, bc2(s), a); z[p1] = __ffma2_rn(pq, bc2(-s), a);
+                }
+            }
+        }
+        if constexpr (I + 1 < L / 2) DitBf2<L, SIGN, NZ, S, I + 1>::run(z);
+        else if constexpr ((1 << S) < L) DitBf2<L, SIGN, NZ, S + 1, 0>::run(z);
+    }
+};
+
+/* In-place L-point FFT on packed complex registers; output k at position fft_out_index<L>(k). */
+template <int L, int SIGN, int NZ = L>
+__device__ __forceinline__ void fft_fma2(float2 (&z)[L])
+{
+    static_assert(L >= 2 && L <= 64 && (L & (L - 1)) == 0, "L must be a power of two <= 64");
+    static_assert(NZ >= 1 && NZ <= L, "at least one non-zero input");
+    DitBf2<L, SIGN, NZ, 1, 0>::run(z);
+}
+
 }  // namespace shwfs
 #endif

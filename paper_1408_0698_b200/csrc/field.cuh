@@ -20,5 +20,15 @@ __device__ __forceinline__ float2 field_value(float ph, float amp, float turns, 
     return make_float2(amp * c, amp * s);
 }
 
+/* the same under unit amplitude (fully lit subapertures) */
+__device__ __forceinline__ float2 field_unit(float ph, float turns, float ramp)
+{
+    float u = fmaf(ph, turns, -ramp);
+    u -= rintf(u);
+    float s, c;
+    __sincosf(u * 6.283185307179586f, &s, &c);
+    return make_float2(c, s);
+}
+
 }  // namespace shwfs
 #endif

@@ -14,6 +14,8 @@
 
 #include "../../include/shwfs.h"
 
+#define SHWFS_PATCH_LIT (1 << 30)
+
 struct shwfs_handle {
     /* geometry */
     int N, S, n, P, b, D, nsub;
@@ -23,12 +25,16 @@ struct shwfs_handle {
     int has_kernels;
     int algo;              /* resolved SHWFS_ALGO_* used by shwfs_measure */
     int algo_explicit;     /* 1: chosen by shwfs_set_algorithm (non-AUTO): no per-call choice between instances */
-    int call_T;            /* > 0 while the host pipeline feeds one call in chunks: the size the per-call choice sees */
+    int sms;               /* multiprocessors of `device` (grid sizing, per-call instance choice)              */
+    int dm_fp32;           /* SHWFS_DM_FP32 was set when shwfs_set_dm ran: keep the FP32 SIMT GEMM for batches    */
     int64_t launches;
 
     /* device tables (owned) */
     float  *d_amp;         /* [N*N] amplitude mask                                             */
     int2   *d_valid;       /* [nsub] (x = sy, y = sx)                                          */
+    int2   *d_patch;       /* [nsub] (x = sx*n | SHWFS_PATCH_LIT, y = sy*n): patch origin in pixels; the flag says
+                              every amplitude of the patch is exactly 1 (the kernel then reads no amplitude) */
+    int     no_tma;        /* SHWFS_NO_TMA was set at create: register-gather instances only (A/B runs)   */
     float  *d_kernels;     /* [nsub*P*P] spatial elongation kernels (kept for lazy tables)     */
     float2 *d_wk_table;    /* lag-domain table M: [nsub][n][2n-1] (or [1][n][2n-1] w/o kernels) */
     int     wk_table_stride; /* elements between subapertures: n*(2n-1), or 0 when shared      */
@@ -60,7 +66,6 @@ struct shwfs_handle {
     float *h_pin[2];       /* pinned staging for pageable callers */
     float *d_phase[2];     /* device frame chunks */
     float *d_slopes;       /* device slopes for the whole call, grown on demand */
-    float *h_slopes_pin;   /* pinned landing buffer for slopes of a pageable caller */
     size_t d_slopes_cap;   /* floats */
     /* bands of lenslet rows with one bounding column extent of their valid subapertures: the host pipeline
      * copies only these (H1 never reads anything else).  band = {first lenslet row, rows, first column,
@@ -79,8 +84,10 @@ struct shwfs_handle {
 /* Lag-domain table M, built once at create in float64 on the device. */
 cudaError_t shwfs_wk_build_table(shwfs_handle *h, cudaStream_t st);
 
-/* Wiener-Khinchin path: slopes (and optionally the binned image B, [T*nsub*D*D]) */
-cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *slopes,
+/* Wiener-Khinchin path: slopes (and optionally the binned image B, [T*nsub*D*D]).  call_T = frames of the
+ * whole API call this launch is a part of (== T unless the host pipeline feeds the call in chunks): the
+ * per-call choice between kernel instances is made on it, so every chunk of one call takes the same instance. */
+cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, int call_T, float *slopes,
                             float *binned_or_null, float *noisy_or_null, unsigned t_base,
                             const float *dm_patch_or_null, int generic, cudaStream_t st);
 
@@ -112,5 +119,20 @@ cudaError_t shwfs_pruned_fft_launch(shwfs_handle *h, const float *phase, int T, 
 int shwfs_pruned_fft_supported(const shwfs_handle *h);
 
 void shwfs_note_cuda_error(cudaError_t e, const char *where);
+
+/* cudaFuncSetAttribute is per device: a launcher keeps one of these per kernel instance and sets the
+ * attribute the first time it runs on each device (a handle's calls arrive with h->device current).  */
+struct shwfs_once_per_device {
+    bool done[64];
+    /* true if `set` still has to run on the current device; mark() after it succeeded */
+    bool pending(int *dev_out)
+    {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        *dev_out = dev;
+        return dev < 0 || dev >= 64 || !done[dev];
+    }
+    void mark(int dev) { if (dev >= 0 && dev < 64) done[dev] = true; }
+};
 
 #endif /* SHWFS_INTERNAL_H_ */

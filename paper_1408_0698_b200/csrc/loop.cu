@@ -296,7 +296,7 @@ cudaError_t shwfs_loop_dm_phase(shwfs_handle *h, const float *coef, int ldc, int
     /* batches go to the tensor cores (dm_umma.cu) when the split operand tiles exist; SHWFS_DM_FP32=1 keeps the
      * FP32 SIMT GEMM below (A/B comparisons) */
     if (T > 8 && h->d_um_modes && h->d_um_coef && h->um_coef_cap >= shwfs_umma_coef_floats(T, M) &&
-        !getenv("SHWFS_DM_FP32"))
+        !h->dm_fp32)
         return shwfs_umma_dm_phase(h, coef, ldc, T, out, st);
     if (h->nsub <= 65535 && (nn == 64 || nn == 100 || nn == 256)) {
         switch (nn) {

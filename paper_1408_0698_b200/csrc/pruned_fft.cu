@@ -6,23 +6,38 @@
  * Steps H1 gather, H2 field, H3 zero-padded P x P DFT, H4 |.|^2/P^2, H6 centre + b x b bin, H7 threshold,
  * H8 centre of gravity of include/shwfs.h, D = P/b = 16 detector pixels per side.
  *
- * Thread mapping: 16 threads (a half-warp) per spot, 8 spots per tile, persistent CTAs striding over the tiles
- * (the gather of the next tile is issued before the column pass of the current one), no CTA-wide barrier.
- *   row pass     thread r < n owns patch row r: 8-byte gathers, sincos, one P-point DIF FFT in registers
- *                whose inputs >= NZ are known zeros (first stage free); the n x P result goes to shared
- *                memory with the columns permuted (u -> (u mod b) * 16 + u / b) so that the column pass
- *                reads conflict-free.  Rows >= n are zero and are never transformed.
+ * Thread mapping: 16 threads (a half-warp) per spot, 8 spots per tile, persistent CTAs striding over the tiles,
+ * no CTA-wide barrier (a half-warp never waits for another).
+ *   H1           TMA instances (n = 16, 16-byte aligned frames): lane 0 of the half-warp issues ONE
+ *                cp.async.bulk.tensor box (16 x 16 fp32, 64-byte swizzle) per spot into a 1 KB staging slot,
+ *                completion on the half-warp's own mbarrier; the box of tile k+1 is requested as soon as the
+ *                row pass of tile k has read the slot, and lands during the column pass.  The gather costs
+ *                no registers and no L1 data-pipe wavefronts (tma.cuh).  Other sizes: thread r gathers patch
+ *                row r by 8-byte loads one tile ahead, in registers.
+ *                Amplitude: subapertures whose n x n amplitudes are all exactly 1 (93 % of config 2) are
+ *                flagged in the patch table at create and read no amplitude at all.
+ *   row pass     thread r < n owns patch row r: sincos, one P-point FFT in registers whose inputs >= NZ are
+ *                known zeros (first stage free); the n x P result goes to shared memory with the columns
+ *                permuted (u -> (u mod b) * 16 + u / b) so that the column pass reads conflict-free.
+ *                Rows >= n are zero and are never transformed.
  *   column pass  thread c owns the b adjacent columns b*c .. b*c+b-1 = detector column c ^ 8: for each, an
  *                NZ-input P-point FFT down the column, |.|^2, and the row half of the b x b bin
  *                accumulated in registers at compile-time positions (the roll by P/2 is an xor, the
- *                bit reversal of the DIF output a renaming).  The thread ends with one detector column.
+ *                bit reversal of the output a renaming).  The thread ends with one detector column.
  *   H7 + H8      cog16 (cog.cuh): max / sums by xor shuffles inside the half-warp; lane 0 writes 8 bytes.
  * Only the phase patch is read from and the two slopes written to HBM.
+ *
+ * The table lookup of a spot (the only dependent load of the gather) is issued two tiles ahead and nothing is
+ * computed from it before the tile it belongs to: in the round-1 kernel the offset arithmetic sat right
+ * behind the lookup and held 18 % of all stall samples (profiles/r02_pf32_tma.md).
  */
+#include <string.h>
+
 #include "internal.h"
 #include "fft_regs.cuh"
 #include "field.cuh"
 #include "cog.cuh"
+#include "tma.cuh"
 
 namespace {
 
@@ -30,11 +45,12 @@ using namespace shwfs;
 
 constexpr int PF_THREADS = 128;
 constexpr int PF_SPOTS = PF_THREADS / 16;
+constexpr int PF_SLOT = 1024;                  /* bytes of one staged 16 x 16 fp32 patch */
 
 struct PfArgs {
     const float *phase;
     const float *amp;
-    const int2 *valid;
+    const int2 *patch;        /* [nsub] {first column of the patch | SHWFS_PATCH_LIT, first row of the patch} */
     float *slopes;
     float *binned;            /* stage-2 debug image [T*nsub*16*16] or null */
     long long frame_stride;
@@ -42,90 +58,173 @@ struct PfArgs {
     float tau, turns, ramp_unit;
 };
 
-template <int P, int NZ>
+template <int P, int NZ, bool TMA>
 struct PfCfg {
     static constexpr int b = P / 16;
     static constexpr int LD = 2 * P + 4;                 /* floats per stored row; LD/4 odd => STS.128 conflict-free */
     static constexpr int TILE = NZ * LD;                 /* floats per spot */
-    static constexpr size_t SMEM = sizeof(float) * (size_t)PF_SPOTS * TILE;
+    static constexpr size_t TILES = sizeof(float) * (size_t)PF_SPOTS * TILE;
+    /* TMA: [slack to a 1 KB boundary][8 staging slots][8 mbarriers][tiles] */
+    static constexpr size_t STAGE = TMA ? (size_t)PF_SPOTS * PF_SLOT + 64 : 0;
+    static constexpr size_t SMEM = TILES + STAGE + (TMA ? 1024 : 0);
+#ifndef PF_TMA_CTAS
+#define PF_TMA_CTAS 4
+#endif
+    static constexpr int MIN_CTAS = P == 64 ? 2 : (TMA ? PF_TMA_CTAS : 4);
     static_assert(P == 16 || P == 32 || P == 64, "P must be 16, 32 or 64 (D = 16)");
     static_assert(NZ <= 16 && NZ <= P && NZ % 2 == 0, "at most 16 non-zero rows, one per thread");
+    static_assert(!TMA || NZ == 16, "the TMA box is 16 x 16");
 };
 
 /* position of column u in a stored row: the b columns of one detector column are P/b apart */
 template <int P>
 __host__ __device__ constexpr int col_pos(int u) { return (u % (P / 16)) * 16 + u / (P / 16); }
 
-/* H1 of one spot row: the NZ/2 pixel pairs of patch row r of spot g (zeros when the row does not exist) */
+/* one spot of the persistent sweep: g = i*T + t (frame fastest), pe = its entry of the patch table */
+struct PfSpot {
+    int g, i, t;
+    int2 pe;
+};
+
+/* H1 of one spot row without TMA: the NZ/2 pixel pairs of patch row r (zeros when the row does not exist) */
 template <int NZ>
-__device__ __forceinline__ void pf_gather(const PfArgs &A, int off, int t, float2 (&ph)[NZ / 2], float2 (&am)[NZ / 2])
+__device__ __forceinline__ void pf_gather(const PfArgs &A, const PfSpot &s, int r, float2 (&ph)[NZ / 2], float2 (&am)[NZ / 2])
 {
+    const bool lit = (s.pe.x & SHWFS_PATCH_LIT) != 0;
 #pragma unroll
     for (int q = 0; q < NZ / 2; ++q) { ph[q] = make_float2(0.f, 0.f); am[q] = make_float2(0.f, 0.f); }
-    if (off >= 0) {                         /* off: pixel offset of this thread's patch row, -1 if there is none */
-        const float2 *pp = reinterpret_cast<const float2 *>(A.phase + (size_t)t * A.frame_stride + off);
+    if (s.g < A.total && r < A.n) {
+        const int off = (s.pe.y + r) * A.N + (s.pe.x & ~SHWFS_PATCH_LIT);
+        const float2 *pp = reinterpret_cast<const float2 *>(A.phase + (size_t)s.t * A.frame_stride + off);
         const float2 *pa = reinterpret_cast<const float2 *>(A.amp + off);
 #pragma unroll
         for (int q = 0; q < NZ / 2; ++q)
-            if (2 * q < A.n) { ph[q] = __ldg(pp + q); am[q] = __ldg(pa + q); }
+            if (2 * q < A.n) {
+                ph[q] = __ldg(pp + q);
+                am[q] = lit ? make_float2(1.f, 1.f) : __ldg(pa + q);
+            }
     }
 }
 
-
-template <int P, int NZ, int MODE>
-__global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel(const PfArgs A)
+template <int P, int NZ, int MODE, bool TMA>
+__global__ void __launch_bounds__(PF_THREADS, PfCfg<P, NZ, TMA>::MIN_CTAS)
+pruned_fft_kernel(const PfArgs A, const __grid_constant__ CUtensorMap tmap)
 {
-    using Cfg = PfCfg<P, NZ>;
+    using Cfg = PfCfg<P, NZ, TMA>;
     constexpr int b = Cfg::b, LD = Cfg::LD, HP = P / 2;
-    extern __shared__ __align__(16) float pf_smem[];
+    extern __shared__ __align__(16) unsigned char pf_smem[];
     const int tid = threadIdx.x, sp = tid >> 4, r = tid & 15;
-    float *tile = pf_smem + sp * Cfg::TILE;
 
-    /* persistent CTAs: CTA b takes tiles b, b + gridDim.x, ... (the host sizes the grid to the resident CTAs of
-     * the device, so a launch has no ragged last wave).  Two tiles of look-ahead: the valid-list lookup (the
-     * only dependent load of the gather) of tile k+2 and the gather of tile k+1 fly during tile k. */
-    const int ntiles = (A.total + PF_SPOTS - 1) / PF_SPOTS;
-    auto row_offset = [&](int tile_id, int &tt) {
-        const int g = tile_id * PF_SPOTS + sp;
-        tt = 0;
-        if (tile_id >= ntiles || g >= A.total || r >= A.n) return -1;
-        const int i = g / A.T;
-        const int2 yx = __ldg(A.valid + i);
-        tt = g - i * A.T;
-        return (yx.x * A.n + r) * A.N + yx.y * A.n;
+    unsigned char *base = pf_smem;
+    if (TMA) base += (1024u - (smem_addr(pf_smem) & 1023u)) & 1023u;        /* the swizzle pattern is in address bits */
+    unsigned char *slot = base + sp * PF_SLOT;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(base + PF_SPOTS * PF_SLOT) + sp;
+    float *tile = reinterpret_cast<float *>(base + Cfg::STAGE) + sp * Cfg::TILE;
+
+    /* persistent CTAs: CTA c takes tiles c, c + gridDim.x, ... (the host sizes the grid to the resident CTAs of
+     * the device, so a launch has no ragged last wave).  (i, t) of the spot advance by a fixed step: no division
+     * in the loop. */
+    const int stride = gridDim.x * PF_SPOTS;
+    const int dq = stride / A.T, dr = stride - dq * A.T;
+    auto advance = [&](PfSpot &s) {
+        s.g += stride; s.i += dq; s.t += dr;
+        if (s.t >= A.T) { s.t -= A.T; ++s.i; }
     };
-    int tt0, tt1;
-    int off0 = row_offset(blockIdx.x, tt0);
-    int off1 = row_offset(blockIdx.x + gridDim.x, tt1);
-    float2 ph[NZ / 2], am[NZ / 2];
-    pf_gather<NZ>(A, off0, tt0, ph, am);
+    auto lookup = [&](PfSpot &s) { s.pe = __ldg(A.patch + min(s.i, A.nsub - 1)); };
+    auto request = [&](const PfSpot &s) {                 /* TMA: one box per spot, issued by the half-warp's lane 0 */
+        if (r == 0 && s.g < A.total) {
+            mbar_expect_tx(bar, PF_SLOT);
+            tma_load_patch(slot, &tmap, s.pe.x & ~SHWFS_PATCH_LIT, s.pe.y, s.t, bar);
+        }
+    };
+
+    PfSpot cur;
+    cur.g = blockIdx.x * PF_SPOTS + sp;
+    cur.i = cur.g / A.T;
+    cur.t = cur.g - cur.i * A.T;
+    lookup(cur);
+    PfSpot nxt = cur;
+    advance(nxt);
+    lookup(nxt);
+
+    float2 ph[TMA ? 1 : NZ / 2], am[TMA ? 1 : NZ / 2];
+    uint32_t parity = 0;
+    if constexpr (TMA) {
+        if (r == 0) {
+            tma_prefetch_map(&tmap);
+            mbar_init(bar, 1);
+            mbar_init_fence();
+        }
+        __syncwarp();
+        request(cur);
+    } else {
+        pf_gather<NZ>(A, cur, r, ph, am);
+    }
 
 #pragma unroll 1
-    for (int tile_id = blockIdx.x; tile_id < ntiles; tile_id += gridDim.x) {
-        const int g = tile_id * PF_SPOTS + sp;
-        const bool live = g < A.total;
-        int i = 0, t = 0;
-        if (live) { i = g / A.T; t = g - i * A.T; }
+    for (; cur.g - sp < A.total; ) {
+        const bool live = cur.g < A.total;
+        const bool lit = (cur.pe.x & SHWFS_PATCH_LIT) != 0;
+        const int o_cur = live ? cur.t * A.nsub + cur.i : -1;     /* all that is left of `cur` after the row pass */
 
-        float re[P], im[P];
+        float2 z[P];                                       /* packed (re, im): FP32x2 butterflies, fft_regs.cuh */
 
         /* ---- row pass: H2 field, P-point FFT of row r (inputs >= NZ are zero) ---- */
         if (r < NZ) {
             if (live && r < A.n) {
+                if constexpr (TMA) {
+                    /* the ramp -(r + k)/(2P) in two steps, -r/(2P) before and the compile-time k/(2P) after the
+                     * data-dependent product: written as one term per pixel the compiler hoists 16 loop-invariant
+                     * ramps out of the tile loop and spills them */
+                    const float nramp_r = -(float)r * (0.5f / (float)P);
+                    const int sw = (r >> 1) & 3;    /* 64-byte swizzle: chunk q of row r sits at chunk q ^ sw */
+                    const float4 *srow = reinterpret_cast<const float4 *>(slot + r * 64);
+                    if (lit) {                      /* every amplitude of the patch is 1: nothing else to read */
+                        mbar_wait(bar, parity);
 #pragma unroll
-                for (int q = 0; q < NZ / 2; ++q) {
-                    const float ramp = (float)(r + 2 * q) * A.ramp_unit;
-                    const float2 e0 = field_value(ph[q].x, am[q].x, A.turns, ramp);
-                    const float2 e1 = field_value(ph[q].y, am[q].y, A.turns, ramp + A.ramp_unit);
-                    re[2 * q] = e0.x; im[2 * q] = e0.y;
-                    re[2 * q + 1] = e1.x; im[2 * q + 1] = e1.y;
+                        for (int q = 0; q < NZ / 4; ++q) {
+                            const float4 v = srow[q ^ sw];
+                            const float pv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                const int k = 4 * q + e;
+                                z[k] = field_unit(fmaf(pv[e], A.turns, nramp_r), 1.0f, (float)k * (0.5f / (float)P));
+                            }
+                        }
+                    } else {                        /* partially lit subaperture: its amplitude row, 16-byte loads */
+                        const float4 *pa = reinterpret_cast<const float4 *>(
+                            A.amp + (size_t)(cur.pe.y + r) * A.N + (cur.pe.x & ~SHWFS_PATCH_LIT));
+                        float4 av[NZ / 4];
+#pragma unroll
+                        for (int q = 0; q < NZ / 4; ++q) av[q] = __ldg(pa + q);
+                        mbar_wait(bar, parity);
+#pragma unroll
+                        for (int q = 0; q < NZ / 4; ++q) {
+                            const float4 v = srow[q ^ sw];
+                            const float pv[4] = {v.x, v.y, v.z, v.w};
+                            const float aa[4] = {av[q].x, av[q].y, av[q].z, av[q].w};
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                const int k = 4 * q + e;
+                                z[k] = field_value(fmaf(pv[e], A.turns, nramp_r), aa[e], 1.0f, (float)k * (0.5f / (float)P));
+                            }
+                        }
+                    }
+                    parity ^= 1u;
+                } else {
+#pragma unroll
+                    for (int q = 0; q < NZ / 2; ++q) {
+                        const float ramp = (float)(r + 2 * q) * A.ramp_unit;
+                        z[2 * q] = field_value(ph[q].x, am[q].x, A.turns, ramp);
+                        z[2 * q + 1] = field_value(ph[q].y, am[q].y, A.turns, ramp + A.ramp_unit);
+                    }
                 }
 #pragma unroll
-                for (int k = NZ; k < P; ++k) { re[k] = 0.f; im[k] = 0.f; }
-                fft_fma<P, -1, NZ>(re, im);
+                for (int k = NZ; k < P; ++k) z[k] = make_float2(0.f, 0.f);
+                fft_fma2<P, -1, NZ>(z);
             } else {
 #pragma unroll
-                for (int k = 0; k < P; ++k) { re[k] = 0.f; im[k] = 0.f; }
+                for (int k = 0; k < P; ++k) z[k] = make_float2(0.f, 0.f);
             }
             float4 *row = reinterpret_cast<float4 *>(tile + r * LD);
 #pragma unroll
@@ -134,36 +233,34 @@ __global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel
                 const int p0 = 2 * q, p1 = 2 * q + 1;
                 const int u0 = (p0 % 16) * b + p0 / 16, u1 = (p1 % 16) * b + p1 / 16;
                 const int x0 = fft_out_index<P>(u0), x1 = fft_out_index<P>(u1);
-                row[q] = make_float4(re[x0], im[x0], re[x1], im[x1]);
+                row[q] = make_float4(z[x0].x, z[x0].y, z[x1].x, z[x1].y);
             }
         }
-        __syncwarp();
+        __syncwarp();                                      /* rows visible; the staging slot has been read */
         /* H1 of the next tile: in flight during the column pass */
-        pf_gather<NZ>(A, off1, tt1, ph, am);
-        off1 = row_offset(tile_id + 2 * gridDim.x, tt1);
+        if constexpr (TMA) request(nxt);
+        else pf_gather<NZ>(A, nxt, r, ph, am);
 
         /* ---- column pass: b columns per thread, |.|^2 and the row half of the bin in registers ---- */
-        float acc[16];
-#pragma unroll
-        for (int R = 0; R < 16; ++R) acc[R] = 0.f;
+        float acc[16];                                     /* one register per detector row between two columns */
 #pragma unroll
         for (int be = 0; be < b; ++be) {
             const float2 *colp = reinterpret_cast<const float2 *>(tile) + be * 16 + r;
 #pragma unroll
-            for (int v = 0; v < NZ; ++v) {
-                const float2 f = colp[v * (LD / 2)];
-                re[v] = f.x; im[v] = f.y;
-            }
+            for (int v = 0; v < NZ; ++v) z[v] = colp[v * (LD / 2)];
 #pragma unroll
-            for (int v = NZ; v < P; ++v) { re[v] = 0.f; im[v] = 0.f; }
-            fft_fma<P, -1, NZ>(re, im);
+            for (int v = NZ; v < P; ++v) z[v] = make_float2(0.f, 0.f);
+            fft_fma2<P, -1, NZ>(z);
 #pragma unroll
             for (int R = 0; R < 16; ++R) {
+                /* (sum re^2, sum im^2) of the b rows of detector row R, one FFMA2 per value */
+                float2 a2 = be == 0 ? make_float2(0.f, 0.f) : make_float2(acc[R], 0.f);
 #pragma unroll
                 for (int al = 0; al < b; ++al) {
                     const int x = fft_out_index<P>((R * b + al) ^ HP);      /* H6: roll by P/2, then bin */
-                    acc[R] = fmaf(re[x], re[x], fmaf(im[x], im[x], acc[R]));
+                    a2 = (be == 0 && al == 0) ? __fmul2_rn(z[x], z[x]) : __ffma2_rn(z[x], z[x], a2);
                 }
+                acc[R] = a2.x + a2.y;
             }
         }
         constexpr float inv_pp = 1.0f / ((float)P * (float)P);
@@ -173,8 +270,8 @@ __global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel
         /* ---- H7 + H8: thread r holds detector column C = r ^ 8 ---- */
         const int C = r ^ 8;
         const float2 sl = cog16<MODE>(acc, C, A.tau);
-        if (live) {
-            const size_t o = (size_t)t * A.nsub + i;
+        if (o_cur >= 0) {
+            const size_t o = (size_t)o_cur;
             if (r == 0) reinterpret_cast<float2 *>(A.slopes)[o] = sl;
             if (A.binned) {
 #pragma unroll
@@ -182,36 +279,48 @@ __global__ void __launch_bounds__(PF_THREADS, P == 64 ? 2 : 4) pruned_fft_kernel
             }
         }
         __syncwarp();                                      /* the tile is rewritten by the next row pass */
+        /* table lookup of the tile after the next: it has the whole next row pass to arrive (the table is a few KB,
+         * L1/L2 resident), and nothing of it is live across a column pass */
+        cur = nxt;
+        advance(nxt);
+        lookup(nxt);
     }
 }
 
-template <int P, int NZ, int MODE>
-cudaError_t launch_pf_mode(const PfArgs &A, cudaStream_t st)
+template <int P, int NZ, int MODE, bool TMA>
+cudaError_t launch_pf_inst(shwfs_handle *h, const PfArgs &A, const CUtensorMap &map, cudaStream_t st)
 {
-    using Cfg = PfCfg<P, NZ>;
-    if (Cfg::SMEM > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(pruned_fft_kernel<P, NZ, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    using Cfg = PfCfg<P, NZ, TMA>;
+    static shwfs_once_per_device attr;
+    static int resident[64];                        /* CTAs each device holds at once */
+    int dev;
+    if (attr.pending(&dev)) {
+        cudaError_t e = cudaFuncSetAttribute(pruned_fft_kernel<P, NZ, MODE, TMA>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
+        int per_sm = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pruned_fft_kernel<P, NZ, MODE, TMA>, PF_THREADS, Cfg::SMEM);
+        if (dev >= 0 && dev < 64) resident[dev] = h->sms * (per_sm > 0 ? per_sm : 1);
+        attr.mark(dev);
     }
     const int ntiles = (A.total + PF_SPOTS - 1) / PF_SPOTS;
-    static int resident = 0;                       /* CTAs the device holds at once */
-    if (resident == 0) {
-        int dev = 0, sms = 0, per_sm = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pruned_fft_kernel<P, NZ, MODE>, PF_THREADS, Cfg::SMEM);
-        resident = sms * (per_sm > 0 ? per_sm : 1);
-    }
-    const int grid = ntiles < resident ? ntiles : resident;
-    pruned_fft_kernel<P, NZ, MODE><<<grid, PF_THREADS, Cfg::SMEM, st>>>(A);
+    const int res = (dev >= 0 && dev < 64 && resident[dev] > 0) ? resident[dev] : h->sms;
+    const int grid = ntiles < res ? ntiles : res;
+    pruned_fft_kernel<P, NZ, MODE, TMA><<<grid, PF_THREADS, Cfg::SMEM, st>>>(A, map);
     return cudaGetLastError();
 }
 
 template <int P, int NZ>
-cudaError_t launch_pf(const PfArgs &A, int mode, cudaStream_t st)
+cudaError_t launch_pf(shwfs_handle *h, const PfArgs &A, cudaStream_t st)
 {
-    return mode == 0 ? launch_pf_mode<P, NZ, 0>(A, st) : launch_pf_mode<P, NZ, 1>(A, st);
+    CUtensorMap map;
+    if constexpr (NZ == 16) {
+        /* TMA instance when a patch is a legal box: n = 16, frames 16-byte aligned with a 16-byte row pitch */
+        if (h->n == 16 && !h->no_tma && shwfs_tma_patch_map(&map, A.phase, h->N, A.T, 16))
+            return h->mode == 0 ? launch_pf_inst<P, NZ, 0, true>(h, A, map, st) : launch_pf_inst<P, NZ, 1, true>(h, A, map, st);
+    }
+    memset(&map, 0, sizeof(map));
+    return h->mode == 0 ? launch_pf_inst<P, NZ, 0, false>(h, A, map, st) : launch_pf_inst<P, NZ, 1, false>(h, A, map, st);
 }
 
 }  // namespace
@@ -225,7 +334,7 @@ cudaError_t shwfs_pruned_fft_launch(shwfs_handle *h, const float *phase, int T, 
                                     cudaStream_t st)
 {
     PfArgs A;
-    A.phase = phase; A.amp = h->d_amp; A.valid = h->d_valid; A.slopes = slopes; A.binned = binned;
+    A.phase = phase; A.amp = h->d_amp; A.patch = h->d_patch; A.slopes = slopes; A.binned = binned;
     A.frame_stride = (long long)h->N * h->N;
     A.T = T; A.N = h->N; A.nsub = h->nsub; A.total = T * h->nsub; A.n = h->n;
     A.tau = h->tau;
@@ -234,9 +343,9 @@ cudaError_t shwfs_pruned_fft_launch(shwfs_handle *h, const float *phase, int T, 
     if (A.total == 0) return cudaSuccess;
     h->launches += 1;
     switch (h->P) {
-    case 16: return h->n <= 8 ? launch_pf<16, 8>(A, h->mode, st) : launch_pf<16, 16>(A, h->mode, st);
-    case 32: return launch_pf<32, 16>(A, h->mode, st);
-    case 64: return launch_pf<64, 16>(A, h->mode, st);
+    case 16: return h->n <= 8 ? launch_pf<16, 8>(h, A, st) : launch_pf<16, 16>(h, A, st);
+    case 32: return launch_pf<32, 16>(h, A, st);
+    case 64: return launch_pf<64, 16>(h, A, st);
     default: return cudaErrorInvalidValue;
     }
 }

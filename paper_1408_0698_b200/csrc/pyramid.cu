@@ -299,13 +299,14 @@ cudaError_t run_chunk(pyrwfs_handle *h, const float *phase, int Tc, float *signa
     A.scale = (float)(1.0 / ((double)h->Kp * pow((double)h->Np, 4.0)));
     const size_t smem = sizeof(float2) * (size_t)(L * (PY_LINES + 1) > PY_LINES * R * (R + 2) ? L * (PY_LINES + 1)
                                                                                               : PY_LINES * R * (R + 2));
-    static bool attr_done = false;
-    if (!attr_done) {
+    static shwfs_once_per_device attr;
+    int dev;
+    if (attr.pending(&dev)) {
         cudaError_t e = cudaFuncSetAttribute(pyr_rows_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(pyr_cols_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(pyr_final_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        attr.mark(dev);
     }
     const int threads = PY_LINES * R;
     pyr_rows_kernel<R><<<dim3((h->N + PY_LINES - 1) / PY_LINES, Tc * h->Kp), threads, smem, st>>>(A);
@@ -471,11 +472,18 @@ int pyrwfs_launch_count(const pyrwfs_handle *h, int64_t *count)
     return SHWFS_OK;
 }
 
+/* pyrwfs_measure / pyrwfs_debug_quadrants launch on the current device: it has to be the handle's */
+static bool pyr_on_device(const pyrwfs_handle *h)
+{
+    int dev = -1;
+    return cudaGetDevice(&dev) == cudaSuccess && dev == h->device;
+}
+
 int pyrwfs_measure(pyrwfs_handle *h, const float *phase_dev, int32_t T, float *signals_dev, void *cuda_stream)
 {
     if (!h || T < 0) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
-    if (!phase_dev || !signals_dev) return SHWFS_EINVAL;
+    if (!phase_dev || !signals_dev || !pyr_on_device(h)) return SHWFS_EINVAL;
     return pyr_run(h, phase_dev, T, signals_dev, nullptr, (cudaStream_t)cuda_stream);
 }
 
@@ -483,7 +491,7 @@ int pyrwfs_debug_quadrants(pyrwfs_handle *h, const float *phase_dev, int32_t T, 
 {
     if (!h || T < 0) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
-    if (!phase_dev || !out_dev) return SHWFS_EINVAL;
+    if (!phase_dev || !out_dev || !pyr_on_device(h)) return SHWFS_EINVAL;
     return pyr_run(h, phase_dev, T, nullptr, out_dev, (cudaStream_t)cuda_stream);
 }
 

@@ -568,14 +568,13 @@ template <int n, int MODE, int EXTK>
 cudaError_t launch_special_mode(const WkArgs &A, cudaStream_t st)
 {
     using Cfg = WkCfg<n>;
-    static bool attr_set[64] = {false};
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (dev >= 0 && dev < 64 && !attr_set[dev]) {
+    static shwfs_once_per_device attr;
+    int dev;
+    if (attr.pending(&dev)) {
         cudaError_t e = cudaFuncSetAttribute(wk_measure_kernel<n, MODE, EXTK>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)WkSmem<n, (EXTK < 2)>::BYTES);
         if (e != cudaSuccess) return e;
-        attr_set[dev] = true;
+        attr.mark(dev);
     }
     const int grid = (A.total + Cfg::SPOTS - 1) / Cfg::SPOTS;
     wk_measure_kernel<n, MODE, EXTK><<<grid, Cfg::THREADS, WkSmem<n, (EXTK < 2)>::BYTES, st>>>(A);
@@ -613,7 +612,7 @@ cudaError_t shwfs_wk_build_table(shwfs_handle *h, cudaStream_t st)
     return cudaGetLastError();
 }
 
-cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *slopes, float *binned,
+cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, int call_T, float *slopes, float *binned,
                             float *noisy, unsigned t_base, const float *dm_patch, int generic, cudaStream_t st)
 {
     WkArgs A;
@@ -638,10 +637,8 @@ cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, float *s
      * one or two frames (the closed-loop step) is less than a wave of their 32-spot CTAs and runs at the latency of one
      * CTA; the half-warp-per-spot FFT instance spreads it over four times as many CTAs without CTA barriers */
     if (!generic && !h->algo_explicit && h->algo == SHWFS_ALGO_WK && h->D == 16 && (h->n == 8 || h->n == 10)) {
-        static int sms = 0;
-        if (sms == 0) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
-        const long long call_spots = (long long)(h->call_T > 0 ? h->call_T : T) * h->nsub;
-        if (call_spots <= 64LL * sms) return shwfs_wk_fft_launch(A, h->n, st);
+        const long long call_spots = (long long)(call_T > T ? call_T : T) * h->nsub;
+        if (call_spots <= 64LL * h->sms) return shwfs_wk_fft_launch(A, h->n, st);
     }
     if (h->algo != SHWFS_ALGO_WK && !generic && shwfs_wk_fft_supported(h))   /* explicit WK: direct sums */
         return shwfs_wk_fft_launch(A, h->n, st);
