@@ -37,6 +37,7 @@ void free_handle(shwfs_handle *h)
     cudaFree(h->d_amp);
     cudaFree(h->d_valid);
     cudaFree(h->d_patch);
+    cudaFree(h->d_sched);
     cudaFree(h->d_kernels);
     cudaFree(h->d_wk_table);
     cudaFree(h->d_khat);
@@ -248,6 +249,8 @@ int shwfs_create(const shwfs_geometry *g, float lambda_m, int32_t pad, int32_t b
         if (e1 == cudaSuccess) e1 = cudaMemcpy(h->d_patch, patch, sizeof(int2) * (size_t)nsub, cudaMemcpyHostToDevice);
         free(patch);
         CU_TRY(e1, "patch table");
+        CU_TRY(cudaMalloc(&h->d_sched, 2 * sizeof(int)), "cudaMalloc(sched)");
+        CU_TRY(cudaMemset(h->d_sched, 0, 2 * sizeof(int)), "cudaMemset(sched)");
     }
     if (h->has_kernels) {
         const size_t kb = sizeof(float) * (size_t)nsub * P * P;

@@ -176,5 +176,23 @@ __device__ __forceinline__ void fft_fma2(float2 (&z)[L])
     DitBf2<L, SIGN, NZ, 1, 0>::run(z);
 }
 
+/* The same transform of x = xr + i xi given as two scalar arrays: the first stage (w = 1 everywhere) is done with
+ * scalar additions that write the (re, im) pairs, the rest is packed.  For inputs that are produced one scalar at
+ * a time (wk_fft.cu step C: two real columns into one complex transform): asking for them as register pairs
+ * pins 2L registers for as long as the first half is live, this form lets them sit anywhere.                */
+template <int L, int SIGN>
+__device__ __forceinline__ void fft_fma2_split(const float (&xr)[L], const float (&xi)[L], float2 (&z)[L])
+{
+    static_assert(L >= 4 && L <= 64 && (L & (L - 1)) == 0, "L must be a power of two in 4..64");
+    constexpr int bits = ilog2(L);
+#pragma unroll
+    for (int I = 0; I < L / 2; ++I) {
+        const int p0 = bitrev(2 * I, bits), p1 = bitrev(2 * I + 1, bits);
+        z[p0] = make_float2(xr[p0] + xr[p1], xi[p0] + xi[p1]);
+        z[p1] = make_float2(xr[p0] - xr[p1], xi[p0] - xi[p1]);
+    }
+    DitBf2<L, SIGN, L, 2, 0>::run(z);
+}
+
 }  // namespace shwfs
 #endif

@@ -34,9 +34,10 @@ struct shwfs_handle {
     int2   *d_valid;       /* [nsub] (x = sy, y = sx)                                          */
     int2   *d_patch;       /* [nsub] (x = sx*n | SHWFS_PATCH_LIT, y = sy*n): patch origin in pixels; the flag says
                               every amplitude of the patch is exactly 1 (the kernel then reads no amplitude) */
+    int    *d_sched;       /* [2] chunk counters of the persistent kernels' dynamic sweep (sweep.cuh), zero between launches */
     int     no_tma;        /* SHWFS_NO_TMA was set at create: register-gather instances only (A/B runs)   */
     float  *d_kernels;     /* [nsub*P*P] spatial elongation kernels (kept for lazy tables)     */
-    float2 *d_wk_table;    /* lag-domain table M: [nsub][n][2n-1] (or [1][n][2n-1] w/o kernels) */
+    float2 *d_wk_table;    /* lag-domain table M: [nsub][2n-1][n] (or [1][2n-1][n] w/o kernels) */
     int     wk_table_stride; /* elements between subapertures: n*(2n-1), or 0 when shared      */
     float2 *d_khat;        /* literal chain: DFT of the re-centred kernel, [nsub][P][P]; lazy  */
 

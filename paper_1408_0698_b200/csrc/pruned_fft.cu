@@ -6,8 +6,8 @@
  * Steps H1 gather, H2 field, H3 zero-padded P x P DFT, H4 |.|^2/P^2, H6 centre + b x b bin, H7 threshold,
  * H8 centre of gravity of include/shwfs.h, D = P/b = 16 detector pixels per side.
  *
- * Thread mapping: 16 threads (a half-warp) per spot, 8 spots per tile, persistent CTAs striding over the tiles,
- * no CTA-wide barrier (a half-warp never waits for another).
+ * Thread mapping: 16 threads (a half-warp) per spot, 8 spots per tile, persistent CTAs each taking a contiguous
+ * run of tiles (sweep.cuh), no CTA-wide barrier (a half-warp never waits for another).
  *   H1           TMA instances (n = 16, 16-byte aligned frames): lane 0 of the half-warp issues ONE
  *                cp.async.bulk.tensor box (16 x 16 fp32, 64-byte swizzle) per spot into a 1 KB staging slot,
  *                completion on the half-warp's own mbarrier; the box of tile k+1 is requested as soon as the
@@ -38,6 +38,7 @@
 #include "field.cuh"
 #include "cog.cuh"
 #include "tma.cuh"
+#include "sweep.cuh"
 
 namespace {
 
@@ -80,21 +81,15 @@ struct PfCfg {
 template <int P>
 __host__ __device__ constexpr int col_pos(int u) { return (u % (P / 16)) * 16 + u / (P / 16); }
 
-/* one spot of the persistent sweep: g = i*T + t (frame fastest), pe = its entry of the patch table */
-struct PfSpot {
-    int g, i, t;
-    int2 pe;
-};
-
 /* H1 of one spot row without TMA: the NZ/2 pixel pairs of patch row r (zeros when the row does not exist) */
 template <int NZ>
-__device__ __forceinline__ void pf_gather(const PfArgs &A, const PfSpot &s, int r, float2 (&ph)[NZ / 2], float2 (&am)[NZ / 2])
+__device__ __forceinline__ void pf_gather(const PfArgs &A, const Spot &s, bool live, int r, float2 (&ph)[NZ / 2], float2 (&am)[NZ / 2])
 {
-    const bool lit = (s.pe.x & SHWFS_PATCH_LIT) != 0;
+    const bool lit = s.lit();
 #pragma unroll
     for (int q = 0; q < NZ / 2; ++q) { ph[q] = make_float2(0.f, 0.f); am[q] = make_float2(0.f, 0.f); }
-    if (s.g < A.total && r < A.n) {
-        const int off = (s.pe.y + r) * A.N + (s.pe.x & ~SHWFS_PATCH_LIT);
+    if (live && r < A.n) {
+        const int off = (s.row0() + r) * A.N + s.col0();
         const float2 *pp = reinterpret_cast<const float2 *>(A.phase + (size_t)s.t * A.frame_stride + off);
         const float2 *pa = reinterpret_cast<const float2 *>(A.amp + off);
 #pragma unroll
@@ -121,31 +116,20 @@ pruned_fft_kernel(const PfArgs A, const __grid_constant__ CUtensorMap tmap)
     uint64_t *bar = reinterpret_cast<uint64_t *>(base + PF_SPOTS * PF_SLOT) + sp;
     float *tile = reinterpret_cast<float *>(base + Cfg::STAGE) + sp * Cfg::TILE;
 
-    /* persistent CTAs: CTA c takes tiles c, c + gridDim.x, ... (the host sizes the grid to the resident CTAs of
-     * the device, so a launch has no ragged last wave).  (i, t) of the spot advance by a fixed step: no division
-     * in the loop. */
-    const int stride = gridDim.x * PF_SPOTS;
-    const int dq = stride / A.T, dr = stride - dq * A.T;
-    auto advance = [&](PfSpot &s) {
-        s.g += stride; s.i += dq; s.t += dr;
-        if (s.t >= A.T) { s.t -= A.T; ++s.i; }
-    };
-    auto lookup = [&](PfSpot &s) { s.pe = __ldg(A.patch + min(s.i, A.nsub - 1)); };
-    auto request = [&](const PfSpot &s) {                 /* TMA: one box per spot, issued by the half-warp's lane 0 */
-        if (r == 0 && s.g < A.total) {
+    /* persistent CTAs (sweep.cuh): the host sizes the grid to the resident CTAs of the device, so a launch has no
+     * ragged last wave */
+    Sweep sw_(A.patch, nullptr, A.T, A.nsub, A.total, 0);      /* strided deal: no table, calls of any size */
+    auto request = [&](const Spot &s) {                   /* TMA: one box per spot, issued by the half-warp's lane 0 */
+        if (r == 0 && sw_.live(s)) {
             mbar_expect_tx(bar, PF_SLOT);
-            tma_load_patch(slot, &tmap, s.pe.x & ~SHWFS_PATCH_LIT, s.pe.y, s.t, bar);
+            tma_load_patch(slot, &tmap, s.col0(), s.row0(), s.t, bar);
         }
     };
 
-    PfSpot cur;
-    cur.g = blockIdx.x * PF_SPOTS + sp;
-    cur.i = cur.g / A.T;
-    cur.t = cur.g - cur.i * A.T;
-    lookup(cur);
-    PfSpot nxt = cur;
-    advance(nxt);
-    lookup(nxt);
+    Spot cur = sw_.first();
+    Spot nxt = cur;
+    sw_.advance(nxt);
+    sw_.lookup(nxt);
 
     float2 ph[TMA ? 1 : NZ / 2], am[TMA ? 1 : NZ / 2];
     uint32_t parity = 0;
@@ -158,13 +142,13 @@ pruned_fft_kernel(const PfArgs A, const __grid_constant__ CUtensorMap tmap)
         __syncwarp();
         request(cur);
     } else {
-        pf_gather<NZ>(A, cur, r, ph, am);
+        pf_gather<NZ>(A, cur, sw_.live(cur), r, ph, am);
     }
 
 #pragma unroll 1
-    for (; cur.g - sp < A.total; ) {
-        const bool live = cur.g < A.total;
-        const bool lit = (cur.pe.x & SHWFS_PATCH_LIT) != 0;
+    for (; sw_.mine(cur); ) {
+        const bool live = sw_.live(cur);
+        const bool lit = cur.lit();
         const int o_cur = live ? cur.t * A.nsub + cur.i : -1;     /* all that is left of `cur` after the row pass */
 
         float2 z[P];                                       /* packed (re, im): FP32x2 butterflies, fft_regs.cuh */
@@ -193,7 +177,7 @@ pruned_fft_kernel(const PfArgs A, const __grid_constant__ CUtensorMap tmap)
                         }
                     } else {                        /* partially lit subaperture: its amplitude row, 16-byte loads */
                         const float4 *pa = reinterpret_cast<const float4 *>(
-                            A.amp + (size_t)(cur.pe.y + r) * A.N + (cur.pe.x & ~SHWFS_PATCH_LIT));
+                            A.amp + (size_t)(cur.row0() + r) * A.N + cur.col0());
                         float4 av[NZ / 4];
 #pragma unroll
                         for (int q = 0; q < NZ / 4; ++q) av[q] = __ldg(pa + q);
@@ -239,7 +223,7 @@ pruned_fft_kernel(const PfArgs A, const __grid_constant__ CUtensorMap tmap)
         __syncwarp();                                      /* rows visible; the staging slot has been read */
         /* H1 of the next tile: in flight during the column pass */
         if constexpr (TMA) request(nxt);
-        else pf_gather<NZ>(A, nxt, r, ph, am);
+        else pf_gather<NZ>(A, nxt, sw_.live(nxt), r, ph, am);
 
         /* ---- column pass: b columns per thread, |.|^2 and the row half of the bin in registers ---- */
         float acc[16];                                     /* one register per detector row between two columns */
@@ -282,9 +266,10 @@ pruned_fft_kernel(const PfArgs A, const __grid_constant__ CUtensorMap tmap)
         /* table lookup of the tile after the next: it has the whole next row pass to arrive (the table is a few KB,
          * L1/L2 resident), and nothing of it is live across a column pass */
         cur = nxt;
-        advance(nxt);
-        lookup(nxt);
+        sw_.advance(nxt);
+        sw_.lookup(nxt);
     }
+    sw_.leave();
 }
 
 template <int P, int NZ, int MODE, bool TMA>
@@ -303,9 +288,9 @@ cudaError_t launch_pf_inst(shwfs_handle *h, const PfArgs &A, const CUtensorMap &
         if (dev >= 0 && dev < 64) resident[dev] = h->sms * (per_sm > 0 ? per_sm : 1);
         attr.mark(dev);
     }
-    const int ntiles = (A.total + PF_SPOTS - 1) / PF_SPOTS;
+    const int need = (A.total + PF_SPOTS - 1) / PF_SPOTS;
     const int res = (dev >= 0 && dev < 64 && resident[dev] > 0) ? resident[dev] : h->sms;
-    const int grid = ntiles < res ? ntiles : res;
+    const int grid = need < res ? need : res;
     pruned_fft_kernel<P, NZ, MODE, TMA><<<grid, PF_THREADS, Cfg::SMEM, st>>>(A, map);
     return cudaGetLastError();
 }

@@ -32,7 +32,8 @@ using namespace shwfs;
 
 /* ------------------------------------------------------------------------------------------------
  * Table M (float64 on the device, stored as float2).  One CTA per subaperture (or one CTA in all
- * when there are no kernels).  Layout M[i][ly][a], a = lx + n - 1.
+ * when there are no kernels).  Layout M[i][a][ly], a = lx + n - 1: lag row ly is a column, so that the threads of
+ * wk_fft.cu (thread = lag row) read 16 consecutive entries per load instead of 16 rows 8(2n-1) bytes apart.
  * ---------------------------------------------------------------------------------------------- */
 __global__ void wk_table_kernel(const float *__restrict__ K, int has_k, int n, int P, int b,
                                 float2 *__restrict__ M)
@@ -85,8 +86,8 @@ __global__ void wk_table_kernel(const float *__restrict__ K, int has_k, int n, i
         }
         const double br = byr * bxr - byi * bxi, bi = byr * bxi + byi * bxr;
         const double scale = inv_pp * (ly >= 1 ? 2.0 : 1.0);
-        M[(size_t)i * n * LX + idx] = make_float2((float)((zr * br - zi * bi) * scale),
-                                                  (float)((zr * bi + zi * br) * scale));
+        M[(size_t)i * n * LX + a * n + ly] = make_float2((float)((zr * br - zi * bi) * scale),
+                                                         (float)((zr * bi + zi * br) * scale));
     }
 }
 
@@ -371,7 +372,7 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkSmem<n, (EXTK < 2)>::MIN_
                 /* first pass: row slot = warp in the H buffer; second pass: same slot in the field buffer,
                  * once every warp has finished reading the field */
                 if (pass == 1) __syncthreads();
-                finish_row<n>(acc, Mi + ly * Cfg::LX, (pass == 0 ? hb : ebuf + lane * Cfg::ES) + warp * 32);
+                finish_row<n>(acc, Mi + ly, (pass == 0 ? hb : ebuf + lane * Cfg::ES) + warp * 32);
             } else {
                 /* several sub-layers: everything up to the table product is linear in the intensity, so the raw
                  * lag row piles up in shared memory and only the last sub-layer pays the table product and
@@ -385,7 +386,7 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkSmem<n, (EXTK < 2)>::MIN_
 #pragma unroll
                     for (int a = 0; a < Cfg::LX; ++a) grow[a] = acc[a];
                 } else {
-                    finish_row<n, true>(acc, Mi + ly * Cfg::LX, hb + ly * Cfg::RS);
+                    finish_row<n, true>(acc, Mi + ly, hb + ly * Cfg::RS);
                 }
             }
         }
@@ -490,7 +491,7 @@ __global__ void __launch_bounds__(GEN_THREADS) wk_generic_kernel(const WkArgs A,
                 gr = fmaf(u.x, v.x, fmaf(u.y, v.y, gr));     /* u * conj(v) */
                 gi = fmaf(u.y, v.x, fmaf(-u.x, v.y, gi));
             }
-        const float2 mv = Mi[idx];
+        const float2 mv = Mi[(idx - ly * LX) * n + ly];
         float2 sv = make_float2(gr * mv.x - gi * mv.y, gr * mv.y + gi * mv.x);
         if (layer > 0) { sv.x += S[idx].x; sv.y += S[idx].y; }      /* sub-layer arrays piled up */
         S[idx] = sv;
@@ -626,6 +627,8 @@ cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, int call
     A.key = make_uint2((unsigned)h->nz_seed, (unsigned)(h->nz_seed >> 32));
     A.t0 = h->nz_first_frame + t_base;
     A.dm_patch = dm_patch;
+    A.patch = h->d_patch;
+    A.sched = h->d_sched;
     A.T = T; A.N = h->N; A.nsub = h->nsub; A.mstride = h->wk_table_stride;
     A.total = T * h->nsub; A.mode = h->mode;
     A.tau = h->tau;
@@ -638,10 +641,10 @@ cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, int call
      * CTA; the half-warp-per-spot FFT instance spreads it over four times as many CTAs without CTA barriers */
     if (!generic && !h->algo_explicit && h->algo == SHWFS_ALGO_WK && h->D == 16 && (h->n == 8 || h->n == 10)) {
         const long long call_spots = (long long)(call_T > T ? call_T : T) * h->nsub;
-        if (call_spots <= 64LL * h->sms) return shwfs_wk_fft_launch(A, h->n, st);
+        if (call_spots <= 64LL * h->sms) return shwfs_wk_fft_launch(h, A, h->n, st);
     }
     if (h->algo != SHWFS_ALGO_WK && !generic && shwfs_wk_fft_supported(h))   /* explicit WK: direct sums */
-        return shwfs_wk_fft_launch(A, h->n, st);
+        return shwfs_wk_fft_launch(h, A, h->n, st);
     if (!generic && shwfs_wk_supported(h, 0)) {
         switch (h->n) {
         case 8: return launch_special<8>(A, st);

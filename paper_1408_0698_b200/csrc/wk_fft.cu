@@ -15,10 +15,14 @@
  * (the closed-loop step, less than a wave of wk.cu's 32-spot CTAs) come here; on batches the direct sums win.
  *
  * Thread mapping: a half-warp per spot, 8 spots per CTA, no CTA-wide barrier; one 16 x 32 complex tile of
- * shared memory per spot is reused by every exchange.
- *   A  thread r owns patch row r: H1 gather (16-byte loads), H2 field (scaled by 2^-5.5 so that the
- *      unnormalised transforms below need no further factor), 32-point FFT of the row (inputs >= 16 are zero)
- *      -> tile[r][u]
+ * shared memory per spot is reused by every exchange.  Every line transform runs on packed (re, im) registers
+ * with FP32x2 butterflies (fft_fma2, fft_regs.cuh).
+ *   A  thread r owns patch row r: H1 gather, H2 field (scaled by 2^-5.5 so that the unnormalised transforms
+ *      below need no further factor), 32-point FFT of the row (inputs >= 16 are zero) -> tile[r][u].
+ *      The plain n = 16 instance (config 5) is persistent and takes its patches by TMA (tma.cuh, sweep.cuh):
+ *      one 16 x 16 box per spot into a 1 KB slot, requested for the CTA's next tile as soon as step A has read
+ *      the slot, so that it lands during steps B-F; fully lit subapertures read no amplitude.  The other
+ *      instances gather with 16- or 8-byte loads at the head of the CTA, one tile per CTA.
  *   B  thread c owns columns c and c + 16: 32-point FFT down each (16 non-zero inputs), S[v][u] = |.|^2; the
  *      two columns run through one copy of the code (a rolled loop): the kernel is straight-line code of
  *      ~3 k instructions per thread and stalls on instruction fetch (ncu: no_instructions first), so code
@@ -38,6 +42,10 @@
 #include "field.cuh"
 #include "cog.cuh"
 #include "noise.cuh"
+#include "tma.cuh"
+#include "sweep.cuh"
+
+#include <string.h>
 
 namespace {
 
@@ -50,41 +58,109 @@ constexpr int WF_SPOTS = WF_THREADS / 16;
 constexpr int WF_LD = 2 * WF_Q + 4;            /* floats per tile row; LD/4 odd => 16-byte row accesses conflict-free */
 constexpr int WF_TILE = WF_ROWS * WF_LD;
 constexpr size_t WF_SMEM = sizeof(float) * (size_t)WF_SPOTS * WF_TILE;
+constexpr int WF_SLOT = 1024;                  /* bytes of one staged 16 x 16 fp32 patch (TMA instance) */
+constexpr size_t WF_STAGE = (size_t)WF_SPOTS * WF_SLOT + 64;      /* slots + one mbarrier per half-warp */
 
 __device__ __forceinline__ constexpr int xq(int k) { return fft_out_index<WF_Q>(k & (WF_Q - 1)); }
 
 /* EXTK as in wk.cu: 0 plain sensor, 1 extensions on one (sub-)layer, 2 several sodium sub-layers (S is linear in the
  * sub-layer intensities: steps A-C run per sub-layer and the separated column transforms pile up in a second
  * tile per spot, each element owned by one thread; D-F run once) */
-template <int n, int MODE, int EXTK>
-__global__ void __launch_bounds__(WF_THREADS, EXTK == 2 ? 3 : 4) wkf_kernel(const WkArgs A)
+template <int n, int MODE, int EXTK, bool TMA>
+__global__ void __launch_bounds__(WF_THREADS, EXTK == 2 ? 3 : 4) wkf_kernel(const WkArgs A, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr bool EXT = EXTK > 0, ML = EXTK == 2;
     static_assert(n % 2 == 0 && n <= WF_ROWS && 2 * n - 1 <= WF_Q, "even n <= 16: one thread per patch row, grid 32 >= 2n-1");
+    static_assert(!TMA || (n == 16 && EXTK == 0), "the TMA box is 16 x 16; extensions gather in registers");
     constexpr int Q = WF_Q, LD = WF_LD, LX = 2 * n - 1;
-    extern __shared__ __align__(16) float wf_smem[];
+    extern __shared__ __align__(16) unsigned char wf_smem[];
     const int tid = threadIdx.x, sp = tid >> 4, r = tid & 15;
-    float *tile = wf_smem + sp * WF_TILE;
-    float *gtile = ML ? wf_smem + (WF_SPOTS + sp) * WF_TILE : tile;      /* where step C leaves g_u[ly] */
+    unsigned char *base = wf_smem;
+    if (TMA) base += (1024u - (smem_addr(wf_smem) & 1023u)) & 1023u;      /* the swizzle pattern is in address bits */
+    unsigned char *slot = base + sp * WF_SLOT;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(base + WF_SPOTS * WF_SLOT) + sp;
+    float *tiles = reinterpret_cast<float *>(base + (TMA ? WF_STAGE : 0));
+    float *tile = tiles + sp * WF_TILE;
+    float *gtile = ML ? tiles + (WF_SPOTS + sp) * WF_TILE : tile;        /* where step C leaves g_u[ly] */
 
-    const int g = blockIdx.x * WF_SPOTS + sp;
-    const bool live = g < A.total;
-    int i = 0, t = 0;
-    if (live) { i = g / A.T; t = g - i * A.T; }
+    /* TMA instance: persistent CTAs striding over the tiles; the others are launched one tile per CTA and run
+     * the loop once */
+    Sweep sw_(A.patch, TMA ? A.sched : nullptr, A.T, A.nsub, A.total, SWEEP_CHUNK);
+    auto request = [&](const Spot &s) {
+        if (r == 0 && sw_.live(s)) {
+            mbar_expect_tx(bar, WF_SLOT);
+            tma_load_patch(slot, &tmap, s.col0(), s.row0(), s.t, bar);
+        }
+    };
+    Spot cur = sw_.first();
+    Spot nxt = cur;
+    uint32_t parity = 0;
+    if constexpr (TMA) {
+        sw_.advance(nxt);
+        sw_.lookup(nxt);
+        if (r == 0) {
+            tma_prefetch_map(&tmap);
+            mbar_init(bar, 1);
+            mbar_init_fence();
+        }
+        __syncwarp();
+        request(cur);
+    }
 
-    float re[Q], im[Q];
+#pragma unroll 1
+    for (; sw_.mine(cur); ) {
+    const bool live = sw_.live(cur);
+    const int i = live ? cur.i : 0, t = live ? cur.t : 0;
+
+    float2 z[Q];
 
     const int n_layers = ML ? A.L : 1;
 #pragma unroll 1
     for (int layer = 0; layer < n_layers; ++layer) {
     /* ---- A: gather, field, row transform (threads r < n) ---- */
     if (r < n) {
+        /* 2^-5.5 on the field = 1/2048 on the intensity: 1/Q^2 of the two unnormalised transforms of S and the
+         * 1/2 of the real-pair separation of step C */
+        float sc = 0.02209708691207961f;
+        if constexpr (TMA) {
+            const float nramp_r = -(float)r * A.ramp_unit;      /* ramp in two steps: see pruned_fft.cu */
+            const float4 *srow = reinterpret_cast<const float4 *>(slot + r * 64);
+            const int sw = (r >> 1) & 3;                        /* 64-byte swizzle: chunk q of row r at chunk q ^ sw */
+            float4 av[n / 4];
+#pragma unroll
+            for (int q = 0; q < n / 4; ++q) av[q] = make_float4(sc, sc, sc, sc);
+            if (live && !cur.lit()) {                           /* partially lit subaperture: its amplitude row */
+                const float4 *pa = reinterpret_cast<const float4 *>(A.amp + (size_t)(cur.row0() + r) * A.N + cur.col0());
+#pragma unroll
+                for (int q = 0; q < n / 4; ++q) {
+                    const float4 w = __ldg(pa + q);
+                    av[q] = make_float4(w.x * sc, w.y * sc, w.z * sc, w.w * sc);
+                }
+            }
+            if (live) {
+                mbar_wait(bar, parity);
+                parity ^= 1u;
+#pragma unroll
+                for (int q = 0; q < n / 4; ++q) {
+                    const float4 v = srow[q ^ sw];
+                    const float pv[4] = {v.x, v.y, v.z, v.w};
+                    const float aa[4] = {av[q].x, av[q].y, av[q].z, av[q].w};
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const int k = 4 * q + e;
+                        z[k] = field_value(fmaf(-(float)k, A.ramp_unit, fmaf(pv[e], A.turns, nramp_r)), aa[e], 1.0f, 0.f);
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < n; ++k) z[k] = make_float2(0.f, 0.f);
+            }
+        } else {
         float pv[n], av[n];
 #pragma unroll
         for (int k = 0; k < n; ++k) { pv[k] = 0.f; av[k] = 0.f; }
         if (live) {
-            const int2 yx = __ldg(A.valid + i);
-            const int off = (yx.x * n + r) * A.N + yx.y * n;
+            const int off = (cur.row0() + r) * A.N + cur.col0();
             const float *pp = A.phase + (size_t)t * A.frame_stride + (ML ? (size_t)layer * A.layer_stride : 0) + off;
             const float *pa = A.amp + off;
             /* PAPER.md:76 "the residual phase (the open loop wavefront subtracted by the DM)" */
@@ -120,9 +196,6 @@ __global__ void __launch_bounds__(WF_THREADS, EXTK == 2 ? 3 : 4) wkf_kernel(cons
                 }
             }
         }
-        /* 2^-5.5 on the field = 1/2048 on the intensity: 1/Q^2 of the two unnormalised transforms of S and the
-         * 1/2 of the real-pair separation of step C */
-        float sc = 0.02209708691207961f;
         float lin0 = 0.f, gx = 0.f, lq = 0.f, dj2 = 0.f;
         const bool sodium = EXT && A.L > 0;
         if (sodium) {
@@ -142,57 +215,57 @@ __global__ void __launch_bounds__(WF_THREADS, EXTK == 2 ? 3 : 4) wkf_kernel(cons
                 const float dk = (float)k - 0.5f * (float)(n - 1);
                 ramp -= fmaf(gx, (float)k, lin0) + lq * (dj2 + dk * dk);
             }
-            const float2 e = field_value(pv[k], av[k] * sc, A.turns, ramp);
-            re[k] = e.x; im[k] = e.y;
+            z[k] = field_value(pv[k], av[k] * sc, A.turns, ramp);
+        }
         }
 #pragma unroll
-        for (int k = n; k < Q; ++k) { re[k] = 0.f; im[k] = 0.f; }
-        fft_fma<Q, -1, n>(re, im);
+        for (int k = n; k < Q; ++k) z[k] = make_float2(0.f, 0.f);
+        fft_fma2<Q, -1, n>(z);
         float4 *row = reinterpret_cast<float4 *>(tile + r * LD);
 #pragma unroll
         for (int q = 0; q < Q / 2; ++q)
-            row[q] = make_float4(re[xq(2 * q)], im[xq(2 * q)], re[xq(2 * q + 1)], im[xq(2 * q + 1)]);
+            row[q] = make_float4(z[xq(2 * q)].x, z[xq(2 * q)].y, z[xq(2 * q + 1)].x, z[xq(2 * q + 1)].y);
     }
     __syncwarp();
+    if constexpr (TMA) request(nxt);             /* the slot has been read: the next tile's patch lands during B-F */
 
-    /* ---- B: column transforms of columns r and r + 16, intensity ---- */
-    float zr[Q], zi[Q];
+    /* ---- B: column transforms of columns r and r + 16, intensity: s0[v] = S[v][r], s1[v] = S[v][r + 16] ---- */
+    float s0[Q], s1[Q];
 #pragma unroll 1                                 /* one copy of the transform's code: the kernel is instruction-fetch bound */
     for (int col = 0; col < 2; ++col) {
         const float2 *colp = reinterpret_cast<const float2 *>(tile) + r + 16 * col;
 #pragma unroll
-        for (int v = 0; v < n; ++v) {
-            const float2 f = colp[v * (LD / 2)];
-            re[v] = f.x; im[v] = f.y;
-        }
+        for (int v = 0; v < n; ++v) z[v] = colp[v * (LD / 2)];
 #pragma unroll
-        for (int v = n; v < Q; ++v) { re[v] = 0.f; im[v] = 0.f; }
-        fft_fma<Q, -1, n>(re, im);
+        for (int v = n; v < Q; ++v) z[v] = make_float2(0.f, 0.f);
+        fft_fma2<Q, -1, n>(z);
 #pragma unroll
         for (int v = 0; v < Q; ++v) {
-            const float s = fmaf(re[xq(v)], re[xq(v)], im[xq(v)] * im[xq(v)]);
-            zi[v] = s;
+            const float2 sq = __fmul2_rn(z[xq(v)], z[xq(v)]);
+            s1[v] = sq.x + sq.y;
         }
         if (col == 0) {
 #pragma unroll
-            for (int v = 0; v < Q; ++v) zr[v] = zi[v];
+            for (int v = 0; v < Q; ++v) s0[v] = s1[v];
         }
     }
     __syncwarp();                                /* every thread has read its columns: the tile can be rewritten */
 
     /* ---- C: both real columns in one complex transform over v, separated by symmetry ---- */
-    fft_fma<Q, -1>(zr, zi);
+    float2 zc[Q];
+    fft_fma2_split<Q, -1>(s0, s1, zc);           /* scalar first stage: s0, s1 need not sit in register pairs */
     {
         float2 *colp = reinterpret_cast<float2 *>(gtile) + r;
 #pragma unroll
         for (int ly = 0; ly < n; ++ly) {
-            const int a = xq(ly), b = xq(Q - ly);
-            /* Z[ly] = g1[ly] + i g2[ly], conj Z[-ly] = g1[ly] - i g2[ly]  (the 1/2 is in the field's scale) */
-            float2 g1 = make_float2(zr[a] + zr[b], zi[a] - zi[b]);
-            float2 g2 = make_float2(zi[a] + zi[b], zr[b] - zr[a]);
+            const float2 za = zc[xq(ly)], zb = zc[xq(Q - ly)];
+            /* Z[ly] = g1[ly] + i g2[ly], conj Z[-ly] = g1[ly] - i g2[ly]  (the 1/2 is in the field's scale):
+             * g1 = Z[ly] + conj Z[-ly], g2 = -i (Z[ly] - conj Z[-ly]) */
+            float2 g1 = __fadd2_rn(za, make_float2(zb.x, -zb.y));
+            float2 g2 = __fadd2_rn(rot_mi2(za), make_float2(zb.y, zb.x));
             if (ML && layer > 0) {
-                const float2 p1 = colp[ly * (LD / 2)], p2 = colp[ly * (LD / 2) + 16];
-                g1.x += p1.x; g1.y += p1.y; g2.x += p2.x; g2.y += p2.y;
+                g1 = __fadd2_rn(g1, colp[ly * (LD / 2)]);
+                g2 = __fadd2_rn(g2, colp[ly * (LD / 2) + 16]);
             }
             colp[ly * (LD / 2)] = g1;
             colp[ly * (LD / 2) + 16] = g2;
@@ -207,33 +280,26 @@ __global__ void __launch_bounds__(WF_THREADS, EXTK == 2 ? 3 : 4) wkf_kernel(cons
 #pragma unroll
         for (int q = 0; q < Q / 2; ++q) {
             const float4 f = row[q];
-            re[2 * q] = f.x; im[2 * q] = f.y; re[2 * q + 1] = f.z; im[2 * q + 1] = f.w;
+            z[2 * q] = make_float2(f.x, f.y); z[2 * q + 1] = make_float2(f.z, f.w);
         }
-        fft_fma<Q, -1>(re, im);
+        /* the thread's row of the tile is free from here to the end of step E: the table row M_i[.][ly = r] is
+         * staged in it while the transform runs */
+        mrow_stage<n>(A.M + (size_t)i * A.mstride + r, tile + r * LD);
+        fft_fma2<Q, -1>(z);
         /* ---- E: table product, alias, x-transform; H[r][0..15] takes the place of the row this thread read ---- */
         float2 acc[LX];
 #pragma unroll
-        for (int a = 0; a < LX; ++a) acc[a] = make_float2(re[xq(a - (n - 1))], im[xq(a - (n - 1))]);
-        const float2 *Mi = A.M + (size_t)i * A.mstride;
-        finish_row<n>(acc, Mi + r * LX, tile + r * LD);
+        for (int a = 0; a < LX; ++a) acc[a] = z[xq(a - (n - 1))];
+        mrow_wait();
+        finish_row2<n>(acc, tile + r * LD, tile + r * LD);
     }
     __syncwarp();
 
     /* ---- F: y-transform (real part), noise, threshold, centre of gravity ---- */
     {
         const int C = r;
-        float yr[16], yi[16];
-#pragma unroll
-        for (int m = 0; m < 16; ++m) {
-            if (m < n) {
-                const float2 v = *reinterpret_cast<const float2 *>(tile + m * LD + 2 * C);
-                yr[m] = v.x; yi[m] = v.y;
-            } else { yr[m] = 0.f; yi[m] = 0.f; }
-        }
-        fft_fma<16, +1, n>(yr, yi);               /* B[R,C] = Re sum_m H[m][C] w_16^(R m) */
         float bcol[16];
-#pragma unroll
-        for (int R = 0; R < 16; ++R) bcol[R] = yr[fft_out_index<16>(R)];
+        ytransform16<n>([&](int m) { return *reinterpret_cast<const float2 *>(tile + m * LD + 2 * C); }, bcol);
         const size_t o = (size_t)t * A.nsub + i;
         if (live && A.binned) {
 #pragma unroll
@@ -249,32 +315,68 @@ __global__ void __launch_bounds__(WF_THREADS, EXTK == 2 ? 3 : 4) wkf_kernel(cons
         const float2 sl = cog16<MODE>(bcol, C, A.tau);
         if (live && C == 0) reinterpret_cast<float2 *>(A.slopes)[o] = sl;
     }
+    __syncwarp();                                /* the tile is rewritten by the next step A */
+    if constexpr (TMA) {
+        cur = nxt;
+        sw_.advance(nxt);
+        sw_.lookup(nxt);                         /* has the whole next step A to arrive */
+    } else {
+        sw_.advance(cur);                        /* one tile per CTA: past the end */
+    }
+    }
+    sw_.leave();
 }
 
-template <int n, int MODE, int EXTK>
-cudaError_t launch_wkf_mode(const WkArgs &A, cudaStream_t st)
+template <int n, int MODE, int EXTK, bool TMA>
+cudaError_t launch_wkf_inst(shwfs_handle *h, const WkArgs &A, const CUtensorMap &map, cudaStream_t st)
 {
-    constexpr size_t smem = EXTK == 2 ? 2 * WF_SMEM : WF_SMEM;
-    static bool attr_set[64] = {false};             /* per device, as in wk.cu */
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (smem > 48 * 1024 && dev >= 0 && dev < 64 && !attr_set[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(wkf_kernel<n, MODE, EXTK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set[dev] = true;
+    constexpr size_t smem = (EXTK == 2 ? 2 * WF_SMEM : WF_SMEM) + (TMA ? WF_STAGE + 1024 : 0);
+    static shwfs_once_per_device attr;
+    static int resident[64];                        /* CTAs each device holds at once (persistent instance) */
+    int dev;
+    if (attr.pending(&dev)) {
+        if (smem > 48 * 1024) {
+            cudaError_t e = cudaFuncSetAttribute(wkf_kernel<n, MODE, EXTK, TMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+        }
+        int per_sm = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, wkf_kernel<n, MODE, EXTK, TMA>, WF_THREADS, smem);
+        if (dev >= 0 && dev < 64) resident[dev] = h->sms * (per_sm > 0 ? per_sm : 1);
+        attr.mark(dev);
     }
-    const int grid = (A.total + WF_SPOTS - 1) / WF_SPOTS;
-    wkf_kernel<n, MODE, EXTK><<<grid, WF_THREADS, smem, st>>>(A);
+    int grid = (A.total + WF_SPOTS - 1) / WF_SPOTS;         /* one tile per CTA */
+    if (TMA) {                                              /* persistent: one chunk of the sweep per warp at least */
+        const int nchunks = (A.total + SWEEP_CHUNK - 1) / SWEEP_CHUNK;
+        const int res = (dev >= 0 && dev < 64 && resident[dev] > 0) ? resident[dev] : h->sms;
+        grid = (nchunks + WF_THREADS / 32 - 1) / (WF_THREADS / 32);
+        if (grid > res) grid = res;
+    }
+    wkf_kernel<n, MODE, EXTK, TMA><<<grid, WF_THREADS, smem, st>>>(A, map);
     return cudaGetLastError();
 }
 
-template <int n>
-cudaError_t launch_wkf(const WkArgs &A, cudaStream_t st)
+template <int n, int MODE, int EXTK>
+cudaError_t launch_wkf_mode(shwfs_handle *h, const WkArgs &A, cudaStream_t st)
 {
-    if (A.L > 1) return A.mode == 0 ? launch_wkf_mode<n, 0, 2>(A, st) : launch_wkf_mode<n, 1, 2>(A, st);
+    CUtensorMap map;
+    if constexpr (n == 16 && EXTK == 0) {
+        /* the persistent instance deals chunks of SWEEP_CHUNK spots dynamically: worth it from ~8 chunks per resident
+         * warp (16 warps per SM) up; smaller calls spread over one-tile CTAs */
+        if (!h->no_tma && (long long)A.total >= 8LL * SWEEP_CHUNK * 16 * h->sms &&
+            shwfs_tma_patch_map(&map, A.phase, A.N, A.T, 16))
+            return launch_wkf_inst<n, MODE, EXTK, true>(h, A, map, st);
+    }
+    memset(&map, 0, sizeof(map));
+    return launch_wkf_inst<n, MODE, EXTK, false>(h, A, map, st);
+}
+
+template <int n>
+cudaError_t launch_wkf(shwfs_handle *h, const WkArgs &A, cudaStream_t st)
+{
+    if (A.L > 1) return A.mode == 0 ? launch_wkf_mode<n, 0, 2>(h, A, st) : launch_wkf_mode<n, 1, 2>(h, A, st);
     if (A.L > 0 || A.flux > 0.f || A.dm_patch != nullptr)
-        return A.mode == 0 ? launch_wkf_mode<n, 0, 1>(A, st) : launch_wkf_mode<n, 1, 1>(A, st);
-    return A.mode == 0 ? launch_wkf_mode<n, 0, 0>(A, st) : launch_wkf_mode<n, 1, 0>(A, st);
+        return A.mode == 0 ? launch_wkf_mode<n, 0, 1>(h, A, st) : launch_wkf_mode<n, 1, 1>(h, A, st);
+    return A.mode == 0 ? launch_wkf_mode<n, 0, 0>(h, A, st) : launch_wkf_mode<n, 1, 0>(h, A, st);
 }
 
 }  // namespace
@@ -284,15 +386,15 @@ int shwfs_wk_fft_supported(const shwfs_handle *h)
     return h->D == 16 && (h->n == 12 || h->n == 14 || h->n == 16);
 }
 
-cudaError_t shwfs_wk_fft_launch(const shwfs::WkArgs &A, int n, cudaStream_t st)
+cudaError_t shwfs_wk_fft_launch(shwfs_handle *h, const shwfs::WkArgs &A, int n, cudaStream_t st)
 {
     static_assert(WF_SMEM <= 48 * 1024, "static limit of dynamic shared memory");
     switch (n) {
-    case 8: return launch_wkf<8>(A, st);
-    case 10: return launch_wkf<10>(A, st);
-    case 12: return launch_wkf<12>(A, st);
-    case 14: return launch_wkf<14>(A, st);
-    case 16: return launch_wkf<16>(A, st);
+    case 8: return launch_wkf<8>(h, A, st);
+    case 10: return launch_wkf<10>(h, A, st);
+    case 12: return launch_wkf<12>(h, A, st);
+    case 14: return launch_wkf<14>(h, A, st);
+    case 16: return launch_wkf<16>(h, A, st);
     default: return cudaErrorInvalidValue;
     }
 }
