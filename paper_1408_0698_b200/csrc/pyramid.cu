@@ -53,52 +53,53 @@ using namespace shwfs;
 
 constexpr int PY_LINES = 8;
 
-/* natural-order copy of a DIF result: out[k] = X[k] */
+/* natural-order copy of a transform result: out[k] = X[k] */
 template <int R>
-__device__ __forceinline__ void unscramble(float (&re)[R], float (&im)[R])
+__device__ __forceinline__ void unscramble(float2 (&z)[R])
 {
 #pragma unroll
     for (int k = 0; k < R; ++k) {
         const int q = fft_out_index<R>(k);
-        if (q > k) {
-            float t = re[k]; re[k] = re[q]; re[q] = t;
-            t = im[k]; im[k] = im[q]; im[q] = t;
-        }
+        if (q > k) { const float2 t = z[k]; z[k] = z[q]; z[q] = t; }
     }
 }
 
-/* One L = R*R point transform of the line owned by the R threads j = 0..R-1 (all in one warp).
- * In : re/im[m] = x[j + R m] (natural order; entries m >= NZ are zero).
- * Out: re/im[q] = X[p + R q], p = this thread's index (natural order).
+/* a * w on packed registers: a_r (w_r, w_i) + a_i (-w_i, w_r), two FP32x2 instructions (fft_regs.cuh) */
+__device__ __forceinline__ float2 cmul2(float2 a, float2 w)
+{
+    return __ffma2_rn(bc2(a.y), rot_pi2(w), __fmul2_rn(bc2(a.x), w));
+}
+
+/* One L = R*R point transform of the line owned by the R threads j = 0..R-1 (all in one warp), on packed
+ * (re, im) registers with FP32x2 butterflies (fft_fma2).
+ * In : z[m] = x[j + R m] (natural order; entries m >= NZ are zero).
+ * Out: z[q] = X[p + R q], p = this thread's index (natural order).
  * X[k] = sum_x x[x] exp(SIGN 2 pi i x k / L).  `line` is this line's R*(R+2) float2 of shared memory.      */
 template <int R, int SIGN, int NZ>
-__device__ __forceinline__ void line_fft(float (&re)[R], float (&im)[R], int j, float2 *__restrict__ line,
+__device__ __forceinline__ void line_fft(float2 (&z)[R], int j, float2 *__restrict__ line,
                                          const float2 *__restrict__ tw)
 {
     constexpr int L = R * R;
-    fft_fma<R, SIGN, NZ>(re, im);
+    fft_fma2<R, SIGN, NZ>(z);
 #pragma unroll
     for (int p = 0; p < R; ++p) {
-        const int x = fft_out_index<R>(p);
-        float a = re[x], b = im[x];
+        float2 a = z[fft_out_index<R>(p)];
         if (p > 0) {
-            const float2 w = __ldg(tw + ((j * p) & (L - 1)));           /* w_L^(j p), conjugated for SIGN < 0 */
-            const float ws = SIGN > 0 ? w.y : -w.y;
-            const float t = a * w.x - b * ws;
-            b = a * ws + b * w.x;
-            a = t;
+            float2 w = __ldg(tw + ((j * p) & (L - 1)));                 /* w_L^(j p), conjugated for SIGN < 0 */
+            if (SIGN < 0) w.y = -w.y;
+            a = cmul2(a, w);
         }
-        line[p * (R + 2) + j] = make_float2(a, b);
+        line[p * (R + 2) + j] = a;
     }
     __syncwarp();
 #pragma unroll
     for (int jj = 0; jj < R; jj += 2) {                                 /* this thread is now p = j */
         const float4 v = *reinterpret_cast<const float4 *>(line + j * (R + 2) + jj);   /* row stride R+2: 16-byte rows */
-        re[jj] = v.x; im[jj] = v.y; re[jj + 1] = v.z; im[jj + 1] = v.w;
+        z[jj] = make_float2(v.x, v.y); z[jj + 1] = make_float2(v.z, v.w);
     }
     __syncwarp();
-    fft_fma<R, SIGN, R>(re, im);
-    unscramble<R>(re, im);
+    fft_fma2<R, SIGN, R>(z);
+    unscramble<R>(z);
 }
 
 /* index of pupil-plane coordinate c (row or column) among the 2N kept ones, or -1 (Q6: copies at +s and -s) */
@@ -130,9 +131,9 @@ __global__ void __launch_bounds__(PY_LINES * R) pyr_rows_kernel(const PyArgs A)
     const int tid = threadIdx.x, b = tid / R, j = tid % R;
     const int tk = blockIdx.y, t = tk / A.Kp, k = tk - t * A.Kp;
     const int y0 = blockIdx.x * PY_LINES, y = y0 + b;
-    float re[R], im[R];
+    float2 z[R];
 #pragma unroll
-    for (int m = 0; m < R; ++m) { re[m] = 0.f; im[m] = 0.f; }
+    for (int m = 0; m < R; ++m) z[m] = make_float2(0.f, 0.f);
     if (y < A.N) {
         const float2 md = __ldg(A.mod + k);                   /* modulation tilt, turns per pixel */
         const float *pp = A.phase + ((size_t)t * A.N + y) * A.N;
@@ -146,16 +147,16 @@ __global__ void __launch_bounds__(PY_LINES * R) pyr_rows_kernel(const PyArgs A)
                 float sn, cs;
                 __sincosf(u * 6.283185307179586f, &sn, &cs);
                 const float a = __ldg(pa + x);
-                re[m] = a * cs; im[m] = a * sn;
+                z[m] = make_float2(a * cs, a * sn);
             }
         }
     }
-    line_fft<R, -1, NZ>(re, im, j, py_smem + b * R * (R + 2), A.tw);
+    line_fft<R, -1, NZ>(z, j, py_smem + b * R * (R + 2), A.tw);
     __syncthreads();
     /* transposed hand-over: stage[u][b] (row padded to 9), then 64-byte segments of A1[tk][u][y0..y0+7] */
     float2 *stage = py_smem;
 #pragma unroll
-    for (int q = 0; q < R; ++q) stage[(j + R * q) * (PY_LINES + 1) + b] = make_float2(re[q], im[q]);
+    for (int q = 0; q < R; ++q) stage[(j + R * q) * (PY_LINES + 1) + b] = z[q];
     __syncthreads();
     float2 *dst = A.A1 + (size_t)tk * L * A.N;
     for (int e = tid; e < L * PY_LINES; e += PY_LINES * R) {
@@ -172,32 +173,31 @@ __global__ void __launch_bounds__(PY_LINES * R, 2) pyr_cols_kernel(const PyArgs 
     extern __shared__ __align__(16) float2 py_smem[];
     const int tid = threadIdx.x, b = tid / R, j = tid % R;
     const int tk = blockIdx.y, u0 = blockIdx.x * PY_LINES, u = u0 + b;
-    float re[R], im[R];
+    float2 z[R];
 #pragma unroll
-    for (int m = 0; m < R; ++m) { re[m] = 0.f; im[m] = 0.f; }
+    for (int m = 0; m < R; ++m) z[m] = make_float2(0.f, 0.f);
     const float2 *src = A.A1 + ((size_t)tk * L + u) * A.N;
 #pragma unroll
     for (int m = 0; m < NZ; ++m) {
         const int y = j + R * m;
-        if (y < A.N) { const float2 v = __ldg(src + y); re[m] = v.x; im[m] = v.y; }
+        if (y < A.N) z[m] = __ldg(src + y);
     }
     float2 *line = py_smem + b * R * (R + 2);
-    line_fft<R, -1, NZ>(re, im, j, line, A.tw);
+    line_fft<R, -1, NZ>(z, j, line, A.tw);
     /* Q3: exp(-2 pi i s (|u~| + |v~|) / Np) at v = j + R q */
     const int ua = u < L / 2 ? u : L - u;
 #pragma unroll
     for (int q = 0; q < R; ++q) {
         const int v = j + R * q, va = v < L / 2 ? v : L - v;
-        const float2 w = __ldg(A.tw + ((A.s * (ua + va)) & (L - 1)));
-        const float a = re[q], c = im[q];
-        re[q] = a * w.x + c * w.y;                            /* times conj(w) */
-        im[q] = c * w.x - a * w.y;
+        float2 w = __ldg(A.tw + ((A.s * (ua + va)) & (L - 1)));
+        w.y = -w.y;                                           /* times conj(w) */
+        z[q] = cmul2(z[q], w);
     }
-    line_fft<R, +1, R>(re, im, j, line, A.tw);
+    line_fft<R, +1, R>(z, j, line, A.tw);
     __syncthreads();
     float2 *stage = py_smem;                                   /* stage[y'][b] */
 #pragma unroll
-    for (int q = 0; q < R; ++q) stage[(j + R * q) * (PY_LINES + 1) + b] = make_float2(re[q], im[q]);
+    for (int q = 0; q < R; ++q) stage[(j + R * q) * (PY_LINES + 1) + b] = z[q];
     __syncthreads();
     float2 *dst = A.A2 + (size_t)tk * 2 * A.N * L;
     /* only the 2N kept rows are written: row r < N is pupil-plane row r + s, row N + d is row (d - s) mod Np
@@ -223,16 +223,13 @@ __global__ void __launch_bounds__(PY_LINES * R, 2) pyr_final_kernel(const PyArgs
     for (int q = 0; q < R; ++q) acc[q] = 0.f;
     float2 *line = py_smem + b * R * (R + 2);
     for (int k = 0; k < A.Kp; ++k) {
-        float re[R], im[R];
+        float2 z[R];
         const float2 *src = A.A2 + (((size_t)t * A.Kp + k) * rows + (live ? r : 0)) * L;
 #pragma unroll
-        for (int m = 0; m < R; ++m) {
-            const float2 v = live ? __ldg(src + j + R * m) : make_float2(0.f, 0.f);
-            re[m] = v.x; im[m] = v.y;
-        }
-        line_fft<R, +1, R>(re, im, j, line, A.tw);
+        for (int m = 0; m < R; ++m) z[m] = live ? __ldg(src + j + R * m) : make_float2(0.f, 0.f);
+        line_fft<R, +1, R>(z, j, line, A.tw);
 #pragma unroll
-        for (int q = 0; q < R; ++q) acc[q] = fmaf(re[q], re[q], fmaf(im[q], im[q], acc[q]));
+        for (int q = 0; q < R; ++q) acc[q] = fmaf(z[q].x, z[q].x, fmaf(z[q].y, z[q].y, acc[q]));
     }
     if (live) {
         float *dst = A.I2 + ((size_t)t * rows + r) * rows;
