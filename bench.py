@@ -38,13 +38,38 @@ F_NOM = {1: 10240, 2: 51200, 3: 153600, 4: 153600, 5: 737280}
 # lanes per SM, FMA = 2 flop): 148 * 128 * 2 * 1.965e9.  Measured FFMA chain on this pool: 72.4 TFLOP/s
 # (profiles/r01_fp32_peak.md).
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-# sm__pipe_fma_cycles_active (fraction of peak) of the dominant kernel in the committed ncu --set full captures
-NCU_FMA_PIPE_ACTIVE = {2: 0.472, 3: 0.636, 4: 0.636, 5: 0.618}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/r01_wk10_full_v5.md, r01_wkf16_full.md, r01_pf32_full.md), keyed by config; None where no
-# capture of that config's kernel exists.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {2: 129117696 + 4491776, 3: 206465280 + 5998336, 4: 206465280 + 5998336,
-                                5: 506622720 + 6679808}
+# Figures that only a profiler can give (FMA-pipe activity, DRAM bytes and executed FP32 flops per launch of the
+# dominant kernel) live in profiles/ncu_constants.json, keyed by the kernel instance name the library reports
+# (shwfs_last_kernel) and stamped with a hash of the sources they were captured at.  They are printed as
+# "not measured in this run" values and become null the moment the sources change (profiles/ncu_constants.md).
+NCU_JSON = ROOT / "profiles" / "ncu_constants.json"
+
+
+def sources_sha1(paths):
+    """sha1 over the named source files (relative to the repo root), in the order given."""
+    import hashlib
+    h = hashlib.sha1()
+    for rel in paths:
+        h.update(rel.encode() + b"\0" + (ROOT / rel).read_bytes())
+    return h.hexdigest()
+
+
+def ncu_constants(kernel):
+    """The committed ncu figures of `kernel`, or (None, why) if there are none for the sources as they stand."""
+    try:
+        table = json.loads(NCU_JSON.read_text())["kernels"]
+    except Exception as e:
+        return None, f"profiles/ncu_constants.json unreadable: {e!r}"
+    ent = table.get(kernel)
+    if ent is None:
+        return None, f"no ncu capture of {kernel} committed"
+    try:
+        now = sources_sha1(ent["sources"])
+    except Exception as e:
+        return None, f"sources of the capture unreadable: {e!r}"
+    if now != ent["sources_sha1"]:
+        return None, f"sources changed since the capture ({ent['capture']}): figures withheld"
+    return ent, f"from {ent['capture']} (ncu, not measured in this run)"
 
 
 def _dist_env():
@@ -156,11 +181,176 @@ def run_reference(args):
 
 
 # ---------------------------------------------------------------------------------------------------
+class Workload:
+    """One config of BASELINE.json on this rank: handles (one per WFS), synthetic frames resident in HBM, outputs."""
+
+    def __init__(self, c, args, L, dev, rank=0, world=1, dm_modes=0, noise_flux=0.0):
+        import torch
+        from paper_1408_0698_b200 import binding as B, workloads as W
+        from paper_1408_0698_b200.distributed import rank_frames
+        self.c, self.L, self.dev, self.torch = c, L, dev, torch
+        frames = self.frames = c.batch
+        my_frames = rank_frames(c.T, frames, rank, world)          # each rank owns its own batch of the stream
+        if L > 0:
+            # the paper's full LGS model (PAPER.md:91, 113: "MAORY configuration and 3 sodium sub-layers"): every
+            # sub-layer has its own wavefront, the elongation comes from the geometry, the kernel is the spot size
+            with B.from_config(c, 0, kernels=None) as probe:
+                yx = probe.valid_yx
+            Ksp = W.spot_size_kernels(c, yx, device=dev)
+            self.sensors = [B.from_config(c, w, kernels=Ksp, valid_yx=yx) for w in range(c.W)]
+            for w, s in enumerate(self.sensors):
+                sod = W.sodium_layers(c, w, L)
+                s.set_sodium(sod["weight"], sod["defocus"], sod["tilt_x"], sod["tilt_y"], (sod["cx"], sod["cy"]))
+            del Ksp
+            layer_frames = [int(t) * L + l for t in my_frames for l in range(L)]
+            self.phase = [W.phase_frames_device(c, w, layer_frames, dev).view(frames, L, c.N, c.N) for w in range(c.W)]
+        else:
+            self.sensors = [B.from_config(c, w) for w in range(c.W)]
+            self.phase = [W.phase_frames_device(c, w, my_frames, dev) for w in range(c.W)]
+        if noise_flux > 0:
+            for w, s in enumerate(self.sensors):
+                s.set_noise(noise_flux / c.n ** 2, args.read_noise, 14080698 + w)
+        self.nsub = self.sensors[0].nsub
+        self.slopes = [torch.empty((frames, self.nsub, 2), dtype=torch.float32, device=dev) for _ in range(c.W)]
+        self.spots_per_step = c.W * frames * self.nsub
+        self.in_bytes = sum(p.numel() * 4 for p in self.phase)
+        self.out_bytes = sum(s.numel() * 4 for s in self.slopes)
+        self.stream = torch.cuda.Stream(dev)
+        # closed-loop neighbours (SURVEY.md 8(f) f3): DM of dm_modes modes, residual fused into the gather
+        self.Mdm = dm_modes
+        if dm_modes > 0:
+            modes = W.dm_modes_device(c, dm_modes, dev)
+            for s in self.sensors:
+                s.set_dm(modes)
+            del modes
+            gen = torch.Generator(device=dev); gen.manual_seed(1408)
+            self.coef = [torch.randn((frames, dm_modes), device=dev, generator=gen) * 0.2 for _ in range(c.W)]
+            self.Rmat = [torch.randn((dm_modes, 2 * self.nsub), device=dev, generator=gen) / self.nsub for _ in range(c.W)]
+            self.cstate = [torch.zeros(dm_modes, device=dev) for _ in range(c.W)]
+
+    def step(self, events=None, closed_loop=False):
+        torch, stream = self.torch, self.stream
+        for w, s in enumerate(self.sensors):
+            if events is not None:
+                e0 = torch.cuda.Event(enable_timing=True); e0.record(stream)
+            if self.Mdm > 0 and closed_loop:
+                with torch.cuda.stream(stream):
+                    s.closed_loop(self.phase[w], self.Rmat[w], 0.3, self.cstate[w], want_history=False, stream=stream)
+            elif self.Mdm > 0:
+                s.measure_residual(self.phase[w], self.coef[w], out=self.slopes[w], stream=stream)
+            else:
+                s.measure(self.phase[w], out=self.slopes[w], stream=stream)
+            if events is not None:
+                e1 = torch.cuda.Event(enable_timing=True); e1.record(stream)
+                events.append((e0, e1))
+
+    def time_device(self, steps, warmup, barrier, sampler=None, closed_loop=False):
+        """W warm-up steps, then K timed steps bracketed by barrier + synchronize on both sides.  Returns total ms
+        (CUDA events on the launching stream), mean ms of one handle's call, kernels launched."""
+        torch, stream = self.torch, self.stream
+        with torch.cuda.stream(stream):
+            for _ in range(warmup):
+                self.step(closed_loop=closed_loop)
+        barrier()
+        l0 = sum(s.launch_count for s in self.sensors)
+        ev = []
+        t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if sampler is not None:
+            sampler.start()
+        with torch.cuda.stream(stream):
+            t_beg.record(stream)
+            for _ in range(steps):
+                self.step(ev, closed_loop=closed_loop)
+            t_end.record(stream)
+        barrier()
+        clocks = sampler.stop() if sampler is not None else None
+        launches = sum(s.launch_count for s in self.sensors) - l0
+        return t_beg.elapsed_time(t_end), float(np.mean([a.elapsed_time(b) for a, b in ev])), int(launches), clocks
+
+    def time_e2e(self, steps, barrier):
+        """The same measurement through shwfs_measure_host_async + shwfs_host_wait from pinned host tensors: H2D of
+        every frame and D2H of the slopes inside the timed region.  Returns seconds, max |host path - device path|."""
+        torch, c = self.torch, self.c
+        h_phase = [torch.empty(tuple(self.phase[0].shape), dtype=torch.float32, pin_memory=True) for _ in range(c.W)]
+        for w in range(c.W):
+            h_phase[w].copy_(self.phase[w])
+        h_slopes = [torch.empty((self.frames, self.nsub, 2), dtype=torch.float32, pin_memory=True) for _ in range(c.W)]
+        for w, s in enumerate(self.sensors):                  # warm-up: allocates the staging buffers
+            s.measure_host(h_phase[w], out=h_slopes[w])
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            for w, s in enumerate(self.sensors):              # the W sensors of the system back to back on the bus
+                s.measure_host_async(h_phase[w], h_slopes[w])
+            for s in self.sensors:
+                s.host_wait()
+        torch.cuda.synchronize(self.dev)
+        dt = time.perf_counter() - t0
+        check = float((h_slopes[0].to(self.dev) - self.slopes[0]).abs().max().item())
+        return dt, check
+
+    def h2d_bytes_per_step(self):
+        c = self.c
+        return sum(s.host_bytes_per_frame * (p.numel() // (c.N * c.N)) for s, p in zip(self.sensors, self.phase))
+
+    def roofline(self, kern_ms):
+        """F_alg x spots per launch / mean launch duration against the derived FP32 peak; beside
+        it the kernel's own executed FP32 flops (from the committed ncu capture of that kernel instance)."""
+        c, L = self.c, self.L
+        spots_per_launch = self.frames * self.nsub
+        fa = f_alg(c, L)
+        ach = fa * spots_per_launch / (kern_ms * 1e-3) / 1e12
+        kernel = self.sensors[0].last_kernel
+        ent, note = ncu_constants(kernel)
+        fx = ent.get("fp32_flops_per_spot") if ent else None
+        return {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": ach / FP32_PEAK_TFLOPS,
+                "traffic": ent.get("dram_bytes_per_launch") if ent else None,
+                "kernel": kernel, "kernel_ms": kern_ms, "spots_per_launch": spots_per_launch,
+                "flops_per_spot": fa, "flops_basis": "F_alg (SURVEY.md 8(d))" if L <= 0 else
+                "L pruned first FFTs + one frame-paired convolution pair (DESIGN.md 7)",
+                "frac_nominal_fft_flops": (F_NOM[c.cfg] * spots_per_launch / (kern_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS
+                                           if L <= 0 else None),
+                "frac_executed": (fx * spots_per_launch / (kern_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS) if fx else None,
+                "flops_executed_per_spot_ncu": fx,
+                "peak_basis": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (measured FFMA chain 72.4)",
+                "fma_pipe_active_ncu": ent.get("fma_pipe_active") if ent else None,
+                "ncu_note": note,
+                "hbm_frac": (self.in_bytes + self.out_bytes) / c.W / (kern_ms * 1e-3) / 1e9 / _hbm_peak()}
+
+    def close(self):
+        for s in self.sensors:
+            s.close()
+        self.phase = self.slopes = None
+        self.torch.cuda.empty_cache()
+
+
+def per_config_entry(cfg_id, L, args, dev, barrier, steps):
+    """One extra workload of the default run: device-resident throughput and roofline of config `cfg_id` (with L
+    sodium sub-layers if L > 0), a few steps, same timing protocol as the headline."""
+    from paper_1408_0698_b200 import workloads as W
+    c = W.CONFIGS[cfg_id]
+    wl = Workload(c, args, L, dev)
+    try:
+        ms_total, kern_ms, launches, _ = wl.time_device(steps, 3, barrier)
+        value = wl.spots_per_step * steps / (ms_total * 1e-3)
+        r = wl.roofline(kern_ms)
+        return {"workload": workload_name(c, L), "value": value, "unit": "spots/s", "steps": steps, "warmup": 3,
+                "wfs_frames_per_s": value / wl.nsub, "system_frames_per_s": value / wl.nsub / c.W,
+                "kernel": r["kernel"], "kernel_ms": kern_ms, "gpu_launches": launches,
+                "roofline": {k: r[k] for k in ("frac", "frac_executed", "frac_nominal_fft_flops", "flops_per_spot",
+                                               "flops_executed_per_spot_ncu", "fma_pipe_active_ncu", "traffic",
+                                               "ncu_note")},
+                "target_50pct_spots_per_s": 0.5 * FP32_PEAK_TFLOPS * 1e12 / f_alg(c, L)}
+    finally:
+        wl.close()
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_1408_0698_b200 import binding as B, workloads as W
-    from paper_1408_0698_b200.distributed import job_throughput, max_over_ranks, rank_frames
+    from paper_1408_0698_b200 import workloads as W
+    from paper_1408_0698_b200.distributed import job_throughput, max_over_ranks
 
     rank, local_rank, world = _dist_env()
     if not torch.cuda.is_available():
@@ -170,90 +360,21 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    c = W.CONFIGS[args.config]
-    frames = c.batch
-    # one handle per WFS (elongation kernels differ by launch point, reading A13), synthetic frames in HBM
-    L = args.sublayers
-    my_frames = rank_frames(c.T, frames, rank, world)          # each rank owns its own batch of the stream
-    if L > 0:
-        # the paper's full LGS model ("MAORY configuration and 3 sodium sub-layers"): every
-        # sub-layer has its own wavefront, the elongation comes from the geometry, the kernel is the spot size
-        with B.from_config(c, 0, kernels=None) as probe:
-            yx = probe.valid_yx
-        Ksp = W.spot_size_kernels(c, yx, device=dev)
-        sensors = [B.from_config(c, w, kernels=Ksp, valid_yx=yx) for w in range(c.W)]
-        for w, s in enumerate(sensors):
-            sod = W.sodium_layers(c, w, L)
-            s.set_sodium(sod["weight"], sod["defocus"], sod["tilt_x"], sod["tilt_y"], (sod["cx"], sod["cy"]))
-        del Ksp
-        layer_frames = [int(t) * L + l for t in my_frames for l in range(L)]
-        phase = [W.phase_frames_device(c, w, layer_frames, dev).view(frames, L, c.N, c.N) for w in range(c.W)]
-    else:
-        sensors = [B.from_config(c, w) for w in range(c.W)]
-        phase = [W.phase_frames_device(c, w, my_frames, dev) for w in range(c.W)]
-    if args.noise_flux > 0:
-        for w, s in enumerate(sensors):
-            s.set_noise(args.noise_flux / c.n ** 2, args.read_noise, 14080698 + w)
-    nsub = sensors[0].nsub
-    slopes = [torch.empty((frames, nsub, 2), dtype=torch.float32, device=dev) for _ in range(c.W)]
-    spots_per_step = c.W * frames * nsub
-    in_bytes = sum(p.numel() * 4 for p in phase)
-    out_bytes = sum(s.numel() * 4 for s in slopes)
-    stream = torch.cuda.Stream(dev)
-
-    # closed-loop neighbours: DM of --dm-modes modes, residual fused into the gather
-    Mdm = args.dm_modes
-    if Mdm > 0:
-        modes = W.dm_modes_device(c, Mdm, dev)
-        for s in sensors:
-            s.set_dm(modes)
-        del modes
-        gen = torch.Generator(device=dev); gen.manual_seed(1408)
-        coef = [torch.randn((frames, Mdm), device=dev, generator=gen) * 0.2 for _ in range(c.W)]
-        Rmat = [torch.randn((Mdm, 2 * nsub), device=dev, generator=gen) / nsub for _ in range(c.W)]
-        cstate = [torch.zeros(Mdm, device=dev) for _ in range(c.W)]
-
-    def step(events=None):
-        for w, s in enumerate(sensors):
-            if events is not None:
-                e0 = torch.cuda.Event(enable_timing=True); e0.record(stream)
-            if Mdm > 0 and args.closed_loop:
-                with torch.cuda.stream(stream):
-                    s.closed_loop(phase[w], Rmat[w], 0.3, cstate[w], want_history=False, stream=stream)
-            elif Mdm > 0:
-                s.measure_residual(phase[w], coef[w], out=slopes[w], stream=stream)
-            else:
-                s.measure(phase[w], out=slopes[w], stream=stream)
-            if events is not None:
-                e1 = torch.cuda.Event(enable_timing=True); e1.record(stream)
-                events.append((e0, e1))
-
     def barrier():
         torch.cuda.synchronize(dev)
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize(dev)
 
+    c = W.CONFIGS[args.config]
+    L, Mdm = args.sublayers, args.dm_modes
+    wl = Workload(c, args, L, dev, rank, world, dm_modes=Mdm, noise_flux=args.noise_flux)
+    nsub, frames, spots_per_step = wl.nsub, wl.frames, wl.spots_per_step
+    warm = max(args.warmup, 3)
+
     # ---- device-resident throughput
-    with torch.cuda.stream(stream):
-        for _ in range(max(args.warmup, 3)):
-            step()
-    barrier()
-    sampler = ClockSampler(local_rank)
-    l0 = sum(s.launch_count for s in sensors)
-    ev = []
-    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler.start()
-    with torch.cuda.stream(stream):
-        t_beg.record(stream)
-        for _ in range(args.steps):
-            step(ev)
-        t_end.record(stream)
-    barrier()
-    clocks = sampler.stop()
-    launches = sum(s.launch_count for s in sensors) - l0
-    ms_total = t_beg.elapsed_time(t_end)
-    kern_ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    ms_total, kern_ms, launches, clocks = wl.time_device(args.steps, warm, barrier, ClockSampler(local_rank),
+                                                         closed_loop=args.closed_loop)
     ms_total = max_over_ranks(ms_total, dev)
     value = job_throughput(spots_per_step, args.steps, ms_total, world)
 
@@ -263,7 +384,7 @@ def run_ours(args):
             spots_per_launch = frames * nsub
             print(json.dumps({
                 "metric": "subaperture_spots_per_s", "value": value, "unit": "spots/s", "n_gpus": world,
-                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps,
+                "steps": args.steps, "warmup": warm, "ms_per_step": ms_total / args.steps,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": workload_name(c, L, args.noise_flux) + f", DM of {Mdm} modes, " +
                            ("sequential pure-integrator loop (shwfs_closed_loop)" if args.closed_loop
@@ -273,70 +394,53 @@ def run_ours(args):
                 "ms_per_wfs_call": kern_ms, "clocks": clocks, "e2e": None, "gpu_launches": int(launches),
                 "dm_flops_per_spot": 2 * Mdm * c.n * c.n,
                 "dm_tflops": 2 * Mdm * c.n * c.n * spots_per_launch / (kern_ms * 1e-3) / 1e12}))
-        for s in sensors:
-            s.close()
+        wl.close()
         if world > 1:
             dist.destroy_process_group()
         return
 
     # ---- end to end from pinned host memory through shwfs_measure_host
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
-    h_phase = [torch.empty(tuple(phase[0].shape), dtype=torch.float32, pin_memory=True) for _ in range(c.W)]
-    for w in range(c.W):
-        h_phase[w].copy_(phase[w])
-    h_slopes = [torch.empty((frames, nsub, 2), dtype=torch.float32, pin_memory=True) for _ in range(c.W)]
-    for w, s in enumerate(sensors):                       # warm-up: allocates the staging buffers
-        s.measure_host(h_phase[w], out=h_slopes[w])
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        for w, s in enumerate(sensors):                   # the W sensors of the system back to back on the bus
-            s.measure_host_async(h_phase[w], h_slopes[w])
-        for s in sensors:
-            s.host_wait()
-    torch.cuda.synchronize(dev)
-    e2e_s = time.perf_counter() - t0
+    e2e_s, e2e_check = wl.time_e2e(e2e_steps, barrier)
     e2e_value = job_throughput(spots_per_step, e2e_steps, 1e3 * max_over_ranks(e2e_s, dev), world)
-    e2e_check = float((h_slopes[0].to(dev) - slopes[0]).abs().max().item())
 
     if rank == 0:
-        spots_per_launch = frames * nsub
-        fa = f_alg(c, L)
-        ach = fa * spots_per_launch / (kern_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                    "frac": ach / FP32_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(c.cfg) if L <= 0 and args.noise_flux <= 0 else None,
-                    "kernel": {B.ALGO_WK: f"wk_measure_kernel<{c.n}>", B.ALGO_WK_FFT: f"wkf_kernel<{c.n}>", B.ALGO_PRUNED_FFT: f"pruned_fft_kernel<{c.P}>",
-                               B.ALGO_LITERAL: f"literal_kernel<{c.P}>"}.get(sensors[0].algorithm, f"algo{sensors[0].algorithm}"),
-                    "kernel_ms": kern_ms, "spots_per_launch": spots_per_launch,
-                    "flops_per_spot": fa, "flops_basis": "F_alg (SURVEY.md 8(d))" if L <= 0 else
-                    "L pruned first FFTs + one frame-paired convolution pair (DESIGN.md 7)",
-                    "frac_nominal_fft_flops": (F_NOM[c.cfg] * spots_per_launch / (kern_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS
-                                               if L <= 0 else None),
-                    "peak_basis": "derived: 148 SM x 128 lanes x 2 x 1.965 GHz (measured FFMA chain 72.4)",
-                    "fma_pipe_active_ncu": NCU_FMA_PIPE_ACTIVE.get(c.cfg) if L <= 0 and args.noise_flux <= 0 else None,
-                    "hbm_frac": (in_bytes + out_bytes) / c.W / (kern_ms * 1e-3) / 1e9 / _hbm_peak()}
-        cpu = None if args.no_cpu_baseline else cpu_baseline(c, args, phase, sensors[0].valid_yx)
+        roofline = wl.roofline(kern_ms)
+        cpu = None if args.no_cpu_baseline else cpu_baseline(c, args, wl.phase, wl.sensors[0].valid_yx)
         out = {
             "metric": "subaperture_spots_per_s", "value": value, "unit": "spots/s", "n_gpus": world,
-            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps,
+            "steps": args.steps, "warmup": warm, "ms_per_step": ms_total / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(c, L, args.noise_flux), "spots_per_step_per_gpu": spots_per_step,
-                       "l2": f"inputs larger than L2 ({in_bytes / 1e6:.0f} MB read per step), no flush"},
+                       "l2": f"inputs larger than L2 ({wl.in_bytes / 1e6:.0f} MB read per step), no flush"},
             "wfs_frames_per_s": value / nsub, "system_frames_per_s": value / nsub / c.W,
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "spots/s",
-                    "h2d_bytes_per_step": sum(s.host_bytes_per_frame * (p.numel() // (c.N * c.N)) for s, p in zip(sensors, phase)),
+                    "h2d_bytes_per_step": wl.h2d_bytes_per_step(),
                     "h2d_note": "only the column runs of valid subapertures cross the bus (shwfs_host_bytes_per_frame); "
-                                f"the pinned host tensors hold {in_bytes} bytes",
-                    "d2h_bytes_per_step": out_bytes,
+                                f"the pinned host tensors hold {wl.in_bytes} bytes",
+                    "d2h_bytes_per_step": wl.out_bytes,
                     "steps": e2e_steps, "api": "shwfs_measure_host_async + shwfs_host_wait (one call per WFS)", "max_abs_diff_vs_device_path": e2e_check},
             "gpu_launches": int(launches),
             "roofline": roofline,
             "cpu_baseline": cpu,
         }
+    wl.close()
+    if rank == 0:
+        # ---- the other north_star configs and the paper's own timing case, a few steps each (single GPU, default run)
+        if args.per_config and world == 1 and L <= 0 and args.noise_flux <= 0:
+            pc = {}
+            for key, cfg_id, Lx in (("2", 2, 0), ("3", 3, 0), ("5", 5, 0), ("4_sublayers3", 4, 3)):
+                if cfg_id == args.config and Lx == 0:
+                    continue
+                try:
+                    pc[key] = per_config_entry(cfg_id, Lx, args, dev, barrier, args.per_config_steps)
+                except Exception as e:     # a failed extra never takes the headline line down with it
+                    pc[key] = {"error": repr(e)}
+            out["per_config"] = pc
+            if not args.no_cpu_baseline:
+                out["cpu_baseline_more"] = cpu_baseline_more(args)
         print(json.dumps(out))
-    for s in sensors:
-        s.close()
     if world > 1:
         dist.destroy_process_group()
 
@@ -443,6 +547,32 @@ def cpu_baseline(c, args, phase_dev, yx_lib=None):
             "sample": f"WFS 0, first {ph.shape[0]} frames of the timed batch = {spots} spots, {dt:.1f} s"}
 
 
+def cpu_baseline_more(args):
+    """SURVEY.md 8(d) 'Oracle timing': the oracle as it stands on config 3 frame 0 in full (4632 spots), on all host
+    cores and on one thread, and on 4 frames of config 5 (all cores)."""
+    from oracle import shwfs_oracle as O
+    from paper_1408_0698_b200 import workloads as W
+    out = {}
+    all_cores = O.max_threads()
+    # the one-thread case goes last: the oracle keeps the thread count it was last given
+    for key, cfg_id, nfr, threads in (("config3_frame0_all_cores", 3, 1, 0), ("config5_4frames_all_cores", 5, 4, 0),
+                                      ("config3_frame0_one_thread", 3, 1, 1)):
+        c = W.CONFIGS[cfg_id]
+        amp = W.pupil_mask(c)
+        yx = O.valid_list(amp, c.n, c.min_illum)
+        K = W.elongation_kernels(c, 0, yx)
+        ph = W.phase_frames(c, 0, range(nfr))
+        t0 = time.perf_counter()
+        O.measure(ph, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K, nthreads=threads)
+        dt = time.perf_counter() - t0
+        spots = nfr * len(yx)
+        out[key] = {"value": spots / dt, "unit": "spots/s", "cores": threads if threads else all_cores,
+                    "kind": "oracle", "sample": f"config {cfg_id}, WFS 0, {nfr} frame(s) = {spots} spots, {dt:.1f} s",
+                    "frames_per_s": nfr / dt,
+                    "extrapolated_s_per_1000_frames_all_wfs": 1000.0 * c.W * dt / nfr}
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -464,6 +594,9 @@ def main():
     ap.add_argument("--pyramid", default=None, choices=["tiny", "lbt"],
                     help="time the pyramid WFS (8(f) f4) on this workloads.PYRAMIDS entry instead of the SH path")
     ap.add_argument("--pyramid-frames", type=int, default=32)
+    ap.add_argument("--no-per-config", dest="per_config", action="store_false",
+                    help="skip the per_config section (configs 2, 3, 5 and config 4 with 3 sodium sub-layers)")
+    ap.add_argument("--per-config-steps", type=int, default=10)
     ap.add_argument("--closed-loop", action="store_true",
                     help="with --dm-modes: run the batch as sequential pure-integrator frames (shwfs_closed_loop)")
     args = ap.parse_args()

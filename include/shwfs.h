@@ -135,6 +135,13 @@ int shwfs_get_algorithm(const shwfs_handle *h, int32_t *algo);
 /* Number of kernels this handle has launched since shwfs_create (bench.py's gpu_launches). */
 int shwfs_launch_count(const shwfs_handle *h, int64_t *count);
 
+/* Name of the sensor kernel instance that the handle's most recent measurement launched, e.g.
+ * "wk_measure_kernel<10,0,0>" (n, threshold mode, extension kind) or "wkf_kernel<16,0,0,tma>": under
+ * SHWFS_ALGO_AUTO the instance is chosen per call (size of the call, alignment of the frames), so the
+ * algorithm id alone does not say what ran.  Copies at most len - 1 characters into name (HOST) and
+ * terminates it; "" before the first launch.  Errors: EINVAL.                                          */
+int shwfs_last_kernel(const shwfs_handle *h, char *name, int32_t len);
+
 /* ---- the paper's full LGS model ------------------------
  * "In the code a laser guide star WF is the results of different, 1 to 5 typically, projections of the beam
  *  on as many sub-layers of the sodium layer [...] For each sub-layer the proper phase shift in Tip Tilt and

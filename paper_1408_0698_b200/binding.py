@@ -27,7 +27,7 @@ EXPORTS = ["shwfs_create", "shwfs_measure", "shwfs_measure_host", "shwfs_destroy
            "shwfs_launch_count", "shwfs_debug_spots", "shwfs_strerror", "shwfs_last_cuda_error",
            "shwfs_version", "shwfs_set_sodium", "shwfs_set_noise", "shwfs_set_dm",
            "shwfs_measure_residual", "shwfs_reconstruct", "shwfs_closed_loop", "shwfs_host_bytes_per_frame",
-           "shwfs_measure_host_async", "shwfs_host_wait"]
+           "shwfs_measure_host_async", "shwfs_host_wait", "shwfs_last_kernel"]
 SHWFS_MAX_LAYERS = 8
 
 
@@ -80,6 +80,7 @@ def load():
     L.shwfs_set_algorithm.argtypes = [vp, i32]
     L.shwfs_get_algorithm.argtypes = [vp, C.POINTER(i32)]
     L.shwfs_launch_count.argtypes = [vp, C.POINTER(i64)]
+    L.shwfs_last_kernel.argtypes = [vp, C.c_char_p, i32]
     L.shwfs_debug_spots.argtypes = [vp, vp, i32, i32, vp, vp]
     L.shwfs_strerror.argtypes = [C.c_int]
     L.shwfs_strerror.restype = C.c_char_p
@@ -171,6 +172,14 @@ class Shwfs:
                 raise ValueError("elong_kernels must be [nsub,P,P]")
             if vy is not None and k.shape[0] != vy.shape[0]:
                 raise ValueError("elong_kernels and valid_yx disagree on nsub")
+            if vy is None and amp.shape[0] == n_sub_side * n_pix:
+                # the library reads nsub * P * P floats from this buffer before it can report nsub: count the valid
+                # subapertures of the rule (include/shwfs.h: mean amplitude of the patch >= min_illum, in double)
+                # first, so that too few kernels raise here instead of being read past their end
+                lit = amp.astype(np.float64).reshape(n_sub_side, n_pix, n_sub_side, n_pix).sum(axis=(1, 3))
+                expect = int((lit / (n_pix * n_pix) >= np.float64(np.float32(min_illum))).sum())
+                if k.shape[0] != expect:
+                    raise ValueError(f"elong_kernels has {k.shape[0]} entries, the valid list {expect}")
             kptr = k.ctypes.data_as(C.c_void_p)
         self._h = None
         self._h = shwfs_create(g, lambda_m, pad, bin, kptr)
@@ -210,6 +219,13 @@ class Shwfs:
         v = C.c_int64()
         _check(load().shwfs_launch_count(self._h, C.byref(v)), "shwfs_launch_count")
         return v.value
+
+    @property
+    def last_kernel(self) -> str:
+        """Name of the kernel instance the most recent measurement launched (shwfs_last_kernel)."""
+        buf = C.create_string_buffer(96)
+        _check(load().shwfs_last_kernel(self._h, buf, 96), "shwfs_last_kernel")
+        return buf.value.decode()
 
     @property
     def host_bytes_per_frame(self) -> int:

@@ -225,6 +225,7 @@ int shwfs_create(const shwfs_geometry *g, float lambda_m, int32_t pad, int32_t b
     CU_TRY(cudaGetDevice(&h->device), "cudaGetDevice");
     CU_TRY(cudaDeviceGetAttribute(&h->sms, cudaDevAttrMultiProcessorCount, h->device), "cudaDeviceGetAttribute");
     h->no_tma = getenv("SHWFS_NO_TMA") != nullptr;
+    h->force_persistent = getenv("SHWFS_FORCE_PERSISTENT") != nullptr;
     if (!shwfs_wk_supported(h, 0) && !shwfs_wk_supported(h, 1) && !shwfs_literal_supported(h) && !shwfs_pruned_fft_supported(h)) { rc = SHWFS_EUNSUPPORTED; goto fail; }
     h->algo = pick_auto(h);
     h->algo_explicit = 0;
@@ -341,6 +342,13 @@ int shwfs_launch_count(const shwfs_handle *h, int64_t *count)
 {
     if (!h || !count) return SHWFS_EINVAL;
     *count = h->launches;
+    return SHWFS_OK;
+}
+
+int shwfs_last_kernel(const shwfs_handle *h, char *name, int32_t len)
+{
+    if (!h || !name || len <= 0) return SHWFS_EINVAL;
+    snprintf(name, (size_t)len, "%s", h->last_kernel ? h->last_kernel : "");
     return SHWFS_OK;
 }
 

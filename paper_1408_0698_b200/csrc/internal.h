@@ -28,6 +28,7 @@ struct shwfs_handle {
     int sms;               /* multiprocessors of `device` (grid sizing, per-call instance choice)              */
     int dm_fp32;           /* SHWFS_DM_FP32 was set when shwfs_set_dm ran: keep the FP32 SIMT GEMM for batches    */
     int64_t launches;
+    const char *last_kernel;   /* name of the sensor kernel instance of the most recent launch (static storage) */
 
     /* device tables (owned) */
     float  *d_amp;         /* [N*N] amplitude mask                                             */
@@ -35,6 +36,8 @@ struct shwfs_handle {
     int2   *d_patch;       /* [nsub] (x = sx*n | SHWFS_PATCH_LIT, y = sy*n): patch origin in pixels; the flag says
                               every amplitude of the patch is exactly 1 (the kernel then reads no amplitude) */
     int    *d_sched;       /* [2] chunk counters of the persistent kernels' dynamic sweep (sweep.cuh), zero between launches */
+    int     force_persistent; /* SHWFS_FORCE_PERSISTENT was set at create: the persistent TMA instances whatever the call size
+                                 (sanitizer runs on small inputs, tests/sanitizer_workloads.py) */
     int     no_tma;        /* SHWFS_NO_TMA was set at create: register-gather instances only (A/B runs)   */
     float  *d_kernels;     /* [nsub*P*P] spatial elongation kernels (kept for lazy tables)     */
     float2 *d_wk_table;    /* lag-domain table M: [nsub][2n-1][n] (or [1][2n-1][n] w/o kernels) */

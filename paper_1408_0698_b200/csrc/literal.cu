@@ -302,6 +302,7 @@ cudaError_t shwfs_literal_launch(shwfs_handle *h, const float *phase, int T, flo
     if (A.total == 0) return cudaSuccess;
     if (h->has_kernels && !h->d_khat) return cudaErrorInvalidValue;
     h->launches += 1;
+    h->last_kernel = h->P == 8 ? "literal_kernel<8>" : h->P == 16 ? "literal_kernel<16>" : h->P == 32 ? "literal_kernel<32>" : "literal_kernel<64>";
     switch (h->P) {
     case 8: return launch_literal_p<8>(A, st);
     case 16: return launch_literal_p<16>(A, st);

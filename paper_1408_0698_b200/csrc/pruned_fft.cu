@@ -31,6 +31,7 @@
  * computed from it before the tile it belongs to: in the round-1 kernel the offset arithmetic sat right
  * behind the lookup and held 18 % of all stall samples (profiles/r02_pf32_tma.md).
  */
+#include <stdio.h>
 #include <string.h>
 
 #include "internal.h"
@@ -288,6 +289,9 @@ cudaError_t launch_pf_inst(shwfs_handle *h, const PfArgs &A, const CUtensorMap &
         if (dev >= 0 && dev < 64) resident[dev] = h->sms * (per_sm > 0 ? per_sm : 1);
         attr.mark(dev);
     }
+    static char name[64];
+    if (!name[0]) snprintf(name, sizeof(name), "pruned_fft_kernel<%d,%d,%d,%s>", P, NZ, MODE, TMA ? "tma" : "ldg");
+    h->last_kernel = name;
     const int need = (A.total + PF_SPOTS - 1) / PF_SPOTS;
     const int res = (dev >= 0 && dev < 64 && resident[dev] > 0) ? resident[dev] : h->sms;
     const int grid = need < res ? need : res;

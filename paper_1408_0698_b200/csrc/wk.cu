@@ -19,6 +19,8 @@
  * MACs instead of three P x P transforms, and needs a D x D rather than P x P final transform.
  * DESIGN.md section 6 has the derivation, the thread mapping and the flop counts.
  */
+#include <stdio.h>
+
 #include "internal.h"
 #include "fft_regs.cuh"
 #include "field.cuh"
@@ -566,9 +568,12 @@ __global__ void __launch_bounds__(GEN_THREADS) wk_generic_kernel(const WkArgs A,
 }
 
 template <int n, int MODE, int EXTK>
-cudaError_t launch_special_mode(const WkArgs &A, cudaStream_t st)
+cudaError_t launch_special_mode(shwfs_handle *h, const WkArgs &A, cudaStream_t st)
 {
     using Cfg = WkCfg<n>;
+    static char name[64];
+    if (!name[0]) snprintf(name, sizeof(name), "wk_measure_kernel<%d,%d,%d>", n, MODE, EXTK);
+    h->last_kernel = name;
     static shwfs_once_per_device attr;
     int dev;
     if (attr.pending(&dev)) {
@@ -583,13 +588,13 @@ cudaError_t launch_special_mode(const WkArgs &A, cudaStream_t st)
 }
 
 template <int n>
-cudaError_t launch_special(const WkArgs &A, cudaStream_t st)
+cudaError_t launch_special(shwfs_handle *h, const WkArgs &A, cudaStream_t st)
 {
     if (A.L > 1)
-        return A.mode == 0 ? launch_special_mode<n, 0, 2>(A, st) : launch_special_mode<n, 1, 2>(A, st);
+        return A.mode == 0 ? launch_special_mode<n, 0, 2>(h, A, st) : launch_special_mode<n, 1, 2>(h, A, st);
     if (A.L > 0 || A.flux > 0.f || A.dm_patch != nullptr)
-        return A.mode == 0 ? launch_special_mode<n, 0, 1>(A, st) : launch_special_mode<n, 1, 1>(A, st);
-    return A.mode == 0 ? launch_special_mode<n, 0, 0>(A, st) : launch_special_mode<n, 1, 0>(A, st);
+        return A.mode == 0 ? launch_special_mode<n, 0, 1>(h, A, st) : launch_special_mode<n, 1, 1>(h, A, st);
+    return A.mode == 0 ? launch_special_mode<n, 0, 0>(h, A, st) : launch_special_mode<n, 1, 0>(h, A, st);
 }
 
 }  // namespace
@@ -647,14 +652,15 @@ cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, int call
         return shwfs_wk_fft_launch(h, A, h->n, st);
     if (!generic && shwfs_wk_supported(h, 0)) {
         switch (h->n) {
-        case 8: return launch_special<8>(A, st);
-        case 10: return launch_special<10>(A, st);
-        case 16: return launch_special<16>(A, st);
+        case 8: return launch_special<8>(h, A, st);
+        case 10: return launch_special<10>(h, A, st);
+        case 16: return launch_special<16>(h, A, st);
         default: return cudaErrorInvalidValue;
         }
     }
     const int n = h->n, D = h->D, LX = 2 * n - 1;
     const size_t smem = sizeof(float2) * (size_t)(n * n + n * LX + D) + sizeof(float) * (size_t)(D * D + 3 * GEN_THREADS);
+    h->last_kernel = "wk_generic_kernel";
     wk_generic_kernel<<<A.total, GEN_THREADS, smem, st>>>(A, n, D);
     return cudaGetLastError();
 }

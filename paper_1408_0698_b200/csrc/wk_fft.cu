@@ -45,6 +45,7 @@
 #include "tma.cuh"
 #include "sweep.cuh"
 
+#include <stdio.h>
 #include <string.h>
 
 namespace {
@@ -344,6 +345,9 @@ cudaError_t launch_wkf_inst(shwfs_handle *h, const WkArgs &A, const CUtensorMap 
         if (dev >= 0 && dev < 64) resident[dev] = h->sms * (per_sm > 0 ? per_sm : 1);
         attr.mark(dev);
     }
+    static char name[64];
+    if (!name[0]) snprintf(name, sizeof(name), "wkf_kernel<%d,%d,%d,%s>", n, MODE, EXTK, TMA ? "tma" : "ldg");
+    h->last_kernel = name;
     int grid = (A.total + WF_SPOTS - 1) / WF_SPOTS;         /* one tile per CTA */
     if (TMA) {                                              /* persistent: one chunk of the sweep per warp at least */
         const int nchunks = (A.total + SWEEP_CHUNK - 1) / SWEEP_CHUNK;
@@ -362,7 +366,7 @@ cudaError_t launch_wkf_mode(shwfs_handle *h, const WkArgs &A, cudaStream_t st)
     if constexpr (n == 16 && EXTK == 0) {
         /* the persistent instance deals chunks of SWEEP_CHUNK spots dynamically: worth it from ~8 chunks per resident
          * warp (16 warps per SM) up; smaller calls spread over one-tile CTAs */
-        if (!h->no_tma && (long long)A.total >= 8LL * SWEEP_CHUNK * 16 * h->sms &&
+        if (!h->no_tma && (h->force_persistent || (long long)A.total >= 8LL * SWEEP_CHUNK * 16 * h->sms) &&
             shwfs_tma_patch_map(&map, A.phase, A.N, A.T, 16))
             return launch_wkf_inst<n, MODE, EXTK, true>(h, A, map, st);
     }
