@@ -19,7 +19,7 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "shwfs_oracle.c"
-_SRCS = [_SRC, _HERE / "shwfs_oracle_lgs.c"]
+_SRCS = [_SRC, _HERE / "shwfs_oracle_lgs.c", _HERE / "shwfs_oracle_poisson.c"]
 _LIB = _HERE / "libshwfs_oracle.so"
 _lib = None
 
@@ -89,8 +89,18 @@ def lib():
                                                _f32p, _i32p, C.c_int, C.c_double, C.c_double, _f64p, _f64p,
                                                _f64p, _f64p, C.c_double, C.c_double, C.c_double, C.c_int,
                                                C.c_void_p, C.c_double, C.c_double, C.c_uint64, _f64p, C.c_int,
-                                               C.c_void_p, C.c_int]
+                                               C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.shwfs_oracle_measure_lgs.restype = C.c_int
+        L.shwfs_oracle_poisson_uniforms.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, _f64p]
+        L.shwfs_oracle_poisson_uniforms.restype = None
+        L.shwfs_oracle_poisson_inversion.argtypes = [C.c_double, C.c_double, C.POINTER(C.c_double)]
+        L.shwfs_oracle_poisson_inversion.restype = C.c_long
+        L.shwfs_oracle_poisson_draw.argtypes = [C.c_double, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32,
+                                                C.POINTER(C.c_double)]
+        L.shwfs_oracle_poisson_draw.restype = C.c_long
+        L.shwfs_oracle_add_noise_poisson.argtypes = [_f64p, C.c_int, C.c_double, C.c_double, C.c_uint64, C.c_uint32,
+                                                     C.c_uint32, _f64p, C.c_void_p]
+        L.shwfs_oracle_add_noise_poisson.restype = None
         _lib = L
     return _lib
 
@@ -273,13 +283,46 @@ def add_noise(B, F, ron, seed, t, i):
     return out
 
 
+def poisson_uniforms(seed, t, i, p, j=0):
+    """N2: the two uniforms of pixel p of spot (t, i), attempt j."""
+    u = np.zeros(2, dtype=np.float64)
+    lib().shwfs_oracle_poisson_uniforms(int(seed), int(t), int(i), int(p), int(j), u)
+    return u
+
+
+def poisson_inversion(lam, u1):
+    """N3: (k, margin) of the sequential search on u1."""
+    m = C.c_double()
+    k = lib().shwfs_oracle_poisson_inversion(float(lam), float(u1), C.byref(m))
+    return int(k), m.value
+
+
+def poisson_draw(lam, seed, t, i, p):
+    """N1 + N3/N4: (k, margin) of pixel p of spot (t, i) at rate lam."""
+    m = C.c_double()
+    k = lib().shwfs_oracle_poisson_draw(float(lam), int(seed), int(t), int(i), int(p), C.byref(m))
+    return int(k), m.value
+
+
+def add_noise_poisson(B, F, ron, seed, t, i, want_margin=False):
+    """N1..N5 on a D x D binned image: Poisson counts at rate F*B plus ron * (the deviate of L5)."""
+    B = _c(B, np.float64)
+    out = np.zeros_like(B)
+    mg = np.zeros_like(B) if want_margin else None
+    lib().shwfs_oracle_add_noise_poisson(B, B.shape[0], float(F), float(ron), int(seed), int(t), int(i), out,
+                                         mg.ctypes.data_as(C.c_void_p) if want_margin else None)
+    return (out, mg) if want_margin else out
+
+
 def measure_lgs(phase, amplitude, valid_yx, n, P, b, dx, *, weight, defocus, tilt_x=None, tilt_y=None,
                 cx=0.0, cy=0.0, c_phi=1.0, tau=0.0, mode=0, kernels=None, flux=0.0, ron=0.0, seed=0,
-                stage=-1, nthreads=0):
+                stage=-1, nthreads=0, photon_model=0, want_margins=False):
     """L1..L6 for every frame and valid subaperture.
 
     phase [T,L,N,N] fp32, or [T,N,N] shared by the L = len(weight) sub-layers.  weight, defocus [rad/m^2],
     tilt_x, tilt_y [rad/m]: per sub-layer; (cx, cy) [m] centre of the quadratic.  flux = F (<= 0: no noise).
+    photon_model 0: Gaussian limit (L4); 1: Poisson counts + read noise (N1..N5, shwfs_oracle_poisson.c), with
+    want_margins also the per-pixel decision margins [T,nsub,D,D] of the draws.
     Returns slopes [T,nsub,2] float64, or (slopes, images[T,nsub,D,D]) for stage 2 (before noise) / 3 (after).
     """
     ph = _c(phase, np.float32)
@@ -309,10 +352,15 @@ def measure_lgs(phase, amplitude, valid_yx, n, P, b, dx, *, weight, defocus, til
         D = P // b
         images = np.zeros((T, nsub, D, D), dtype=np.float64)
         iptr = images.ctypes.data_as(C.c_void_p)
+    margins = np.ones((T, nsub, P // b, P // b), dtype=np.float64) if want_margins else None
     rc = lib().shwfs_oracle_measure_lgs(ph, T, L, int(shared), N, n, P, b, am, yx, nsub, float(c_phi), float(dx),
                                         w, de, tx, ty, float(cx), float(cy), float(tau), int(mode), kptr,
                                         float(flux), float(ron), int(seed), slopes, int(stage), iptr,
-                                        int(nthreads))
+                                        int(nthreads), int(photon_model),
+                                        margins.ctypes.data_as(C.c_void_p) if want_margins else None)
     if rc:
         raise RuntimeError(f"shwfs_oracle_measure_lgs failed with code {rc}")
-    return (slopes, images) if stage >= 0 else slopes
+    out = (slopes, images) if stage >= 0 else slopes
+    if want_margins:
+        return (*out, margins) if stage >= 0 else (out, margins)
+    return out

@@ -33,6 +33,7 @@
  *       z0 = rho1 cos(2 pi u1), z1 = rho1 sin(2 pi u1), z2 = rho2 cos(2 pi u3), z3 = rho2 sin(2 pi u3),
  *       rho1 = sqrt(-2 ln u0), rho2 = sqrt(-2 ln u2).
  *   L6  threshold + centre of gravity (O8, O9) on the noisy image.
+ *   (photon_model = 1 replaces L4 by true Poisson counts plus read noise: steps N1..N5 of shwfs_oracle_poisson.c.)
  *
  * Pins (tests/test_oracle_lgs_pins.py, -m "not gpu"): J1 one layer with w=1, a=0, g=0 equals
  * shwfs_oracle_measure; J2 the binned image is the weighted sum of single-layer binned images; J3 a tilt
@@ -61,6 +62,8 @@ void shwfs_oracle_intensity(const double *E, int P, double *I);
 int shwfs_oracle_convolve_fft(const double *I, const float *K, int P, double *C);
 void shwfs_oracle_centre(const double *C, int P, double *Sh);
 void shwfs_oracle_bin(const double *Sh, int P, int b, double *B);
+void shwfs_oracle_add_noise_poisson(const double *B, int D, double F, double ron, uint64_t seed, uint32_t t,
+                                    uint32_t i, double *counts, double *margin_out);   /* shwfs_oracle_poisson.c */
 void shwfs_oracle_threshold_cog(const double *B, int D, double tau, int mode, double *slope_xy);
 
 /* ------------------------------------------------------------------ L1
@@ -146,7 +149,7 @@ int shwfs_oracle_spot_lgs(const float *const *phase_layers, int L, const double 
                           double cy, const float *amplitude, int N, int n, int P, int b, int sy, int sx,
                           double c_phi, double dx, double tau, int mode, const float *K, double F,
                           double ron, uint64_t seed, uint32_t t, uint32_t i, double *slope_xy,
-                          double *img2, double *img3)
+                          double *img2, double *img3, int photon_model, double *margin3)
 {
     size_t PP = (size_t)P * P;
     int D = P / b;
@@ -174,7 +177,8 @@ int shwfs_oracle_spot_lgs(const float *const *phase_layers, int L, const double 
         shwfs_oracle_centre(C, P, Sh);
         shwfs_oracle_bin(Sh, P, b, B);
         if (img2) memcpy(img2, B, sizeof(double) * (size_t)D * D);
-        shwfs_oracle_add_noise(B, D, F, ron, seed, t, i, Bn);                                     /* L4, L5 */
+        if (photon_model == 1) shwfs_oracle_add_noise_poisson(B, D, F, ron, seed, t, i, Bn, margin3);    /* N1..N5 */
+        else shwfs_oracle_add_noise(B, D, F, ron, seed, t, i, Bn);                                /* L4, L5 */
         if (img3) memcpy(img3, Bn, sizeof(double) * (size_t)D * D);
         shwfs_oracle_threshold_cog(Bn, D, tau, mode, slope_xy);                                   /* L6 */
     }
@@ -191,7 +195,7 @@ int shwfs_oracle_measure_lgs(const float *phase, int T, int L, int shared_phase,
                              double dx, const double *weight, const double *defocus, const double *tilt_x,
                              const double *tilt_y, double cx, double cy, double tau, int mode,
                              const float *kernels, double F, double ron, uint64_t seed, double *slopes,
-                             int stage, double *images, int nthreads)
+                             int stage, double *images, int nthreads, int photon_model, double *margins)
 {
     if (!phase || !amplitude || !valid_yx || !slopes || !weight || !defocus || T < 0 || L < 1 || L > 64 ||
         n <= 0 || n > P || b <= 0 || P % b || N % n || (stage >= 0 && !images) || (stage >= 0 && stage < 2) ||
@@ -211,11 +215,12 @@ int shwfs_oracle_measure_lgs(const float *phase, int T, int L, int shared_phase,
         for (int l = 0; l < L; ++l)
             layers[l] = shared_phase ? phase + (size_t)t * fr : phase + ((size_t)t * L + l) * fr;
         double *im = (stage >= 0) ? images + (size_t)w * img_sz : NULL;
+        double *mg = margins ? margins + (size_t)w * img_sz : NULL;      /* [T,nsub,D,D], photon_model 1 only */
         int rc = shwfs_oracle_spot_lgs(layers, L, weight, defocus, tilt_x, tilt_y, cx, cy, amplitude, N, n, P,
                                        b, valid_yx[2 * i], valid_yx[2 * i + 1], c_phi, dx, tau, mode,
                                        kernels ? kernels + (size_t)i * P * P : NULL, F, ron, seed,
                                        (uint32_t)t, (uint32_t)i, slopes + 2 * (size_t)w,
-                                       stage == 2 ? im : NULL, stage == 3 ? im : NULL);
+                                       stage == 2 ? im : NULL, stage == 3 ? im : NULL, photon_model, mg);
         if (rc) {
 #pragma omp atomic write
             fail = 1;
