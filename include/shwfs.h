@@ -168,18 +168,24 @@ typedef struct {
 /* s == NULL returns to the single-layer sensor.  Arrays are copied.  Errors: EINVAL, EUNSUPPORTED, ENOMEM. */
 int shwfs_set_sodium(shwfs_handle *h, const shwfs_sodium *s);
 
-/* Detector noise on the binned image B before H7 (reading B4):
+/* Detector noise on the binned image B before H7.  photon_model 0 (reading B4):
  *      counts = flux * B + sqrt(max(flux * B, 0) + read_noise^2) * z,   z ~ N(0,1)
  * (photon noise in its Gaussian limit plus read noise), z from Philox4x32-10 with key = seed and counter =
  * (p/4, i, first_frame + t, 0), p = C*D + R the column-major pixel index, Box-Muller on the output pairs
- * (csrc/noise.cuh).  flux = photo-electrons per unit of B (a fully lit subaperture of unit amplitude and
+ * (csrc/noise.cuh).  photon_model 1 (reading B4'): true photon statistics,
+ *      counts = k + read_noise * z,   k ~ Poisson(max(flux * B, 0)),
+ * k drawn from the uniforms of the blocks with counter = (p/2, i, first_frame + t, 1 + attempt) by inversion for
+ * rates under 30 and by the transformed-rejection method PTRS (Hoermann 1993) above; z as in model 0.
+ * flux = photo-electrons per unit of B (a fully lit subaperture of unit amplitude and
  * unit weights has sum B = n^2 sum K).  nz == NULL or flux <= 0 switches the noise off.  first_frame lets
- * successive calls continue one noise stream.  Requires the lag-domain algorithm, as shwfs_set_sodium.   */
+ * successive calls continue one noise stream.  Requires the lag-domain algorithm, as shwfs_set_sodium.
+ * Errors: EINVAL (negative or non-finite read_noise, photon_model not 0 or 1), EUNSUPPORTED.                 */
 typedef struct {
   float    flux;
   float    read_noise;      /* electrons rms, >= 0 */
   uint64_t seed;
   uint32_t first_frame;
+  int32_t  photon_model;    /* 0: Gaussian limit of the photon noise; 1: Poisson counts */
 } shwfs_noise;
 int shwfs_set_noise(shwfs_handle *h, const shwfs_noise *nz);
 

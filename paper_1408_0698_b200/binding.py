@@ -48,7 +48,8 @@ class ShwfsSodium(C.Structure):
 
 class ShwfsNoise(C.Structure):
     """struct shwfs_noise of include/shwfs.h."""
-    _fields_ = [("flux", C.c_float), ("read_noise", C.c_float), ("seed", C.c_uint64), ("first_frame", C.c_uint32)]
+    _fields_ = [("flux", C.c_float), ("read_noise", C.c_float), ("seed", C.c_uint64), ("first_frame", C.c_uint32),
+                ("photon_model", C.c_int32)]
 
 
 class ShwfsError(RuntimeError):
@@ -262,9 +263,11 @@ class Shwfs:
         _check(load().shwfs_set_sodium(self._h, C.byref(sd)), "shwfs_set_sodium")
         self._layers = 1 if shared_phase else int(w.shape[0])
 
-    def set_noise(self, flux: float = 0.0, read_noise: float = 0.0, seed: int = 0, first_frame: int = 0):
-        """Detector noise before the centroid (flux <= 0 switches it off)."""
-        nz = ShwfsNoise(float(flux), float(read_noise), int(seed), int(first_frame))
+    def set_noise(self, flux: float = 0.0, read_noise: float = 0.0, seed: int = 0, first_frame: int = 0,
+                  photon_model: int = 0):
+        """Detector noise before the centroid (flux <= 0 switches it off).  photon_model 0: Gaussian limit of the
+        photon noise, 1: Poisson counts (include/shwfs.h)."""
+        nz = ShwfsNoise(float(flux), float(read_noise), int(seed), int(first_frame), int(photon_model))
         _check(load().shwfs_set_noise(self._h, C.byref(nz)), "shwfs_set_noise")
 
     # -- closed-loop neighbours (include/shwfs.h: shwfs_set_dm, shwfs_measure_residual, shwfs_reconstruct,

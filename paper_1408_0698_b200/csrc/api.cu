@@ -414,8 +414,10 @@ int shwfs_set_noise(shwfs_handle *h, const shwfs_noise *nz)
     if (!h) return SHWFS_EINVAL;
     if (!nz || !(nz->flux > 0.f)) { h->nz_flux = 0.f; return SHWFS_OK; }
     if (!isfinite(nz->flux) || !(nz->read_noise >= 0.f) || !isfinite(nz->read_noise)) return SHWFS_EINVAL;
+    if (nz->photon_model != 0 && nz->photon_model != 1) return SHWFS_EINVAL;
     if (!shwfs_wk_supported(h, 0) && !shwfs_wk_supported(h, 1)) return SHWFS_EUNSUPPORTED;
     h->nz_flux = nz->flux; h->nz_ron = nz->read_noise; h->nz_seed = nz->seed; h->nz_first_frame = nz->first_frame;
+    h->nz_model = nz->photon_model;
     return SHWFS_OK;
 }
 

@@ -50,6 +50,7 @@ struct shwfs_handle {
     float   sod_sw[SHWFS_MAX_LAYERS];   /* sqrt(w_l) */
     float2 *d_sod_g;                    /* [L][nsub] (2 a_l (r_i - r_c) + g_l) dx / 2pi, turns/pixel */
     float   nz_flux, nz_ron;
+    int     nz_model;                   /* shwfs_noise.photon_model */
     uint64_t nz_seed;
     uint32_t nz_first_frame;
 

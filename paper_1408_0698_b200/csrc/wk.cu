@@ -424,7 +424,7 @@ __global__ void __launch_bounds__(WkCfg<n>::THREADS, WkSmem<n, (EXTK < 2)>::MIN_
                 for (int R = 0; R < 16; ++R) A.binned[(o * 16 + R) * 16 + C] = bcol[R];
             }
             if (EXT && A.flux > 0.f) {
-                add_noise_col16(bcol, C, A.key, A.t0 + (unsigned)inf.y, (unsigned)max(inf.z, 0), A.flux, A.ron2);
+                add_noise_col16(bcol, C, A.key, A.t0 + (unsigned)inf.y, (unsigned)max(inf.z, 0), A.flux, A.ron2, A.photon_model);
                 if (inf.z >= 0 && A.noisy) {
 #pragma unroll
                     for (int R = 0; R < 16; ++R) A.noisy[(o * 16 + R) * 16 + C] = bcol[R];
@@ -522,7 +522,12 @@ __global__ void __launch_bounds__(GEN_THREADS) wk_generic_kernel(const WkArgs A,
             const int R = px / D, C = px - R * D, p = C * D + R;
             float z[4];
             normal4(A.key, A.t0 + (unsigned)t, (unsigned)i, (unsigned)(p >> 2), z);
-            B[px] = noisy_count(B[px], A.flux, A.ron2, z[p & 3]);
+            if (A.photon_model == 1) {
+                const uint4 x = philox4x32_10(make_uint4((unsigned)(p >> 1), (unsigned)i, A.t0 + (unsigned)t, 1u), A.key);
+                B[px] = fmaf(sqrtf(A.ron2), z[p & 3], poisson_count(B[px], A.flux, x, A.key, A.t0 + (unsigned)t, (unsigned)i, (unsigned)p));
+            } else {
+                B[px] = noisy_count(B[px], A.flux, A.ron2, z[p & 3]);
+            }
             if (A.noisy) A.noisy[o * D * D + px] = B[px];
         }
         __syncthreads();
@@ -628,7 +633,7 @@ cudaError_t shwfs_wk_launch(shwfs_handle *h, const float *phase, int T, int call
     A.sod_g = h->d_sod_g; A.noisy = noisy; A.layer_stride = 0; A.L = h->sod_L;
     for (int l = 0; l < SHWFS_MAX_LAYERS; ++l) { A.sod_q[l] = h->sod_q[l]; A.sod_sw[l] = h->sod_sw[l]; }
     if (h->sod_L > 0 && !h->sod_shared) { A.layer_stride = A.frame_stride; A.frame_stride *= h->sod_L; }
-    A.flux = h->nz_flux; A.ron2 = h->nz_ron * h->nz_ron;
+    A.flux = h->nz_flux; A.ron2 = h->nz_ron * h->nz_ron; A.photon_model = h->nz_model;
     A.key = make_uint2((unsigned)h->nz_seed, (unsigned)(h->nz_seed >> 32));
     A.t0 = h->nz_first_frame + t_base;
     A.dm_patch = dm_patch;

@@ -29,6 +29,7 @@ struct WkArgs {
     float sod_q[SHWFS_MAX_LAYERS];   /* curvature a_l dx^2 / 2pi, turns/pixel^2                             */
     float sod_sw[SHWFS_MAX_LAYERS];  /* sqrt(w_l): folded into the amplitude                                */
     float flux, ron2;
+    int photon_model;            /* 0 Gaussian limit of the photon noise, 1 Poisson counts (noise.cuh) */
     uint2 key;
     unsigned t0;
     /* closed-loop neighbour (EXT instances only): residual = wavefront - DM phase.  The DM

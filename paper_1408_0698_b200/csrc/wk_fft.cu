@@ -307,7 +307,7 @@ __global__ void __launch_bounds__(WF_THREADS, EXTK == 2 ? 3 : 4) wkf_kernel(cons
             for (int R = 0; R < 16; ++R) A.binned[(o * 16 + R) * 16 + C] = bcol[R];
         }
         if (EXT && A.flux > 0.f) {
-            add_noise_col16(bcol, C, A.key, A.t0 + (unsigned)t, (unsigned)i, A.flux, A.ron2);
+            add_noise_col16(bcol, C, A.key, A.t0 + (unsigned)t, (unsigned)i, A.flux, A.ron2, A.photon_model);
             if (live && A.noisy) {
 #pragma unroll
                 for (int R = 0; R < 16; ++R) A.noisy[(o * 16 + R) * 16 + C] = bcol[R];

@@ -40,7 +40,7 @@ def _check_guards(buf, n):
 
 
 CASES = [  # (config, every n-th subaperture, frames, algorithm name, force the persistent instances)
-    (1, 1, 4, "ALGO_WK", False), (1, 1, 4, "ALGO_WK_FFT", False), (1, 1, 4, "ALGO_LITERAL", False),
+    (1, 1, 4, "ALGO_WK", False), (1, 1, 4, "ALGO_AUTO", False), (1, 1, 4, "ALGO_LITERAL", False),
     (2, 3, 5, "ALGO_PRUNED_FFT", False), (2, 3, 5, "ALGO_WK", False),
     (3, 4, 37, "ALGO_WK", False), (3, 4, 3, "ALGO_AUTO", False), (3, 40, 3, "ALGO_WK_GENERIC", False),
     (5, 4, 9, "ALGO_WK_FFT", True), (5, 4, 9, "ALGO_WK_FFT", False),

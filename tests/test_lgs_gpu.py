@@ -236,3 +236,81 @@ def test_sodium_and_noise_argument_checking(gpu):
         with pytest.raises(B.ShwfsError) as e:
             s.set_noise(10.0, 1.0)
         assert e.value.code == B.SHWFS_EUNSUPPORTED
+
+
+# margin below which a Poisson draw may legitimately come out differently in fp32.  The device's rate F*B differs
+# from the oracle's by ~2e-6 of the spot's peak rate (the measured image error; the tolerance is 1e-4), i.e. by
+# d = 2e-6 x rate at the bright pixels.  In the inversion branch that moves every CDF value by at most d x pmf
+# < 1e-5; in the rejection branch it moves the argument of the floor by d itself.  Clear = decided by more than
+# 1e-4 + 1e-5 x rate (five times the measured error; the fp32 search itself adds ~1e-6).
+def _poisson_clear(margin, rate):
+    return margin > 1e-4 + 1e-5 * rate
+
+
+@pytest.mark.parametrize("flux_total,ron", [(300.0, 0.0), (300.0, 3.0), (40000.0, 2.0)])
+def test_config3_poisson_noise_matches_oracle(gpu, oracle, flux_total, ron):
+    """photon_model = 1 (SURVEY.md 8(f) f2 as written: Poisson photon noise + Gaussian read noise).  The counts
+    are integers decided by floating-point comparisons, so the statement is the one of the hard-mask threshold
+    test: on every pixel whose draw was decided by a margin larger than rounding (_poisson_clear; the oracle
+    reports the margin of each draw) the device count equals the oracle's exactly (with read noise: to 1e-4 of the peak);
+    on spots whose 256 pixels are all clear the slopes agree to 1e-3 px; the remaining pixels differ by at most
+    one count (inversion, rate < 30) or stay within 8 sigma of the rate (rejection branch, where a flipped
+    acceptance moves on to the next attempt).  300 e-/subaperture exercises the inversion branch, 40000 the
+    transformed rejection."""
+    torch, B = gpu
+    c = W.CONFIGS[3]
+    amp = W.pupil_mask(c)
+    T = 2
+    ph = W.phase_frames(c, 0, range(T))
+    yx = oracle.valid_list(amp, c.n, c.min_illum)[::3].copy()
+    K = W.elongation_kernels(c, 0, yx)
+    F, seed = flux_total / c.n ** 2, 0x14080698000000A7
+    kw = dict(weight=[1.0], defocus=[0.0], tau=c.tau, kernels=K, flux=F, ron=ron, seed=seed, photon_model=1)
+    want, wimg, margin = oracle.measure_lgs(ph, amp, yx, c.n, c.P, c.b, c.dx, stage=3, want_margins=True, **kw)
+    _, clean_img = oracle.measure_lgs(ph, amp, yx, c.n, c.P, c.b, c.dx, weight=[1.0], defocus=[0.0], tau=c.tau,
+                                      kernels=K, stage=2)
+    rate = np.maximum(F * clean_img, 0.0)
+    assert (rate >= 30).any() == (flux_total > 1000)                  # which branch the case exercises
+    clear = _poisson_clear(margin, rate)
+    bright = flux_total > 1000            # rates of thousands: the clearance 1e-5 x rate is a few percent of a count
+    assert clear.mean() > (0.95 if bright else 0.99), clear.mean()
+    spot_clear = clear.all(axis=(2, 3))
+    assert bright or spot_clear.mean() > 0.3, spot_clear.mean()
+    with B.from_config(c, 0, kernels=K, valid_yx=yx) as s:
+        s.set_noise(F, ron, seed, photon_model=1)
+        phd = torch.from_numpy(ph).cuda()
+        for a in _wk_algos(s, B):
+            s.algorithm = a
+            got = s.measure(phd).cpu().numpy()
+            img = s.debug_spots(phd, 3).cpu().numpy().astype(np.float64)
+            d = np.abs(img - wimg)
+            if ron == 0.0:
+                assert np.all(img == np.round(img)) and img.min() >= 0
+                assert np.all(d[clear] == 0.0), (a, d[clear].max(), int((d[clear] > 0).sum()))
+            else:
+                pk = wimg.max(axis=(2, 3), keepdims=True)
+                assert (d / pk)[clear].max() <= IMAGE_TOL, (a, (d / pk)[clear].max())
+            low = ~clear & (rate < 29.9)
+            assert d[low].max(initial=0.0) <= 1.0 + 1e-3, (a, d[low].max())
+            high = ~clear & (rate >= 29.9)
+            assert np.all(d[high] <= 8.0 * np.sqrt(rate[high]) + 2.0)
+            # slopes: wherever the noisy image is the oracle's (every all-clear spot, and every other spot whose
+            # unclear draws happened to fall the same way), the centroid is the oracle's
+            same = (d <= (1e-6 if ron == 0.0 else IMAGE_TOL * wimg.max(axis=(2, 3), keepdims=True))).all(axis=(2, 3))
+            assert np.all(same[spot_clear]) and same.mean() > (0.05 if bright else 0.3), same.mean()
+            assert np.abs(got - want)[same].max() <= SLOPE_TOL, (a, np.abs(got - want)[same].max())
+            # elsewhere a handful of +-1 counts moves it by (lever arm / photo-electrons) each
+            assert np.abs(got - want).max() <= (0.02 if bright else 0.5)
+            # and the unclear pixels are as rare on the device as the margins say: no systematic disagreement
+            assert (d > 0.5).mean() <= 2.0 * (~clear).mean() + 1e-4
+        # the two models draw from one seed but are different noise; model 0 is unchanged by the new field
+        s.algorithm = B.ALGO_WK
+        s.set_noise(F, max(ron, 1.0), seed, photon_model=0)
+        g0 = s.measure(phd).cpu().numpy()
+        w0 = oracle.measure_lgs(ph, amp, yx, c.n, c.P, c.b, c.dx, weight=[1.0], defocus=[0.0], tau=c.tau, kernels=K,
+                                flux=F, ron=max(ron, 1.0), seed=seed)
+        assert np.abs(g0 - w0).max() <= SLOPE_TOL
+    with B.from_config(c, 0, kernels=K, valid_yx=yx) as s:
+        nz = B.ShwfsNoise(1.0, 1.0, 1, 0, 2)
+        import ctypes
+        assert B.load().shwfs_set_noise(s._h, ctypes.byref(nz)) == B.SHWFS_EINVAL
