@@ -25,6 +25,7 @@
 #include <string.h>
 
 #include <new>
+#include <type_traits>
 
 #include "internal.h"
 #include "fft_regs.cuh"
@@ -70,27 +71,58 @@ __device__ __forceinline__ float2 cmul2(float2 a, float2 w)
     return __ffma2_rn(bc2(a.y), rot_pi2(w), __fmul2_rn(bc2(a.x), w));
 }
 
+/* All products W0 * g^q, q = 0 .. 2^BITS - 1, from the BITS table values pw[b] = g^(2^b): a depth-first walk over
+ * the binary expansions of q, one complex product per q and no product more than BITS deep (the rounding of a
+ * q-fold recurrence would be q deep), a handful of registers live.  emit(q, w) is called once per q with q a
+ * compile-time constant.  Replaces one table lookup per q: at 32 lookups per thread and line with addresses
+ * scattered over the table, the L1 data pipe of pyr_cols_kernel ran at 80 % of its wavefront peak and
+ * long_scoreboard was its first stall (profiles/r02_pyramid.md). */
+template <int BITS>
+struct PowWalk {
+    template <int Q, int B, typename F>
+    __device__ __forceinline__ static void node(float2 w, const float2 (&pw)[BITS], F &emit)
+    {
+        emit(std::integral_constant<int, Q>(), w);
+        if constexpr (B >= 0) below<Q, B>(w, pw, emit);
+    }
+    /* children of Q: set one more bit among bits B .. 0 */
+    template <int Q, int B, typename F>
+    __device__ __forceinline__ static void below(float2 w, const float2 (&pw)[BITS], F &emit)
+    {
+        node<Q + (1 << B), B - 1>(cmul2(w, pw[B]), pw, emit);
+        if constexpr (B > 0) below<Q, B - 1>(w, pw, emit);
+    }
+    template <typename F>
+    __device__ __forceinline__ static void run(float2 w0, const float2 (&pw)[BITS], F emit)
+    {
+        node<0, BITS - 1>(w0, pw, emit);
+    }
+};
+
 /* One L = R*R point transform of the line owned by the R threads j = 0..R-1 (all in one warp), on packed
  * (re, im) registers with FP32x2 butterflies (fft_fma2).
  * In : z[m] = x[j + R m] (natural order; entries m >= NZ are zero).
  * Out: z[q] = X[p + R q], p = this thread's index (natural order).
- * X[k] = sum_x x[x] exp(SIGN 2 pi i x k / L).  `line` is this line's R*(R+2) float2 of shared memory.      */
+ * X[k] = sum_x x[x] exp(SIGN 2 pi i x k / L).  `line` is this line's R*(R+2) float2 of shared memory.
+ * The twiddles w_L^(j p), p = 0..R-1, are the powers of w_L^j: log2 R table reads and a PowWalk.            */
 template <int R, int SIGN, int NZ>
 __device__ __forceinline__ void line_fft(float2 (&z)[R], int j, float2 *__restrict__ line,
                                          const float2 *__restrict__ tw)
 {
-    constexpr int L = R * R;
+    constexpr int L = R * R, BITS = ilog2(R);
     fft_fma2<R, SIGN, NZ>(z);
+    float2 pw[BITS];
 #pragma unroll
-    for (int p = 0; p < R; ++p) {
-        float2 a = z[fft_out_index<R>(p)];
-        if (p > 0) {
-            float2 w = __ldg(tw + ((j * p) & (L - 1)));                 /* w_L^(j p), conjugated for SIGN < 0 */
-            if (SIGN < 0) w.y = -w.y;
-            a = cmul2(a, w);
-        }
-        line[p * (R + 2) + j] = a;
+    for (int b = 0; b < BITS; ++b) {
+        pw[b] = __ldg(tw + ((j << b) & (L - 1)));                       /* w_L^(j 2^b), conjugated for SIGN < 0 */
+        if (SIGN < 0) pw[b].y = -pw[b].y;
     }
+    PowWalk<BITS>::run(make_float2(1.f, 0.f), pw, [&](auto pc, float2 w) {
+        constexpr int p = decltype(pc)::value;
+        float2 a = z[fft_out_index<R>(p)];
+        if (p > 0) a = cmul2(a, w);
+        line[p * (R + 2) + j] = a;
+    });
     __syncwarp();
 #pragma unroll
     for (int jj = 0; jj < R; jj += 2) {                                 /* this thread is now p = j */
@@ -184,14 +216,23 @@ __global__ void __launch_bounds__(PY_LINES * R, 2) pyr_cols_kernel(const PyArgs 
     }
     float2 *line = py_smem + b * R * (R + 2);
     line_fft<R, -1, NZ>(z, j, line, A.tw);
-    /* Q3: exp(-2 pi i s (|u~| + |v~|) / Np) at v = j + R q */
-    const int ua = u < L / 2 ? u : L - u;
+    /* Q3: exp(-2 pi i s (|u~| + |v~|) / Np) at v = j + R q.  |v~| = v for q < R/2 and L - v above, so the phase
+     * index runs s (ua + j) + (R s) q over the lower half of q and s (ua - j) - (R s) q over the upper one: two
+     * table reads for the ends and a PowWalk over the powers of w^(R s) for each half. */
+    {
+        constexpr int HB = ilog2(R) - 1, H = R / 2;
+        const int ua = u < L / 2 ? u : L - u;
+        float2 st[HB], stc[HB];
 #pragma unroll
-    for (int q = 0; q < R; ++q) {
-        const int v = j + R * q, va = v < L / 2 ? v : L - v;
-        float2 w = __ldg(A.tw + ((A.s * (ua + va)) & (L - 1)));
-        w.y = -w.y;                                           /* times conj(w) */
-        z[q] = cmul2(z[q], w);
+        for (int b = 0; b < HB; ++b) {
+            st[b] = __ldg(A.tw + ((A.s * R << b) & (L - 1)));           /* w^(R s 2^b) */
+            stc[b] = make_float2(st[b].x, -st[b].y);
+        }
+        float2 lo = __ldg(A.tw + ((A.s * (ua + j)) & (L - 1)));                     /* q = 0   */
+        float2 hi = __ldg(A.tw + ((A.s * (ua - j) - A.s * R * H) & (L - 1)));        /* q = R/2 */
+        lo.y = -lo.y; hi.y = -hi.y;                                     /* the mask is the conjugate */
+        PowWalk<HB>::run(lo, stc, [&](auto qc, float2 w) { constexpr int q = decltype(qc)::value; z[q] = cmul2(z[q], w); });
+        PowWalk<HB>::run(hi, st, [&](auto qc, float2 w) { constexpr int q = decltype(qc)::value; z[H + q] = cmul2(z[H + q], w); });
     }
     line_fft<R, +1, R>(z, j, line, A.tw);
     __syncthreads();
