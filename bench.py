@@ -46,11 +46,17 @@ NCU_JSON = ROOT / "profiles" / "ncu_constants.json"
 
 
 def sources_sha1(paths):
-    """sha1 over the named source files (relative to the repo root), in the order given."""
+    """sha1 over the CODE of the named source files (relative to the repo root), in the order given: C comments
+    and white space are dropped first, so that rewording a comment does not disown a capture but any change a
+    compiler could see does."""
     import hashlib
+    import re
     h = hashlib.sha1()
     for rel in paths:
-        h.update(rel.encode() + b"\0" + (ROOT / rel).read_bytes())
+        text = (ROOT / rel).read_text()
+        text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)
+        text = re.sub(r"//[^\n]*", " ", text)
+        h.update(rel.encode() + b"\0" + "".join(text.split()).encode())
     return h.hexdigest()
 
 
@@ -496,6 +502,7 @@ def run_pyramid(args):
         dt = time.perf_counter() - t0
         cpu = {"value": nfr / dt, "unit": "frames/s", "cores": 1, "kind": "oracle",
                "sample": f"{nfr} frame(s), numpy fft2 oracle, {dt:.1f} s"}
+    pent, pnote = ncu_constants(f"pyr_cols_kernel<{32 if p.Np == 1024 else 16}>")
     print(json.dumps({
         "metric": "pyramid_wfs_frames_per_s", "value": value, "unit": "frames/s", "n_gpus": 1, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -505,7 +512,10 @@ def run_pyramid(args):
                                f"{nvalid} valid pixels, {T}-frame batches"},
         "clocks": clocks, "e2e": None, "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                     "frac": ach / FP32_PEAK_TFLOPS, "traffic": None, "kernel": "pyr_cols_kernel (+ rows, final)",
+                     "frac": ach / FP32_PEAK_TFLOPS, "traffic": (pent or {}).get("dram_bytes_per_launch"),
+                     "traffic_note": "pyr_cols_kernel, one 16-frame chunk per launch; " + pnote,
+                     "fma_pipe_active_ncu": (pent or {}).get("fma_pipe_active"),
+                     "kernel": "pyr_cols_kernel (+ rows, final)",
                      "flops_per_frame": flops, "flops_basis": "5 L log2 L per line of the pruned passes (DESIGN.md 14)"},
         "cpu_baseline": cpu}))
 

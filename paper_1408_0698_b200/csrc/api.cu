@@ -93,6 +93,10 @@ int ensure_khat(shwfs_handle *h)
 
 }  // namespace
 
+#ifndef SHWFS_TMA_L2PROMO
+#define SHWFS_TMA_L2PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+#endif
+
 /* tma.cuh: the driver's encoder is fetched through the runtime, so the library links against cudart only */
 bool shwfs_tma_patch_map(CUtensorMap *out, const float *base, int N, long long frames, int n)
 {
@@ -119,7 +123,7 @@ bool shwfs_tma_patch_map(CUtensorMap *out, const float *base, int N, long long f
     const cuuint32_t one[3] = {1, 1, 1};
     const CUtensorMapSwizzle sw = n == 16 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE;
     return encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float *>(base), dim, stride, box, one,
-                  CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, sw, SHWFS_TMA_L2PROMO,
                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 

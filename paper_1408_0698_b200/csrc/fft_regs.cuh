@@ -116,7 +116,7 @@ __host__ __device__ constexpr int fft_out_index(int k) { return bitrev(k, ilog2(
  * A general butterfly is 3 instructions instead of 6, a trivial one (w = 1, +-i) 2 FADD2 instead of 4 FADD:
  * 194 instructions at L = 32 (162 pruned to 16 inputs) against 388 (324).  The FMA pipe does the same work
  * (an FP32x2 instruction occupies it for two cycles); what is halved is the issue slots, which is what
- * bounded the line transforms (profiles/r02_pf32_tma.md: issue 76 %, FMA pipe 59 %).  Arithmetic and
+ * bounded the line transforms (profiles/r02_pf32.md: issue 76 %, FMA pipe 59 %).  Arithmetic and
  * rounding are those of fft_fma, element for element.
  * ------------------------------------------------------------------------------------------------------- */
 __device__ __forceinline__ float2 rot_pi2(float2 b) { return make_float2(-b.y, b.x); }     /* +i b */

@@ -6,12 +6,12 @@
  * Steps H1 gather, H2 field, H3 zero-padded P x P DFT, H4 |.|^2/P^2, H6 centre + b x b bin, H7 threshold,
  * H8 centre of gravity of include/shwfs.h, D = P/b = 16 detector pixels per side.
  *
- * Thread mapping: 16 threads (a half-warp) per spot, 8 spots per tile, persistent CTAs each taking a contiguous
- * run of tiles (sweep.cuh), no CTA-wide barrier (a half-warp never waits for another).
+ * Thread mapping: 16 threads (a half-warp) per spot, two spots per warp and step, persistent warps striding over
+ * the spot pairs (sweep.cuh, strided deal), no CTA-wide barrier (a half-warp never waits for another).
  *   H1           TMA instances (n = 16, 16-byte aligned frames): lane 0 of the half-warp issues ONE
  *                cp.async.bulk.tensor box (16 x 16 fp32, 64-byte swizzle) per spot into a 1 KB staging slot,
- *                completion on the half-warp's own mbarrier; the box of tile k+1 is requested as soon as the
- *                row pass of tile k has read the slot, and lands during the column pass.  The gather costs
+ *                completion on the half-warp's own mbarrier; the box of the warp's next step is requested as soon
+ *                as the row pass of this step has read the slot, and lands during the column pass.  The gather costs
  *                no registers and no L1 data-pipe wavefronts (tma.cuh).  Other sizes: thread r gathers patch
  *                row r by 8-byte loads one tile ahead, in registers.
  *                Amplitude: subapertures whose n x n amplitudes are all exactly 1 (93 % of config 2) are
@@ -27,9 +27,9 @@
  *   H7 + H8      cog16 (cog.cuh): max / sums by xor shuffles inside the half-warp; lane 0 writes 8 bytes.
  * Only the phase patch is read from and the two slopes written to HBM.
  *
- * The table lookup of a spot (the only dependent load of the gather) is issued two tiles ahead and nothing is
- * computed from it before the tile it belongs to: in the round-1 kernel the offset arithmetic sat right
- * behind the lookup and held 18 % of all stall samples (profiles/r02_pf32_tma.md).
+ * The table lookup of a spot (the only dependent load of the gather) is issued a step ahead and nothing is
+ * computed from it before the step it belongs to: in the round-1 kernel the offset arithmetic sat right
+ * behind the lookup and held 18 % of all stall samples (profiles/r02_pf32.md).
  */
 #include <stdio.h>
 #include <string.h>

@@ -4,7 +4,7 @@
  * phase[T][N][N], copied global -> shared memory by cp.async.bulk.tensor and signalled on an mbarrier.
  * BASELINE.json:north_star: "float4/TMA-staged loads of the phase patches".
  *
- * Why it matters here (profiles/r02_pf32_tma.md): with one thread per patch row the per-thread vector loads
+ * Why it matters here (profiles/r02_pf32.md): with one thread per patch row the per-thread vector loads
  * of a 16 x 16 patch touch 32 different 128-byte lines per warp instruction; the L1 data pipe ran at 88 % of
  * its wavefront peak on config 2 and was the bound of the kernel.  A TMA box does not pass through the LSU
  * data pipe at all and needs no address registers.
