@@ -97,7 +97,8 @@ int shwfs_create(const shwfs_geometry *g, float lambda_m, int32_t pad, int32_t b
  * slopes[t][i][0] = x-slope, [1] = y-slope, in binned detector pixels about the detector centre;
  * i indexes the valid list.  Positive x-slope <=> phase increasing with x (the column index).
  * T == 0 is a successful no-op.  Non-finite phase values are not checked: they reach only that spot's
- * slopes.  Errors: EINVAL (null h, null pointers with T > 0, T < 0), ECUDA (launch failure).           */
+ * slopes.  Errors: EINVAL (null h, null pointers with T > 0, T < 0, phase_dev not 16-byte aligned, another
+ * device current), ECUDA (launch failure).                                                               */
 int shwfs_measure(shwfs_handle *h, const float *phase_dev, int32_t T, float *slopes_dev,
                   void *cuda_stream);
 

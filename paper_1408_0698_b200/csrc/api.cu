@@ -475,6 +475,9 @@ static bool on_device(const shwfs_handle *h)
     return cudaGetDevice(&dev) == cudaSuccess && dev == h->device;
 }
 
+/* include/shwfs.h: frames are 16-byte aligned (vector loads and TMA boxes start on their first pixel) */
+static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
 static bool ext_on(const shwfs_handle *h) { return h->sod_L > 0 || h->nz_flux > 0.f; }
 
 /* frames of phase per time step t: L when every sub-layer has its own wavefront */
@@ -515,7 +518,7 @@ int shwfs_measure(shwfs_handle *h, const float *phase_dev, int32_t T, float *slo
 {
     if (!h || T < 0) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
-    if (!phase_dev || !slopes_dev || !on_device(h)) return SHWFS_EINVAL;
+    if (!phase_dev || !slopes_dev || !on_device(h) || !aligned16(phase_dev)) return SHWFS_EINVAL;
     return run_path(h, phase_dev, T, T, slopes_dev, -1, nullptr, 0u, (cudaStream_t)cuda_stream);
 }
 
@@ -524,7 +527,7 @@ int shwfs_measure_residual(shwfs_handle *h, const float *phase_dev, const float 
 {
     if (!h || T < 0 || h->dm_M <= 0) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
-    if (!phase_dev || !coef_dev || !slopes_dev || !on_device(h)) return SHWFS_EINVAL;
+    if (!phase_dev || !coef_dev || !slopes_dev || !on_device(h) || !aligned16(phase_dev)) return SHWFS_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t need = (size_t)T * h->nsub * h->n * h->n;
     if (h->dm_patch_cap < need) {
@@ -568,7 +571,7 @@ int shwfs_closed_loop(shwfs_handle *h, const float *phase_dev, const float *R_de
 {
     if (!h || T < 0 || h->dm_M <= 0 || !isfinite(gain)) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
-    if (!phase_dev || !R_dev || !coef_dev || !slopes_dev || !on_device(h)) return SHWFS_EINVAL;
+    if (!phase_dev || !R_dev || !coef_dev || !slopes_dev || !on_device(h) || !aligned16(phase_dev)) return SHWFS_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t step = (size_t)h->N * h->N * frames_per_step(h);
     const int K = 2 * h->nsub;
@@ -594,7 +597,7 @@ int shwfs_debug_spots(shwfs_handle *h, const float *phase_dev, int32_t T, int32_
 {
     if (!h || T < 0 || stage < 0 || stage > 3) return SHWFS_EINVAL;
     if (T == 0) return SHWFS_OK;
-    if (!phase_dev || !out_dev || !on_device(h)) return SHWFS_EINVAL;
+    if (!phase_dev || !out_dev || !on_device(h) || !aligned16(phase_dev)) return SHWFS_EINVAL;
     /* the debug path needs somewhere to put the slopes it also computes */
     const size_t need = 2 * (size_t)T * h->nsub;
     if (h->d_slopes_cap < need) {

@@ -6,8 +6,9 @@
  * Steps H1 gather, H2 field, H3 zero-padded P x P DFT, H4 |.|^2/P^2, H6 centre + b x b bin, H7 threshold,
  * H8 centre of gravity of include/shwfs.h, D = P/b = 16 detector pixels per side.
  *
- * Thread mapping: 16 threads (a half-warp) per spot, two spots per warp and step, persistent warps striding over
- * the spot pairs (sweep.cuh, strided deal), no CTA-wide barrier (a half-warp never waits for another).
+ * Thread mapping: 16 threads (a half-warp) per spot, two spots per warp and step, persistent warps that are dealt
+ * chunks of four spots from a counter (sweep.cuh; small calls: a strided deal), no CTA-wide barrier (a half-warp
+ * never waits for another).
  *   H1           TMA instances (n = 16, 16-byte aligned frames): lane 0 of the half-warp issues ONE
  *                cp.async.bulk.tensor box (16 x 16 fp32, 64-byte swizzle) per spot into a 1 KB staging slot,
  *                completion on the half-warp's own mbarrier; the box of the warp's next step is requested as soon
@@ -48,6 +49,7 @@ using namespace shwfs;
 constexpr int PF_THREADS = 128;
 constexpr int PF_SPOTS = PF_THREADS / 16;
 constexpr int PF_SLOT = 1024;                  /* bytes of one staged 16 x 16 fp32 patch */
+constexpr int PF_CHUNK = 4;                    /* spots per chunk of the dynamic deal: two warp steps */
 
 struct PfArgs {
     const float *phase;
@@ -55,6 +57,8 @@ struct PfArgs {
     const int2 *patch;        /* [nsub] {first column of the patch | SHWFS_PATCH_LIT, first row of the patch} */
     float *slopes;
     float *binned;            /* stage-2 debug image [T*nsub*16*16] or null */
+    int *sched;               /* chunk counters of the dynamic deal (sweep.cuh) */
+    int chunk;                /* spots per chunk of the dynamic deal, 0 = strided deal */
     long long frame_stride;
     int T, N, nsub, total, n;
     float tau, turns, ramp_unit;
@@ -119,7 +123,7 @@ pruned_fft_kernel(const PfArgs A, const __grid_constant__ CUtensorMap tmap)
 
     /* persistent CTAs (sweep.cuh): the host sizes the grid to the resident CTAs of the device, so a launch has no
      * ragged last wave */
-    Sweep sw_(A.patch, nullptr, A.T, A.nsub, A.total, 0);      /* strided deal: no table, calls of any size */
+    Sweep sw_(A.patch, A.chunk ? A.sched : nullptr, A.T, A.nsub, A.total, A.chunk);      /* chunk 0: strided deal */
     auto request = [&](const Spot &s) {                   /* TMA: one box per spot, issued by the half-warp's lane 0 */
         if (r == 0 && sw_.live(s)) {
             mbar_expect_tx(bar, PF_SLOT);
@@ -295,7 +299,13 @@ cudaError_t launch_pf_inst(shwfs_handle *h, const PfArgs &A, const CUtensorMap &
     const int need = (A.total + PF_SPOTS - 1) / PF_SPOTS;
     const int res = (dev >= 0 && dev < 64 && resident[dev] > 0) ? resident[dev] : h->sms;
     const int grid = need < res ? need : res;
-    pruned_fft_kernel<P, NZ, MODE, TMA><<<grid, PF_THREADS, Cfg::SMEM, st>>>(A, map);
+    /* calls of at least four steps per resident warp: chunks of PF_CHUNK spots dealt from the handle's counter
+     * (1.15e9 against 1.09e9 spots/s on config 2: the warps of an SM do not run at the same speed and a static deal
+     * ends with 3.2 of 4 warps per scheduler resident; chunks of 2 / 8 spots: 1.09 / 1.13e9); smaller calls:
+     * strided */
+    PfArgs B = A;
+    B.chunk = (long long)A.total >= 4LL * PF_SPOTS * res ? PF_CHUNK : 0;
+    pruned_fft_kernel<P, NZ, MODE, TMA><<<grid, PF_THREADS, Cfg::SMEM, st>>>(B, map);
     return cudaGetLastError();
 }
 
@@ -323,7 +333,7 @@ cudaError_t shwfs_pruned_fft_launch(shwfs_handle *h, const float *phase, int T, 
                                     cudaStream_t st)
 {
     PfArgs A;
-    A.phase = phase; A.amp = h->d_amp; A.patch = h->d_patch; A.slopes = slopes; A.binned = binned;
+    A.phase = phase; A.amp = h->d_amp; A.patch = h->d_patch; A.slopes = slopes; A.binned = binned; A.sched = h->d_sched; A.chunk = 0;
     A.frame_stride = (long long)h->N * h->N;
     A.T = T; A.N = h->N; A.nsub = h->nsub; A.total = T * h->nsub; A.n = h->n;
     A.tau = h->tau;

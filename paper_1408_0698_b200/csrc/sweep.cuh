@@ -9,7 +9,7 @@
  *            without a per-subaperture table (pruned_fft.cu) and every one-tile-per-CTA launch use it.
  *   dynamic  the spots are cut into chunks of `chunk_spots` consecutive spots; a warp works through a chunk and
  *            then takes the next free chunk from a global counter (atomicAdd by lane 0, one grab per chunk,
- *            issued a chunk ahead).  The first chunk of a warp is its own global warp index, the counter hands
+ *            issued a chunk ahead and not waited for until that chunk is entered).  The first chunk of a warp is its own global warp index, the counter hands
  *            out the rest.  For large launches of the kernels that read a table row per spot (wk_fft.cu).
  * Why dynamic: with a static split (strided or contiguous) the CTAs of an SM do not run at the
  * same speed -- the warp scheduler prefers some warp slots -- and the slowest CTA of each SM ran on alone at the
@@ -46,7 +46,8 @@ struct Sweep {
     int chunk_spots;          /* dynamic deal: spots per chunk (even) */
     int half;                 /* 0 / 1: which spot of the warp's pair this thread works on */
     int c_end;                /* first spot past the chunk the look-ahead spot is in */
-    int next_chunk;           /* the chunk after that (already grabbed) */
+    int pending;              /* lane 0: the counter value the atomicAdd for the chunk after that returned -- read
+                                 (and so waited for) only when that chunk is entered, a whole chunk later */
     int n_warps;
 
     /* counter == nullptr: static deal, warp w of the launch takes chunks w, w + n_warps, ... */
@@ -59,13 +60,7 @@ struct Sweep {
         dq = step / T;
         dr = step - dq * T;
         c_end = 0x7fffffff;
-        next_chunk = 0;
-    }
-    __device__ __forceinline__ int grab()
-    {
-        int c = 0;
-        if ((threadIdx.x & 31) == 0) c = atomicAdd(counter, 1);
-        return n_warps + __shfl_sync(0xffffffffu, c, 0);
+        pending = 0;
     }
     __device__ __forceinline__ void enter(Spot &s, int chunk)
     {
@@ -73,7 +68,7 @@ struct Sweep {
         s.i = s.g / T;
         s.t = s.g - s.i * T;
         c_end = (chunk + 1) * chunk_spots;
-        next_chunk = grab();
+        if ((threadIdx.x & 31) == 0) pending = atomicAdd(counter, 1);       /* the chunk after this one */
     }
     /* the warp's first spot */
     __device__ __forceinline__ Spot first()
@@ -96,7 +91,7 @@ struct Sweep {
         s.g += counter != nullptr ? 2 : 2 * n_warps;
         s.i += dq; s.t += dr;
         if (s.t >= T) { s.t -= T; ++s.i; }
-        if (s.g >= c_end) enter(s, next_chunk);     /* dynamic deal only (strided: c_end is never reached) */
+        if (s.g >= c_end) enter(s, n_warps + __shfl_sync(0xffffffffu, pending, 0));   /* dynamic deal only */
     }
     __device__ __forceinline__ void lookup(Spot &s) const { s.pe = __ldg(patch + min(s.i, nsub - 1)); }
     /* the spot's pair is work (its chunk exists); the spot itself may still lie past the last one: live() */

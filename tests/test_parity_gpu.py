@@ -339,3 +339,36 @@ def test_all_six_wfs_frames_0_1_499_999_in_full(gpu, oracle, cfg_id):
         worst = max(worst, err)
         assert err <= SLOPE_TOL, (cfg_id, w, err)
     assert worst <= 1e-4          # measured margin: two orders below the tolerance
+
+
+def test_register_gather_instance_and_alignment_contract(gpu, oracle, monkeypatch):
+    """Config 2 takes its patches by TMA; SHWFS_NO_TMA (read at shwfs_create) selects the register-gather instance
+    of the same kernel, which must give the same slopes; the library says which instance ran (shwfs_last_kernel).
+    Frames that are not 16-byte aligned are outside the contract of include/shwfs.h: SHWFS_EINVAL, nothing launched."""
+    torch, B = gpu
+    c = W.CONFIGS[2]
+    amp = W.pupil_mask(c)
+    T = 2
+    ph = W.phase_frames(c, 0, range(T))
+    phd = torch.from_numpy(ph).cuda()
+    want = None
+    for no_tma, kind in ((False, "tma"), (True, "ldg")):
+        if no_tma:
+            monkeypatch.setenv("SHWFS_NO_TMA", "1")
+        else:
+            monkeypatch.delenv("SHWFS_NO_TMA", raising=False)
+        with B.from_config(c, 0) as s:
+            if want is None:
+                want = oracle.measure(ph, amp, s.valid_yx, c.n, c.P, c.b, tau=c.tau)
+            got = s.measure(phd).cpu().numpy()
+            assert s.last_kernel == f"pruned_fft_kernel<32,16,0,{kind}>", s.last_kernel
+            assert np.abs(got - want).max() <= SLOPE_TOL, (kind, np.abs(got - want).max())
+            buf = torch.zeros(ph.size + 4, dtype=torch.float32, device="cuda")
+            out = torch.empty((T, s.nsub, 2), dtype=torch.float32, device="cuda")
+            n0 = s.launch_count
+            for shift in (1, 2):
+                view = buf[shift:shift + ph.size]
+                assert view.data_ptr() % 16 != 0
+                rc = B.load().shwfs_measure(s._h, view.data_ptr(), T, out.data_ptr(), None)
+                assert rc == B.SHWFS_EINVAL
+            assert s.launch_count == n0
