@@ -372,3 +372,41 @@ def test_register_gather_instance_and_alignment_contract(gpu, oracle, monkeypatc
                 rc = B.load().shwfs_measure(s._h, view.data_ptr(), T, out.data_ptr(), None)
                 assert rc == B.SHWFS_EINVAL
             assert s.launch_count == n0
+
+
+def test_dynamic_deal_ragged_tails_match_oracle(gpu, oracle, monkeypatch):
+    """The persistent instances deal chunks of consecutive spots to warps from a counter (csrc/sweep.cuh).  Totals
+    that are odd, not a multiple of the chunk, smaller than one chunk per warp, and two calls back to back on one
+    handle (the last warp re-arms the counter): every spot against the oracle.
+    config 5 geometry (wkf_kernel<16,..,tma>, chunks of 16) on a subset of subapertures with the persistent instance
+    forced; config 2 (pruned_fft_kernel<32,16,..,tma>, chunks of 4) at a size that takes the dynamic deal by itself."""
+    torch, B = gpu
+    monkeypatch.setenv("SHWFS_FORCE_PERSISTENT", "1")
+    c = W.CONFIGS[5]
+    amp = W.pupil_mask(c)
+    full = oracle.valid_list(amp, c.n, c.min_illum)
+    yx = full[::7][:661].copy()
+    K = W.elongation_kernels(c, 0, yx)
+    with B.from_config(c, 0, kernels=K, valid_yx=yx) as s:
+        for T in (3, 1, 3):
+            ph = W.phase_frames(c, 0, range(T))
+            assert (T * len(yx)) % 2 == 1
+            want = oracle.measure(ph, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K)
+            got = s.measure(torch.from_numpy(ph).cuda()).cpu().numpy()
+            assert s.last_kernel == "wkf_kernel<16,0,0,tma>", s.last_kernel
+            assert np.abs(got - want).max() <= SLOPE_TOL, (T, np.abs(got - want).max())
+    monkeypatch.delenv("SHWFS_FORCE_PERSISTENT")
+    c = W.CONFIGS[2]
+    amp = W.pupil_mask(c)
+    yx = oracle.valid_list(amp, c.n, c.min_illum)[:1211].copy()
+    T = 17
+    ph = W.phase_frames(c, 0, [t % 4 for t in range(T)])
+    assert (T * len(yx)) % 4 == 3 and T * len(yx) >= 4 * 8 * 4 * 148
+    want = oracle.measure(ph[:4], amp, yx, c.n, c.P, c.b, tau=c.tau)
+    with B.from_config(c, 0, valid_yx=yx) as s:
+        phd = torch.from_numpy(ph).cuda()
+        for rep in range(2):
+            got = s.measure(phd).cpu().numpy()
+            assert s.last_kernel == "pruned_fft_kernel<32,16,0,tma>"
+            for t in range(T):
+                assert np.abs(got[t] - want[t % 4]).max() <= SLOPE_TOL, (rep, t)
