@@ -33,6 +33,8 @@
  * comparisons on rates that differ from the oracle's by rounding; where the margin is larger than that, the
  * integer must be the same on both sides (tests/test_lgs_gpu.py), elsewhere it may differ.
  *
+ * Every function below is pinned; what no pin can reach are this build's conventions (the paper says only
+ * "noise-added"): the counter layout of N2, the rate of 30 at which N3 hands over to N4, noise on the binned image.
  * Pins (tests/test_oracle_poisson_pins.py, -m "not gpu"): P1 N3 equals the quantile function of the Poisson
  * distribution (scipy.stats.poisson.ppf) for every u1 clear of a step; P2 mean = variance = lambda and a chi^2
  * test against the Poisson pmf at lambda = 0.3, 3, 29.9 (N3) and 30, 300 (N4); P3 (k - lambda) / sqrt(lambda)
