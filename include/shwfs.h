@@ -36,7 +36,12 @@
  *   - The enqueue-only calls (shwfs_measure, _measure_residual, _reconstruct, _closed_loop, _debug_spots)
  *     must be made with the handle's device current (the one that was current at shwfs_create) and return
  *     SHWFS_EINVAL otherwise; the other calls switch to it and back themselves.
- *   - A handle is not thread-safe; distinct handles are independent (one handle = one WFS).
+ *   - A handle is not thread-safe; distinct handles are independent (one handle = one WFS).  Calls on ONE handle
+ *     must also not overlap on the GPU: enqueue them on one stream, or order the streams with events.  The handle
+ *     owns device state that a call uses while it runs (the chunk counter from which the persistent kernels are
+ *     dealt their spots, the DM-phase scratch of shwfs_measure_residual); two calls of one handle running at the
+ *     same time on different streams would share it.  Different handles may run concurrently (bench.py runs the six
+ *     LGS sensors that way).
  */
 #ifndef SHWFS_H_
 #define SHWFS_H_
