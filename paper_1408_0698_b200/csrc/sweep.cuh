@@ -101,7 +101,13 @@ struct Sweep {
     __device__ __forceinline__ void leave() const
     {
         if (counter != nullptr && (threadIdx.x & 31) == 0) {
-            if (atomicAdd(counter + 1, 1) == n_warps - 1) { counter[0] = 0; counter[1] = 0; }
+            /* this warp's grabs (the last one is never read) are ordered before its "done", and every warp's "done"
+             * before the reset: the fences make that hold by the memory model, not just by the path to L2 */
+            __threadfence();
+            if (atomicAdd(counter + 1, 1) == n_warps - 1) {
+                __threadfence();
+                counter[0] = 0; counter[1] = 0;
+            }
         }
     }
 };

@@ -72,8 +72,9 @@ def test_sensor_kernels_are_deterministic_and_stay_in_bounds(gpu, monkeypatch, c
         assert bool(torch.isfinite(ref).all())
         for rep in range(REPS):
             keep = _busy(torch, side) if rep % 4 == 0 else None
+            out.fill_(float("nan"))                 # a spot the deal skipped would otherwise keep its old value
             s.measure(ph, out=out)
-            assert torch.equal(out, ref), (rep, s.last_kernel, float((out - ref).abs().max()))
+            assert torch.equal(out, ref), (rep, s.last_kernel, int((out != ref).sum()))
             del keep
         names.add(s.last_kernel)
         _check_guards(buf, out.numel())
@@ -116,6 +117,7 @@ def test_lgs_and_loop_kernels_are_deterministic(gpu):
         ref = s.measure_residual(ph1, coef).clone()
         for rep in range(REPS // 2):
             keep = _busy(torch, side) if rep % 4 == 0 else None
+            out.fill_(float("nan"))
             s.measure_residual(ph1, coef, out=out)
             assert torch.equal(out, ref), rep
             del keep

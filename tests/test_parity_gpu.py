@@ -392,7 +392,8 @@ def test_dynamic_deal_ragged_tails_match_oracle(gpu, oracle, monkeypatch):
             ph = W.phase_frames(c, 0, range(T))
             assert (T * len(yx)) % 2 == 1
             want = oracle.measure(ph, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K)
-            got = s.measure(torch.from_numpy(ph).cuda()).cpu().numpy()
+            out = torch.full((T, len(yx), 2), float("nan"), dtype=torch.float32, device="cuda")   # skipped spot = NaN
+            got = s.measure(torch.from_numpy(ph).cuda(), out=out).cpu().numpy()
             assert s.last_kernel == "wkf_kernel<16,0,0,tma>", s.last_kernel
             assert np.abs(got - want).max() <= SLOPE_TOL, (T, np.abs(got - want).max())
     monkeypatch.delenv("SHWFS_FORCE_PERSISTENT")
@@ -406,7 +407,8 @@ def test_dynamic_deal_ragged_tails_match_oracle(gpu, oracle, monkeypatch):
     with B.from_config(c, 0, valid_yx=yx) as s:
         phd = torch.from_numpy(ph).cuda()
         for rep in range(2):
-            got = s.measure(phd).cpu().numpy()
+            out = torch.full((T, len(yx), 2), float("nan"), dtype=torch.float32, device="cuda")
+            got = s.measure(phd, out=out).cpu().numpy()
             assert s.last_kernel == "pruned_fft_kernel<32,16,0,tma>"
             for t in range(T):
                 assert np.abs(got[t] - want[t % 4]).max() <= SLOPE_TOL, (rep, t)
