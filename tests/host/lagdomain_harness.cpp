@@ -5,11 +5,16 @@
  *     csrc/wk_common.cuh  H5 + x half of H6   finish_row (scalar) and finish_row2 (packed, staged table row in the
  *                         visiting order of term_lag / term_m / term_first);  y half of H6   ytransform16
  *     csrc/cog.cuh        H7 + H8   cog16, its half-warp xor shuffles simulated (see shuffle16 below)
- * compiled AS THEY ARE for the host.  What the harness supplies itself: the autocorrelation G of the device-made fp32
- * field, by the plain double sums of its definition, and the table M from the formula of DESIGN.md 6.1
+ * compiled AS THEY ARE for the host, and
+ *     csrc/wk.cu          H0   wk_table_kernel, the float64 table M, cut out of the .cu file as text
+ *                         ("wk_table_extract.inc", written by tests/test_lagdomain_host.py) and run with ONE simulated
+ *                         thread per block (its loops stride by blockDim.x; the dynamic shared array is a plain buffer).
+ * What the harness supplies itself: the autocorrelation G of the device-made fp32 field, by the plain double sums of
+ * its definition (the kernels' own sums: tests/test_wk_acc_host.py), and -- as a cross-check of the table kernel only
+ * -- M from the formula of DESIGN.md 6.1
  *     M[ly,lx] = Z[ly,lx] beta(ly) beta(lx) / P^2 (x 2 for ly >= 1),  beta(l) = sum_{alpha<b} w^(alpha l),
- *     Z = DFT of the spatial kernel at (-ly,-lx), or (-1)^(ly+lx) without kernels,   w = exp(2 pi i / P)
- * (on the device those are wk_measure_kernel / wkf_kernel and wk_table_kernel: GPU tests only).  So a green run says:
+ *     Z = DFT of the spatial kernel at (-ly,-lx), or (-1)^(ly+lx) without kernels,   w = exp(2 pi i / P).
+ * So a green run says:
  * the identity B[R,C] = Re sum G M w_D^(R ly + C lx) with its centring, binning and aliasing mod 16, AS THE DEVICE
  * CODE EVALUATES IT, reproduces the oracle's binned image to 1e-4 of the peak and its slopes to 1e-3 px (north_star).
  * Built and run by tests/test_lagdomain_host.py (gcc + g++, no GPU).  Test infrastructure only.
@@ -46,6 +51,14 @@ static inline float __shfl_xor_sync(unsigned, float v, int o)
 #include "../../paper_1408_0698_b200/csrc/field.cuh"
 #include "../../paper_1408_0698_b200/csrc/cog.cuh"
 
+/* wk_table_kernel on the host: one thread per block */
+struct Dim { unsigned x, y, z; };
+static Dim threadIdx = {0, 0, 0}, blockIdx = {0, 0, 0}, blockDim = {1, 1, 1};
+static inline void __syncthreads() {}
+static inline void sincospi(double x, double *s, double *c) { *s = std::sin(M_PI * x); *c = std::cos(M_PI * x); }
+static double2 tmp[64 * 63];                   /* the kernel's `extern __shared__ double2 tmp[]`: [P][2n-1] */
+#include "wk_table_extract.inc"
+
 extern "C" {
 void shwfs_oracle_field(const float *phase_frame, const float *amplitude, int N, int n, int P, int sy, int sx,
                         double c_phi, double *e);
@@ -61,7 +74,7 @@ using namespace shwfs;
 typedef std::complex<double> cd;
 
 static std::mt19937 rng(140806u);
-static double worst_img = 0, worst_slope = 0;
+static double worst_img = 0, worst_slope = 0, worst_table = 0;
 
 template <int MODE>
 static float2 shuffle16(const float (&B)[16][16], float tau)
@@ -133,6 +146,20 @@ static bool one_spot(int P, int b, bool with_kernel, float tau, int mode, float 
             const cd m = Z * by * bx / (double)(P * P) * (ly >= 1 ? 2.0 : 1.0);
             M[(size_t)a * n + ly] = make_float2((float)m.real(), (float)m.imag());
         }
+    /* H0 as the device builds it; must agree with the formula, and is what the product below uses */
+    {
+        std::vector<float2> Md((size_t)LX * n);
+        blockIdx.x = 0;
+        wk_table_kernel(with_kernel ? K.data() : nullptr, with_kernel ? 1 : 0, n, P, b, Md.data());
+        double mscale = 0;
+        for (const float2 &v : M) mscale = std::fmax(mscale, std::hypot((double)v.x, (double)v.y));
+        for (size_t q = 0; q < M.size(); ++q) {
+            const double e = std::hypot((double)Md[q].x - M[q].x, (double)Md[q].y - M[q].y) / mscale;
+            worst_table = std::fmax(worst_table, e);
+            if (!(e <= 1e-6)) { std::printf("FAIL: n=%d P=%d b=%d kernel=%d: table entry %zu off by %.3g of the largest\n", n, P, b, (int)with_kernel, q, e); return false; }
+        }
+        M = Md;
+    }
     float Bs[16][16], Bp[16][16];
     float Hs[n][32], Hp[n][32];
     for (int ly = 0; ly < n; ++ly) {
@@ -209,6 +236,7 @@ int main()
         if (!one_spot<12>(32, 2, true, tau, mode, ps)) return 1;
         spots += 6;
     }
-    std::printf("ok %d spots, worst image error %.3g of the peak, worst slope error %.3g px\n", spots, worst_img, worst_slope);
+    std::printf("ok %d spots, device table within %.3g of the formula, worst image error %.3g of the peak, worst slope error %.3g px\n",
+                spots, worst_table, worst_img, worst_slope);
     return 0;
 }
