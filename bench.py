@@ -215,7 +215,7 @@ class Workload:
             self.phase = [W.phase_frames_device(c, w, my_frames, dev) for w in range(c.W)]
         if noise_flux > 0:
             for w, s in enumerate(self.sensors):
-                s.set_noise(noise_flux / c.n ** 2, args.read_noise, 14080698 + w)
+                s.set_noise(noise_flux / c.n ** 2, args.read_noise, 14080698 + w, photon_model=args.photon_model)
         self.nsub = self.sensors[0].nsub
         self.slopes = [torch.empty((frames, self.nsub, 2), dtype=torch.float32, device=dev) for _ in range(c.W)]
         self.spots_per_step = c.W * frames * self.nsub
@@ -540,7 +540,8 @@ def cpu_baseline(c, args, phase_dev, yx_lib=None):
         kw = dict(weight=sod["weight"] if L > 0 else [1.0], defocus=sod["defocus"] if L > 0 else [0.0],
                   tilt_x=sod["tilt_x"] if L > 0 else None, tilt_y=sod["tilt_y"] if L > 0 else None,
                   cx=sod["cx"], cy=sod["cy"], tau=c.tau, kernels=K,
-                  flux=args.noise_flux / c.n ** 2, ron=args.read_noise, seed=14080698)
+                  flux=args.noise_flux / c.n ** 2, ron=args.read_noise, seed=14080698,
+                  photon_model=args.photon_model)
         run = lambda p: O.measure_lgs(p, amp, yx, c.n, c.P, c.b, c.dx, **kw)
         nfr = max(1, args.cpu_frames // max(L, 1))
     else:
@@ -599,6 +600,8 @@ def main():
     ap.add_argument("--noise-flux", type=float, default=0.0,
                     help="> 0: detector noise, photo-electrons per fully lit subaperture per frame (8(f) f2)")
     ap.add_argument("--read-noise", type=float, default=3.0)
+    ap.add_argument("--photon-model", type=int, default=0, choices=[0, 1],
+                    help="with --noise-flux: 0 = Gaussian limit of the photon noise, 1 = Poisson counts (include/shwfs.h)")
     ap.add_argument("--dm-modes", type=int, default=0,
                     help="M > 0: subtract a DM of M modes inside the gather (8(f) f3, shwfs_measure_residual)")
     ap.add_argument("--pyramid", default=None, choices=["tiny", "lbt"],
