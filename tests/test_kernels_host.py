@@ -1,0 +1,179 @@
+"""Whole kernels of csrc/ on the host: the kernel is cut out of its .cu file as text, compiled by g++ with the headers
+it includes as they are, and run thread by thread on the coroutine SIMT machine of tests/host/simt.h (shared memory,
+shuffles, __syncwarp / __syncthreads, the chunk counter of the dynamic deal, TMA boxes with their swizzle and
+mbarriers) on the same seeded inputs as the float64 oracle: binned images within 1e-4 of the spot peak, slopes within
+1e-3 px (north_star), for every spot.  Each case runs under three thread orders (ascending, descending, seeded
+random between synchronisation points) and must give bit-identical results: a barrier the code needs and does not
+have shows up as a difference.  CPU-side parity of device code, thread mapping included: no GPU."""
+import dataclasses
+import re
+import shutil
+import struct
+import subprocess
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+from oracle import shwfs_oracle as O
+from paper_1408_0698_b200 import workloads as W
+
+ROOT = Path(__file__).resolve().parent.parent
+CSRC = ROOT / "paper_1408_0698_b200" / "csrc"
+CUDA_INC = Path("/usr/local/cuda/include")
+PATCH_LIT = 1 << 30
+
+needs_toolchain = pytest.mark.skipif(shutil.which("g++") is None or not (CUDA_INC / "cuda_runtime.h").exists(),
+                                     reason="needs g++ and the CUDA headers")
+
+
+def small_config(base: int, S: int, **kw) -> W.WfsConfig:
+    """The geometry of config `base` on S x S subapertures: same n, P, b, pixel size and wavelength; the pupil radii
+    scaled to the smaller grid so that fully lit, partially lit and dark subapertures all occur."""
+    c = W.CONFIGS[base]
+    N = S * c.n
+    r_out = 0.5 * N * c.dx
+    return dataclasses.replace(c, N=N, S=S, r_out=r_out, r_in=r_out * c.r_in / c.r_out if c.r_out else 0.0,
+                               screen_M=256, **kw)
+
+
+def cut(src: str, begin: str, end: str) -> str:
+    assert src.count(begin) == 1 and src.count(end) == 1, (begin, end)
+    block = src[src.index(begin):src.index(end)]
+    assert "<<<" not in block
+    return block
+
+
+def build_harness(tmp_path: Path, name: str) -> Path:
+    exe = tmp_path / name
+    r = subprocess.run(["g++", "-std=c++17", "-O0", "-ffp-contract=off", f"-I{CUDA_INC}", f"-I{tmp_path}",
+                        "-Wno-attributes", "-Wno-psabi", "-o", str(exe), str(ROOT / "tests" / "host" / f"{name}.cpp")],
+                       capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stderr[-3000:]
+    return exe
+
+
+def patch_table(amp: np.ndarray, yx: np.ndarray, n: int) -> np.ndarray:
+    """What shwfs_create puts into the handle (api.cu, "patch table"): origin in pixels, flag for all-ones patches."""
+    out = np.zeros((len(yx), 2), np.int32)
+    for i, (sy, sx) in enumerate(yx):
+        lit = bool(np.all(amp[sy * n:(sy + 1) * n, sx * n:(sx + 1) * n] == 1.0))
+        out[i] = (sx * n | (PATCH_LIT if lit else 0), sy * n)
+    return out
+
+
+def compare(got_slopes, got_img, want_slopes, want_img, tau, mode, label):
+    assert not np.isnan(got_slopes).any() and not np.isnan(got_img).any(), f"{label}: a spot was never written"
+    peak = want_img.max(axis=(2, 3), keepdims=True)
+    ierr = float((np.abs(got_img - want_img) / peak).max())
+    assert ierr <= 1e-4, (label, ierr)
+    serr = np.abs(got_slopes - want_slopes).max(axis=2)
+    if mode == 1:
+        # hard mask: compare the spots none of whose pixels sits within rounding of the threshold (tests/test_parity_gpu.py)
+        clear = (np.abs(want_img - tau * peak) > 2e-4 * peak).all(axis=(2, 3))
+        assert clear.mean() > 0.5, label
+        serr = serr[clear]
+    assert float(serr.max()) <= 1e-3, (label, float(serr.max()))
+    return ierr, float(serr.max())
+
+
+# ---------------------------------------------------------------- pruned_fft_kernel (config 2's kernel)
+
+PF_CASES = [
+    # base config, S, T, mode, tau, instances [(tma, chunk, lazy)]
+    (2, 6, 5, 0, 0.10, [(0, 0, 0), (1, 0, 0), (1, 4, 1), (0, 4, 0)]),     # n = 16, P = 32: <32,16>
+    (1, 10, 3, 0, 0.0, [(0, 0, 0), (0, 4, 0)]),                           # config 1 itself, n = 8, P = 16: <16,8>
+    (3, 8, 3, 1, 0.10, [(0, 0, 0)]),                                      # n = 10 < NZ = 16, P = 32, hard threshold
+    (5, 6, 3, 0, 0.10, [(1, 4, 0), (0, 0, 0)]),                           # n = 16, P = 64, b = 4: <64,16>
+]
+
+
+def pf_extract(tmp_path: Path, mutate=None) -> None:
+    src = (CSRC / "pruned_fft.cu").read_text()
+    block = cut(src, "constexpr int PF_THREADS", "template <int P, int NZ, int MODE, bool TMA>\ncudaError_t launch_pf_inst")
+    block, k = re.subn(r"extern __shared__ __align__\(16\) unsigned char pf_smem\[\];",
+                       "unsigned char *pf_smem = simt::smem();", block)
+    assert k == 1 and "pruned_fft_kernel(const PfArgs A" in block and "cog16<MODE>" in block
+    if mutate is not None:
+        assert block.count(mutate[0]) == 1, mutate[0]
+        block = block.replace(mutate[0], mutate[1])
+    (tmp_path / "pf_kernel_extract.inc").write_text(block)
+
+
+def pf_run(exe, tmp_path, c, T, nsub, mode, tau, ph, amp, table, tma, chunk, lazy, grid, order, seed):
+    """One simulated launch; returns (slopes, binned images, stdout) or None when the harness reports a failure."""
+    fin, fout = tmp_path / "in.bin", tmp_path / "out.bin"
+    with open(fin, "wb") as f:
+        f.write(struct.pack("14i", c.N, c.n, c.P, T, nsub, mode, tma, chunk, grid, order, seed, lazy, 0, 0))
+        f.write(struct.pack("2f", tau, 1.0))
+        f.write(ph.astype(np.float32).tobytes())
+        f.write(amp.astype(np.float32).tobytes())
+        f.write(table.tobytes())
+    r = subprocess.run([str(exe), str(fin), str(fout)], capture_output=True, text=True, timeout=600)
+    if r.returncode != 0 or not r.stdout.startswith("ok "):
+        assert r.stdout.startswith("FAIL"), r.stdout[-500:] + r.stderr[-500:]
+        return None
+    raw = np.fromfile(fout, np.float32)
+    ns, ni = T * nsub * 2, T * nsub * 256
+    got = raw[:ns].reshape(T, nsub, 2).astype(np.float64)
+    img = raw[ns:ns + ni].reshape(T, nsub, 16, 16).astype(np.float64)
+    counters = raw[ns + ni:].view(np.int32)
+    assert (counters == 0).all(), f"chunk counters not re-armed: {counters}"
+    return got, img, r.stdout
+
+
+@needs_toolchain
+def test_pruned_fft_kernel_whole_on_the_host(tmp_path):
+    pf_extract(tmp_path)
+    exe = build_harness(tmp_path, "pf_kernel_harness")
+
+    runs = 0
+    for base, S, T, mode, tau, instances in PF_CASES:
+        c = W.CONFIGS[1] if (base, S) == (1, 10) else small_config(base, S)
+        amp = W.pupil_mask(c)
+        yx = O.valid_list(amp, c.n, c.min_illum)
+        ph = W.phase_frames(c, 0, range(T))
+        nsub = len(yx)
+        table = patch_table(amp, yx, c.n)
+        lit = (table[:, 0] & PATCH_LIT) != 0
+        if base != 1:
+            assert lit.any() and (~lit).any(), "the case should have both kinds of subaperture"
+        want, wimg = O.measure(ph, amp, yx, c.n, c.P, c.b, tau=tau, mode=mode, stage=2)
+        for tma, chunk, lazy in instances:
+            first = None
+            for order, grid in ((0, 3), (1, 3), (2, 2)):
+                if chunk:
+                    # the launcher deals chunks only when every warp has work; keep that in the small case
+                    grid = max(1, min(grid, (T * nsub) // (4 * chunk)))
+                label = f"config {base} S={S} tma={tma} chunk={chunk} lazy={lazy} order={order} grid={grid}"
+                out = pf_run(exe, tmp_path, c, T, nsub, mode, tau, ph, amp, table, tma, chunk, lazy, grid, order, 1408 + runs)
+                assert out is not None, label
+                got, img, stdout = out
+                words = stdout.split()
+                boxes = int(words[words.index("boxes") + 1])
+                assert boxes == (T * nsub if tma else 0) and words[-1] == "0", f"{label}: {stdout}"
+                compare(got, img, want, wimg, tau, mode, label)
+                # same arithmetic whatever the thread order and the grid: bit-identical
+                if first is None:
+                    first = (got, img)
+                else:
+                    assert np.array_equal(first[0], got) and np.array_equal(first[1], img), f"{label}: depends on the thread order"
+                runs += 1
+    assert runs == 27
+
+    # the machine does see a missing barrier: without the __syncwarp between the row pass and the column pass the
+    # register-gather instance reads rows nobody has written yet (wrong images), and the TMA instance re-arms a
+    # staging slot other lanes still wait for (the launch hangs)
+    pf_extract(tmp_path, ("__syncwarp();                                      /* rows visible; the staging slot has been read */", ""))
+    mutant = build_harness(tmp_path, "pf_kernel_harness")
+    c = small_config(2, 6)
+    amp = W.pupil_mask(c)
+    yx = O.valid_list(amp, c.n, c.min_illum)
+    ph = W.phase_frames(c, 0, range(2))
+    table = patch_table(amp, yx, c.n)
+    want, wimg = O.measure(ph, amp, yx, c.n, c.P, c.b, tau=0.1, stage=2)
+    for tma in (0, 1):
+        out = pf_run(mutant, tmp_path, c, 2, len(yx), 0, 0.1, ph, amp, table, tma, 0, 0, 2, 0, 1)
+        if out is not None:
+            with pytest.raises(AssertionError):
+                compare(out[0], out[1], want, wimg, 0.1, 0, "mutant")
