@@ -54,7 +54,7 @@ struct Cta {
 
 struct Thread {
     ucontext_t ctx;
-    std::vector<unsigned char> stack;
+    unsigned char *stack = nullptr;  /* not zero-filled: most of it is never touched */
     Dim tid, bid;
     Cta *cta;
     Warp *warp;
@@ -137,10 +137,10 @@ static bool launch(int grid, int block, size_t smem_bytes, Order order, unsigned
             T.warp = &ctas[c].warps[t / 32];
             T.lane = t % 32;
             T.warp->live++;
-            T.stack.resize(stack_bytes);
+            T.stack = static_cast<unsigned char *>(std::malloc(stack_bytes));
             getcontext(&T.ctx);
-            T.ctx.uc_stack.ss_sp = T.stack.data();
-            T.ctx.uc_stack.ss_size = T.stack.size();
+            T.ctx.uc_stack.ss_sp = T.stack;
+            T.ctx.uc_stack.ss_size = stack_bytes;
             T.ctx.uc_link = &g_main;
             makecontext(&T.ctx, trampoline, 0);
         }
@@ -166,9 +166,10 @@ static bool launch(int grid, int block, size_t smem_bytes, Order order, unsigned
         left -= finished;
         /* a whole round in which no barrier was released and nobody finished: every thread only re-checked the
          * barrier it sits at, and nothing can change that any more */
-        if (g_progress == before) { if (++idle_rounds > 2) return false; }
+        if (g_progress == before) { if (++idle_rounds > 2) return false; }     /* (stacks left to the exit) */
         else idle_rounds = 0;
     }
+    for (Thread &T : th) std::free(T.stack);
     return true;
 }
 
@@ -249,6 +250,13 @@ static inline float2 __ffma2_rn(float2 a, float2 b, float2 c) { return make_floa
 static inline float2 __fadd2_rn(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 static inline float2 __fmul2_rn(float2 a, float2 b) { return make_float2(a.x * b.x, a.y * b.y); }
 extern "C" void __sincosf(float x, float *s, float *c) noexcept { *s = sinf(x); *c = cosf(x); }
+extern "C" float __logf(float x) noexcept { return logf(x); }
+extern "C" float __expf(float x) noexcept { return expf(x); }
+static inline uint32_t __umulhi(uint32_t a, uint32_t b) { return (uint32_t)(((uint64_t)a * b) >> 32); }
+static inline void sincospi(double x, double *s, double *c) { *s = std::sin(M_PI * x); *c = std::cos(M_PI * x); }
+static inline void sincospif(float x, float *s, float *c) { *s = (float)std::sin(M_PI * (double)x); *c = (float)std::cos(M_PI * (double)x); }
+#undef __noinline__
+#define __noinline__ __attribute__((noinline))
 static inline size_t __cvta_generic_to_shared(const void *p) { return (size_t)p; }
 
 /* csrc/tma.cuh, simulated (the header itself is inline PTX) */

@@ -1,0 +1,119 @@
+/*
+ * wk_kernel_harness.cpp -- the lag-domain kernels of csrc/wk.cu run WHOLE on the host: wk_table_kernel (H0, the
+ * float64 table M), wk_measure_kernel<n, MODE, EXTK> (the headline kernel of configs 3/4: H1 .. H8 of
+ * include/shwfs.h, one CTA of n/2 warps per 32 spots, four barrier-fenced phases, second-pass rows of H written over
+ * the field buffer) and wk_generic_kernel, cut out of the .cu file as text ("wk_kernel_extract.inc", written by
+ * tests/test_kernels_host.py) with the headers they include compiled as they are, on the coroutine SIMT machine of
+ * simt.h -- every thread of every CTA, its shared memory, __syncthreads and half-warp shuffles.
+ *
+ * usage: wk_kernel_harness in.bin out.bin
+ *   in.bin   int32[12] {N, n, P, b, T, nsub, mode, has_k, generic, order, seed, L}, float[2] {tau, c_phi},
+ *            float sod_q[8], sod_sw[8], phase[T*(L>1 ? L : 1)*N*N] (L > 1: one wavefront per sub-layer), amp[N*N],
+ *            int32 valid[nsub*2] (sy, sx), float K[has_k ? nsub*P*P : 0], float sod_g[L*nsub*2]
+ *   out.bin  slopes[T*nsub*2], binned[T*nsub*D*D]
+ * What the harness supplies itself is what the launchers (host code of wk.cu) do: the WkArgs and the grids.
+ * The comparison with the float64 oracle is the Python test's.  Test infrastructure only.
+ */
+#include "simt.h"
+
+#include "../../paper_1408_0698_b200/csrc/internal.h"
+#include "../../paper_1408_0698_b200/csrc/fft_regs.cuh"
+#include "../../paper_1408_0698_b200/csrc/field.cuh"
+#include "../../paper_1408_0698_b200/csrc/cog.cuh"
+#include "../../paper_1408_0698_b200/csrc/noise.cuh"
+#include "../../paper_1408_0698_b200/csrc/wk_common.cuh"
+
+namespace {
+using namespace shwfs;
+#include "wk_kernel_extract.inc"
+
+struct Job {
+    int N, n, P, b, T, nsub, mode, has_k, generic, order, seed, L;
+    float tau, c_phi;
+    float sod_q[8], sod_sw[8];
+};
+
+template <int n, int MODE, int EXTK>
+bool run(const Job &J, const WkArgs &A)
+{
+    using Cfg = WkCfg<n>;
+    const int grid = (A.total + Cfg::SPOTS - 1) / Cfg::SPOTS;
+    return simt::launch(grid, Cfg::THREADS, WkSmem<n, (EXTK < 2)>::BYTES, (simt::Order)J.order, (unsigned)J.seed,
+                        [&]() { wk_measure_kernel<n, MODE, EXTK>(A); });
+}
+
+template <int n>
+bool special(const Job &J, const WkArgs &A)
+{
+    if (A.L > 1) return A.mode == 0 ? run<n, 0, 2>(J, A) : run<n, 1, 2>(J, A);
+    if (A.L > 0) return A.mode == 0 ? run<n, 0, 1>(J, A) : run<n, 1, 1>(J, A);
+    return A.mode == 0 ? run<n, 0, 0>(J, A) : run<n, 1, 0>(J, A);
+}
+}  // namespace
+
+int main(int argc, char **argv)
+{
+    if (argc != 3) return 2;
+    static_assert(SHWFS_MAX_LAYERS == 8, "the job header carries 8 sub-layers");
+    FILE *f = std::fopen(argv[1], "rb");
+    if (!f) return 2;
+    Job J;
+    if (std::fread(&J, 4, 12, f) != 12 || std::fread(&J.tau, 4, 18, f) != 18) return 2;
+    const int D = J.P / J.b, LX = 2 * J.n - 1, layers = J.L > 1 ? J.L : 1;
+    const size_t NN = (size_t)J.N * J.N, total = (size_t)J.T * J.nsub;
+    std::vector<float> phase(NN * J.T * layers), amp(NN), K(J.has_k ? (size_t)J.nsub * J.P * J.P : 0);
+    std::vector<int2> valid(J.nsub);
+    std::vector<float2> sod_g((size_t)J.L * J.nsub);
+    if (std::fread(phase.data(), 4, phase.size(), f) != phase.size() || std::fread(amp.data(), 4, NN, f) != NN ||
+        std::fread(valid.data(), 8, valid.size(), f) != valid.size() || std::fread(K.data(), 4, K.size(), f) != K.size() ||
+        std::fread(sod_g.data(), 8, sod_g.size(), f) != sod_g.size()) return 2;
+    std::fclose(f);
+
+    /* H0: as shwfs_wk_build_table launches it */
+    const int blocks = J.has_k ? J.nsub : 1;
+    std::vector<float2> M((size_t)blocks * LX * J.n);
+    if (!simt::launch(blocks, 128, J.has_k ? sizeof(double2) * (size_t)J.P * LX : 0, (simt::Order)J.order, (unsigned)J.seed,
+                      [&]() { wk_table_kernel(K.data(), J.has_k, J.n, J.P, J.b, M.data()); })) {
+        std::printf("FAIL: the table launch dead-locked\n");
+        return 1;
+    }
+
+    std::vector<float> slopes(total * 2, NAN), binned(total * D * D, NAN);
+    WkArgs A;
+    std::memset(&A, 0, sizeof(A));
+    A.phase = phase.data(); A.amp = amp.data(); A.valid = valid.data(); A.M = M.data();
+    A.slopes = slopes.data(); A.binned = binned.data();
+    A.frame_stride = (long long)NN;
+    A.sod_g = sod_g.data(); A.L = J.L;
+    for (int l = 0; l < 8; ++l) { A.sod_q[l] = J.sod_q[l]; A.sod_sw[l] = J.sod_sw[l]; }
+    if (J.L > 1) { A.layer_stride = A.frame_stride; A.frame_stride *= J.L; }
+    A.T = J.T; A.N = J.N; A.nsub = J.nsub; A.mstride = J.has_k ? LX * J.n : 0;
+    A.total = (int)total; A.mode = J.mode;
+    A.tau = J.tau;
+    A.turns = (float)((double)J.c_phi / 6.283185307179586476925286766559);
+    A.ramp_unit = 0.5f / (float)J.P;
+
+    bool ok = false;
+    if (J.generic) {
+        const size_t smem = sizeof(float2) * (size_t)(J.n * J.n + J.n * LX + D) + sizeof(float) * (size_t)(D * D + 3 * GEN_THREADS);
+        ok = simt::launch(A.total, GEN_THREADS, smem, (simt::Order)J.order, (unsigned)J.seed,
+                          [&]() { wk_generic_kernel(A, J.n, D); });
+    } else {
+        if (D != 16) { std::printf("FAIL: the specialised kernel is for D = 16\n"); return 1; }
+        switch (J.n) {
+        case 8: ok = special<8>(J, A); break;
+        case 10: ok = special<10>(J, A); break;
+        case 16: ok = special<16>(J, A); break;
+        default: return 2;
+        }
+    }
+    if (!ok) { std::printf("FAIL: the launch dead-locked\n"); return 1; }
+
+    f = std::fopen(argv[2], "wb");
+    if (!f) return 2;
+    std::fwrite(slopes.data(), 4, slopes.size(), f);
+    std::fwrite(binned.data(), 4, binned.size(), f);
+    std::fclose(f);
+    std::printf("ok switches %ld\n", simt::g_switches);
+    return 0;
+}

@@ -177,3 +177,105 @@ def test_pruned_fft_kernel_whole_on_the_host(tmp_path):
         if out is not None:
             with pytest.raises(AssertionError):
                 compare(out[0], out[1], want, wimg, 0.1, 0, "mutant")
+
+
+# ---------------------------------------------------------------- wk.cu: table kernel + the headline kernel
+
+def wk_extract(tmp_path: Path, mutate=None) -> None:
+    src = (CSRC / "wk.cu").read_text()
+    block = cut(src, "__global__ void wk_table_kernel(", "template <int n, int MODE, int EXTK>\ncudaError_t launch_special_mode")
+    block, k1 = re.subn(r"extern __shared__ double2 tmp\[\];", "double2 *tmp = reinterpret_cast<double2 *>(simt::smem());", block)
+    block, k2 = re.subn(r"extern __shared__ __align__\(16\) float smem\[\];",
+                        "float *smem = reinterpret_cast<float *>(simt::smem());", block)
+    assert (k1, k2) == (1, 2) and "wk_measure_kernel(const WkArgs A)" in block and "wk_generic_kernel(const WkArgs A" in block
+    if mutate is not None:
+        assert block.count(mutate[0]) == 1, mutate[0]
+        block = block.replace(mutate[0], mutate[1])
+    (tmp_path / "wk_kernel_extract.inc").write_text(block)
+
+
+def wk_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, generic, order, seed, L=0, sod_q=(), sod_sw=(), sod_g=None):
+    nsub = len(yx)
+    fin, fout = tmp_path / "in.bin", tmp_path / "out.bin"
+    with open(fin, "wb") as f:
+        f.write(struct.pack("12i", c.N, c.n, c.P, c.b, T, nsub, mode, int(K is not None), generic, order, seed, L))
+        f.write(struct.pack("2f", tau, 1.0))
+        f.write(np.resize(np.asarray(list(sod_q) + [0.0] * 8, np.float32), 8).tobytes())
+        f.write(np.resize(np.asarray(list(sod_sw) + [0.0] * 8, np.float32), 8).tobytes())
+        f.write(np.ascontiguousarray(ph, np.float32).tobytes())
+        f.write(np.ascontiguousarray(amp, np.float32).tobytes())
+        f.write(np.ascontiguousarray(yx, np.int32).tobytes())
+        if K is not None:
+            f.write(np.ascontiguousarray(K, np.float32).tobytes())
+        if sod_g is not None:
+            f.write(np.ascontiguousarray(sod_g, np.float32).tobytes())
+    r = subprocess.run([str(exe), str(fin), str(fout)], capture_output=True, text=True, timeout=900)
+    if r.returncode != 0 or not r.stdout.startswith("ok "):
+        assert r.stdout.startswith("FAIL"), r.stdout[-500:] + r.stderr[-500:]
+        return None
+    raw = np.fromfile(fout, np.float32)
+    D = c.P // c.b
+    ns = T * nsub * 2
+    return raw[:ns].reshape(T, nsub, 2).astype(np.float64), raw[ns:].reshape(T, nsub, D, D).astype(np.float64)
+
+
+WK_CASES = [
+    # base config, S, T, mode, tau, elongation kernels, generic kernel too
+    (3, 8, 3, 0, 0.10, True, True),       # n = 10, P = 32, b = 2 with per-subaperture kernels: the headline instance
+    (3, 8, 1, 1, 0.10, False, False),     # the same without kernels (shared table), hard threshold
+    (1, 10, 3, 0, 0.0, False, True),      # config 1 itself: n = 8, P = 16, b = 1
+    (5, 6, 2, 0, 0.10, True, False),      # n = 16, P = 64, b = 4 with kernels
+]
+
+
+@needs_toolchain
+def test_lag_domain_kernels_whole_on_the_host(tmp_path):
+    wk_extract(tmp_path)
+    exe = build_harness(tmp_path, "wk_kernel_harness")
+    runs = 0
+    for base, S, T, mode, tau, with_k, generic_too in WK_CASES:
+        c = W.CONFIGS[1] if (base, S) == (1, 10) else small_config(base, S)
+        amp = W.pupil_mask(c)
+        yx = O.valid_list(amp, c.n, c.min_illum)
+        ph = W.phase_frames(c, 0, range(T))
+        K = W.elongation_kernels(c, 0, yx) if with_k else None
+        assert (T * len(yx)) % 32 != 0, "the last CTA should be ragged"
+        want, wimg = O.measure(ph, amp, yx, c.n, c.P, c.b, tau=tau, mode=mode, kernels=K, stage=2)
+        first = None
+        for order in (0, 1, 2):
+            label = f"config {base} S={S} kernels={with_k} order={order}"
+            out = wk_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, 0, order, 698 + runs)
+            assert out is not None, label
+            compare(out[0], out[1], want, wimg, tau, mode, label)
+            if first is None:
+                first = out
+            else:
+                assert np.array_equal(first[0], out[0]) and np.array_equal(first[1], out[1]), f"{label}: depends on the thread order"
+            runs += 1
+        if generic_too and mode == 0:
+            # the size-generic kernel: one frame, an independently written cross-check of the same table
+            out = wk_run(exe, tmp_path, c, 1, yx, mode, tau, ph[:1], amp, K, 1, 2, 5)
+            assert out is not None
+            compare(out[0], out[1], want[:1], wimg[:1], tau, mode, f"config {base} generic")
+            runs += 1
+    assert runs == 14
+
+    # the barrier the round-1 review worried about: the second-pass rows of H overwrite the field buffer "behind one
+    # __syncthreads()" -- without it a warp that finishes its lag row early destroys field rows other warps still
+    # read, and the machine shows it (wrong images under at least one thread order)
+    wk_extract(tmp_path, ("if (pass == 1) __syncthreads();", ""))
+    mutant = build_harness(tmp_path, "wk_kernel_harness")
+    c = small_config(3, 8)
+    amp = W.pupil_mask(c)
+    yx = O.valid_list(amp, c.n, c.min_illum)
+    ph = W.phase_frames(c, 0, range(1))
+    want, wimg = O.measure(ph, amp, yx, c.n, c.P, c.b, tau=0.1, stage=2)
+    caught = 0
+    for order in (0, 1, 2):
+        out = wk_run(mutant, tmp_path, c, 1, yx, 0, 0.1, ph, amp, None, 0, order, 9)
+        try:
+            assert out is not None
+            compare(out[0], out[1], want, wimg, 0.1, 0, "mutant")
+        except AssertionError:
+            caught += 1
+    assert caught >= 1
