@@ -6,8 +6,16 @@
  * tests/test_kernels_host.py) with the headers they include compiled as they are, on the coroutine SIMT machine of
  * simt.h -- every thread of every CTA, its shared memory, __syncthreads and half-warp shuffles.
  *
+ * Likewise wkf_kernel of csrc/wk_fft.cu (config 5's kernel, and what SHWFS_ALGO_AUTO gives one- and two-frame calls at
+ * n = 8, 10: the autocorrelation by 32-point FFTs, a half-warp per spot, six steps on one shared-memory tile fenced
+ * by __syncwarp only), cut out as "wkf_kernel_extract.inc": the one-tile-per-CTA register-gather instances and the
+ * persistent TMA instance with its dynamic deal.  Its table row staging (mrow_stage / mrow_wait of wk_common.cuh:
+ * 2n-1 cp.async copies of 8 bytes, inline PTX) is restated below as the plain copies it performs.
+ *
  * usage: wk_kernel_harness in.bin out.bin
- *   in.bin   int32[12] {N, n, P, b, T, nsub, mode, has_k, generic, order, seed, L}, float[2] {tau, c_phi},
+ *   in.bin   int32[14] {N, n, P, b, T, nsub, mode, has_k, kernel, order, seed, L, grid, lazy_tma}, float[2] {tau, c_phi},
+ *            kernel: 0 wk_measure_kernel, 1 wk_generic_kernel, 2 wkf_kernel (one tile per CTA), 3 wkf_kernel (TMA,
+ *            persistent, `grid` CTAs)
  *            float sod_q[8], sod_sw[8], phase[T*(L>1 ? L : 1)*N*N] (L > 1: one wavefront per sub-layer), amp[N*N],
  *            int32 valid[nsub*2] (sy, sx), float K[has_k ? nsub*P*P : 0], float sod_g[L*nsub*2]
  *   out.bin  slopes[T*nsub*2], binned[T*nsub*D*D]
@@ -22,13 +30,23 @@
 #include "../../paper_1408_0698_b200/csrc/cog.cuh"
 #include "../../paper_1408_0698_b200/csrc/noise.cuh"
 #include "../../paper_1408_0698_b200/csrc/wk_common.cuh"
+#include "../../paper_1408_0698_b200/csrc/sweep.cuh"
 
 namespace {
 using namespace shwfs;
 #include "wk_kernel_extract.inc"
 
+/* what the cp.async copies of mrow_stage do: entry k of the staged row is M_i[term_lag(k)][ly] */
+template <int n>
+void host_mrow_stage(const float2 *Mcol, float *dst)
+{
+    for (int k = 0; k < 2 * n - 1; ++k) reinterpret_cast<float2 *>(dst)[k] = Mcol[term_lag<n>(k) * n];
+}
+inline void host_mrow_wait() {}
+#include "wkf_kernel_extract.inc"
+
 struct Job {
-    int N, n, P, b, T, nsub, mode, has_k, generic, order, seed, L;
+    int N, n, P, b, T, nsub, mode, has_k, kernel, order, seed, L, grid, lazy;
     float tau, c_phi;
     float sod_q[8], sod_sw[8];
 };
@@ -49,6 +67,24 @@ bool special(const Job &J, const WkArgs &A)
     if (A.L > 0) return A.mode == 0 ? run<n, 0, 1>(J, A) : run<n, 1, 1>(J, A);
     return A.mode == 0 ? run<n, 0, 0>(J, A) : run<n, 1, 0>(J, A);
 }
+
+template <int n, int MODE>
+bool run_wkf(const Job &J, const WkArgs &A, const CUtensorMap *map)
+{
+    if constexpr (n == 16) {
+        if (J.kernel == 3)
+            return simt::launch(J.grid, WF_THREADS, WF_SMEM + WF_STAGE + 1024, (simt::Order)J.order, (unsigned)J.seed,
+                                [&]() { wkf_kernel<n, MODE, 0, true>(A, *map); });
+    }
+    return simt::launch((A.total + WF_SPOTS - 1) / WF_SPOTS, WF_THREADS, WF_SMEM, (simt::Order)J.order, (unsigned)J.seed,
+                        [&]() { wkf_kernel<n, MODE, 0, false>(A, *map); });
+}
+
+template <int n>
+bool wkf(const Job &J, const WkArgs &A, const CUtensorMap *map)
+{
+    return A.mode == 0 ? run_wkf<n, 0>(J, A, map) : run_wkf<n, 1>(J, A, map);
+}
 }  // namespace
 
 int main(int argc, char **argv)
@@ -58,7 +94,7 @@ int main(int argc, char **argv)
     FILE *f = std::fopen(argv[1], "rb");
     if (!f) return 2;
     Job J;
-    if (std::fread(&J, 4, 12, f) != 12 || std::fread(&J.tau, 4, 18, f) != 18) return 2;
+    if (std::fread(&J, 4, 14, f) != 14 || std::fread(&J.tau, 4, 18, f) != 18) return 2;
     const int D = J.P / J.b, LX = 2 * J.n - 1, layers = J.L > 1 ? J.L : 1;
     const size_t NN = (size_t)J.N * J.N, total = (size_t)J.T * J.nsub;
     std::vector<float> phase(NN * J.T * layers), amp(NN), K(J.has_k ? (size_t)J.nsub * J.P * J.P : 0);
@@ -93,8 +129,40 @@ int main(int argc, char **argv)
     A.turns = (float)((double)J.c_phi / 6.283185307179586476925286766559);
     A.ramp_unit = 0.5f / (float)J.P;
 
+    /* the patch table and chunk counters of the handle (api.cu, shwfs_create) */
+    std::vector<int2> patch(J.nsub);
+    for (int i = 0; i < J.nsub; ++i) {
+        const int y0 = valid[i].x * J.n, x0 = valid[i].y * J.n;
+        bool lit = true;
+        for (int j = 0; j < J.n && lit; ++j)
+            for (int k = 0; k < J.n; ++k)
+                if (amp[(size_t)(y0 + j) * J.N + x0 + k] != 1.0f) { lit = false; break; }
+        patch[i] = make_int2(x0 | (lit ? SHWFS_PATCH_LIT : 0), y0);
+    }
+    int sched[2] = {0, 0};
+    A.patch = patch.data();
+    A.sched = sched;
+    CUtensorMap map;
+    std::memset(&map, 0, sizeof(map));
+    const simt::TmaMap tm{phase.data(), J.N, J.T, 16};
+    std::memcpy(&map, &tm, sizeof(tm));
+    simt::lazy_tma = J.lazy != 0;
+
     bool ok = false;
-    if (J.generic) {
+    if (J.kernel >= 2) {
+        if (D != 16 || (J.kernel == 3 && J.n != 16)) { std::printf("FAIL: no such instance\n"); return 1; }
+        switch (J.n) {
+        case 8: ok = wkf<8>(J, A, &map); break;
+        case 10: ok = wkf<10>(J, A, &map); break;
+        case 12: ok = wkf<12>(J, A, &map); break;
+        case 14: ok = wkf<14>(J, A, &map); break;
+        case 16: ok = wkf<16>(J, A, &map); break;
+        default: return 2;
+        }
+        if (sched[0] != 0 || sched[1] != 0) { std::printf("FAIL: chunk counters not re-armed\n"); return 1; }
+        if (!simt::g_pending.empty()) { std::printf("FAIL: a requested box was never waited for\n"); return 1; }
+        if (J.kernel == 3 && simt::g_boxes != (long)total) { std::printf("FAIL: %ld boxes for %zu spots\n", simt::g_boxes, total); return 1; }
+    } else if (J.kernel == 1) {
         const size_t smem = sizeof(float2) * (size_t)(J.n * J.n + J.n * LX + D) + sizeof(float) * (size_t)(D * D + 3 * GEN_THREADS);
         ok = simt::launch(A.total, GEN_THREADS, smem, (simt::Order)J.order, (unsigned)J.seed,
                           [&]() { wk_generic_kernel(A, J.n, D); });

@@ -181,6 +181,20 @@ def test_pruned_fft_kernel_whole_on_the_host(tmp_path):
 
 # ---------------------------------------------------------------- wk.cu: table kernel + the headline kernel
 
+def wkf_extract(tmp_path: Path, mutate=None) -> None:
+    src = (CSRC / "wk_fft.cu").read_text()
+    block = cut(src, "constexpr int WF_ROWS = 16;", "template <int n, int MODE, int EXTK, bool TMA>\ncudaError_t launch_wkf_inst")
+    block, k1 = re.subn(r"extern __shared__ __align__\(16\) unsigned char wf_smem\[\];", "unsigned char *wf_smem = simt::smem();", block)
+    # the table row staging is inline PTX (cp.async): the harness restates its copies
+    block, k2 = re.subn(r"\bmrow_stage<n>\(", "host_mrow_stage<n>(", block)
+    block, k3 = re.subn(r"\bmrow_wait\(\)", "host_mrow_wait()", block)
+    assert (k1, k2, k3) == (1, 1, 1) and "wkf_kernel(const WkArgs A" in block
+    if mutate is not None:
+        assert block.count(mutate[0]) == 1, mutate[0]
+        block = block.replace(mutate[0], mutate[1])
+    (tmp_path / "wkf_kernel_extract.inc").write_text(block)
+
+
 def wk_extract(tmp_path: Path, mutate=None) -> None:
     src = (CSRC / "wk.cu").read_text()
     block = cut(src, "__global__ void wk_table_kernel(", "template <int n, int MODE, int EXTK>\ncudaError_t launch_special_mode")
@@ -192,13 +206,16 @@ def wk_extract(tmp_path: Path, mutate=None) -> None:
         assert block.count(mutate[0]) == 1, mutate[0]
         block = block.replace(mutate[0], mutate[1])
     (tmp_path / "wk_kernel_extract.inc").write_text(block)
+    wkf_extract(tmp_path)
 
 
-def wk_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, generic, order, seed, L=0, sod_q=(), sod_sw=(), sod_g=None):
+def wk_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, kernel, order, seed, L=0, sod_q=(), sod_sw=(), sod_g=None,
+           grid=0, lazy=0):
+    """kernel: 0 wk_measure_kernel, 1 wk_generic_kernel, 2 wkf_kernel one tile per CTA, 3 wkf_kernel persistent (TMA)."""
     nsub = len(yx)
     fin, fout = tmp_path / "in.bin", tmp_path / "out.bin"
     with open(fin, "wb") as f:
-        f.write(struct.pack("12i", c.N, c.n, c.P, c.b, T, nsub, mode, int(K is not None), generic, order, seed, L))
+        f.write(struct.pack("14i", c.N, c.n, c.P, c.b, T, nsub, mode, int(K is not None), kernel, order, seed, L, grid, lazy))
         f.write(struct.pack("2f", tau, 1.0))
         f.write(np.resize(np.asarray(list(sod_q) + [0.0] * 8, np.float32), 8).tobytes())
         f.write(np.resize(np.asarray(list(sod_sw) + [0.0] * 8, np.float32), 8).tobytes())
@@ -273,6 +290,66 @@ def test_lag_domain_kernels_whole_on_the_host(tmp_path):
     caught = 0
     for order in (0, 1, 2):
         out = wk_run(mutant, tmp_path, c, 1, yx, 0, 0.1, ph, amp, None, 0, order, 9)
+        try:
+            assert out is not None
+            compare(out[0], out[1], want, wimg, 0.1, 0, "mutant")
+        except AssertionError:
+            caught += 1
+    assert caught >= 1
+
+
+# ---------------------------------------------------------------- wk_fft.cu: autocorrelation by FFT (config 5's kernel)
+
+WKF_CASES = [
+    # base config, S, T, mode, tau, elongation kernels, n override, instances [(kernel, grid, lazy)]
+    (5, 6, 5, 0, 0.10, True, None, [(2, 0, 0), (3, 2, 0), (3, 3, 1)]),    # n = 16, P = 64, b = 4: ldg, persistent TMA
+    (3, 8, 2, 0, 0.10, True, None, [(2, 0, 0)]),                          # n = 10: what AUTO gives a two-frame call
+    (1, 10, 1, 1, 0.05, False, None, [(2, 0, 0)]),                        # config 1 itself, n = 8, hard threshold
+    (5, 6, 1, 0, 0.10, True, 12, [(2, 0, 0)]),                            # n = 12 (threads r >= n idle), P = 64
+    (2, 6, 1, 0, 0.10, False, 14, [(2, 0, 0)]),                           # n = 14, P = 32, shared table
+]
+
+
+@needs_toolchain
+def test_fft_autocorrelation_kernel_whole_on_the_host(tmp_path):
+    wk_extract(tmp_path)
+    exe = build_harness(tmp_path, "wk_kernel_harness")
+    runs = 0
+    for base, S, T, mode, tau, with_k, n_over, instances in WKF_CASES:
+        c = W.CONFIGS[1] if (base, S) == (1, 10) else small_config(base, S)
+        if n_over is not None:
+            c = dataclasses.replace(c, n=n_over, N=S * n_over, r_out=0.5 * S * n_over * c.dx,
+                                    r_in=0.5 * S * n_over * c.dx * W.CONFIGS[base].r_in / W.CONFIGS[base].r_out)
+        amp = W.pupil_mask(c)
+        yx = O.valid_list(amp, c.n, c.min_illum)
+        ph = W.phase_frames(c, 0, range(T))
+        K = W.elongation_kernels(c, 0, yx) if with_k else None
+        want, wimg = O.measure(ph, amp, yx, c.n, c.P, c.b, tau=tau, mode=mode, kernels=K, stage=2)
+        for kernel, grid, lazy in instances:
+            first = None
+            for order in (0, 1, 2):
+                label = f"config {base} S={S} n={c.n} kernel={kernel} grid={grid} lazy={lazy} order={order}"
+                out = wk_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, kernel, order, 55 + runs, grid=grid, lazy=lazy)
+                assert out is not None, label
+                compare(out[0], out[1], want, wimg, tau, mode, label)
+                if first is None:
+                    first = out
+                else:
+                    assert np.array_equal(first[0], out[0]) and np.array_equal(first[1], out[1]), f"{label}: depends on the thread order"
+                runs += 1
+    assert runs == 21
+
+    # a missing __syncwarp between step C (every thread writes its two columns of g) and step D (a thread reads a row)
+    wkf_extract(tmp_path, ("    }   /* sub-layers */\n    __syncwarp();", "    }   /* sub-layers */\n"))
+    mutant = build_harness(tmp_path, "wk_kernel_harness")
+    c = small_config(5, 6)
+    amp = W.pupil_mask(c)
+    yx = O.valid_list(amp, c.n, c.min_illum)
+    ph = W.phase_frames(c, 0, range(1))
+    want, wimg = O.measure(ph, amp, yx, c.n, c.P, c.b, tau=0.1, stage=2)
+    caught = 0
+    for order in (0, 1, 2):
+        out = wk_run(mutant, tmp_path, c, 1, yx, 0, 0.1, ph, amp, None, 2, order, 9)
         try:
             assert out is not None
             compare(out[0], out[1], want, wimg, 0.1, 0, "mutant")
