@@ -356,3 +356,98 @@ def test_fft_autocorrelation_kernel_whole_on_the_host(tmp_path):
         except AssertionError:
             caught += 1
     assert caught >= 1
+
+
+# ---------------------------------------------------------------- literal.cu: the chain as the paper words it
+
+def lit_extract(tmp_path: Path, mutate=None) -> None:
+    src = (CSRC / "literal.cu").read_text()
+    block = cut(src, "constexpr int LIT_THREADS = 128;", "template <int P, int NZ>\ncudaError_t launch_literal")
+    block, k1 = re.subn(r"extern __shared__ __align__\(16\) float2 lit_smem\[\];",
+                        "float2 *lit_smem = reinterpret_cast<float2 *>(simt::smem());", block)
+    block, k2 = re.subn(r"extern __shared__ double2 ksm\[\];", "double2 *ksm = reinterpret_cast<double2 *>(simt::smem());", block)
+    assert (k1, k2) == (1, 1) and "literal_kernel(const LitArgs A)" in block and "literal_khat_kernel(" in block
+    if mutate is not None:
+        assert block.count(mutate[0]) == 1, mutate[0]
+        block = block.replace(mutate[0], mutate[1])
+    (tmp_path / "lit_kernel_extract.inc").write_text(block)
+
+
+def lit_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, stage, order, seed):
+    nsub = len(yx)
+    fin, fout = tmp_path / "in.bin", tmp_path / "out.bin"
+    with open(fin, "wb") as f:
+        f.write(struct.pack("12i", c.N, c.n, c.P, c.b, T, nsub, mode, int(K is not None), stage, order, seed, 0))
+        f.write(struct.pack("2f", tau, 1.0))
+        f.write(np.ascontiguousarray(ph, np.float32).tobytes())
+        f.write(np.ascontiguousarray(amp, np.float32).tobytes())
+        f.write(np.ascontiguousarray(yx, np.int32).tobytes())
+        if K is not None:
+            f.write(np.ascontiguousarray(K, np.float32).tobytes())
+    r = subprocess.run([str(exe), str(fin), str(fout)], capture_output=True, text=True, timeout=900)
+    if r.returncode != 0 or not r.stdout.startswith("ok "):
+        assert r.stdout.startswith("FAIL"), r.stdout[-500:] + r.stderr[-500:]
+        return None
+    raw = np.fromfile(fout, np.float32)
+    side = c.P // c.b if stage == 2 else c.P
+    ns = T * nsub * 2
+    return raw[:ns].reshape(T, nsub, 2).astype(np.float64), raw[ns:].reshape(T, nsub, side, side).astype(np.float64)
+
+
+LIT_CASES = [
+    # base config, S, T, mode, tau, elongation kernels, stages
+    (3, 8, 2, 0, 0.10, True, (2, 1)),     # n = 10, P = 32 <32,32>: binned image and the convolved image before binning
+    (2, 6, 1, 1, 0.10, False, (2, 0)),    # n = 16, P = 32 <32,16>: no kernels, hard threshold; stage 0 = intensity
+    (1, 10, 3, 0, 0.0, False, (2,)),      # config 1 itself: P = 16 <16,8>, two spots per warp
+    (5, 4, 1, 0, 0.10, True, (2,)),       # P = 64 <64,32>: two warps per spot, reductions through shared memory
+]
+
+
+@needs_toolchain
+def test_literal_chain_kernels_whole_on_the_host(tmp_path):
+    lit_extract(tmp_path)
+    exe = build_harness(tmp_path, "lit_kernel_harness")
+    runs = 0
+    for base, S, T, mode, tau, with_k, stages in LIT_CASES:
+        c = W.CONFIGS[1] if (base, S) == (1, 10) else small_config(base, S)
+        amp = W.pupil_mask(c)
+        yx = O.valid_list(amp, c.n, c.min_illum)
+        ph = W.phase_frames(c, 0, range(T))
+        K = W.elongation_kernels(c, 0, yx) if with_k else None
+        for stage in stages:
+            want, wimg = O.measure(ph, amp, yx, c.n, c.P, c.b, tau=tau, mode=mode, kernels=K, stage=stage)
+            first = None
+            for order in (0, 1, 2):
+                label = f"config {base} S={S} stage={stage} order={order}"
+                out = lit_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, stage, order, 77 + runs)
+                assert out is not None, label
+                if stage == 2:
+                    compare(out[0], out[1], want, wimg, tau, mode, label)
+                else:
+                    peak = wimg.max(axis=(2, 3), keepdims=True)
+                    assert float((np.abs(out[1] - wimg) / peak).max()) <= 1e-4, label
+                if first is None:
+                    first = out
+                else:
+                    assert np.array_equal(first[0], out[0]) and np.array_equal(first[1], out[1]), f"{label}: depends on the thread order"
+                runs += 1
+    assert runs == 18
+
+    # without the barrier between the centred image written to shared memory and the binning that reads it
+    lit_extract(tmp_path, ("    for (int v = 0; v < P; ++v) Sh[(v ^ HP) * LD + (r ^ HP)] = re[v];\n    __syncthreads();",
+                           "    for (int v = 0; v < P; ++v) Sh[(v ^ HP) * LD + (r ^ HP)] = re[v];\n"))
+    mutant = build_harness(tmp_path, "lit_kernel_harness")
+    c = small_config(3, 8)
+    amp = W.pupil_mask(c)
+    yx = O.valid_list(amp, c.n, c.min_illum)
+    ph = W.phase_frames(c, 0, range(1))
+    want, wimg = O.measure(ph, amp, yx, c.n, c.P, c.b, tau=0.1, stage=2)
+    caught = 0
+    for order in (0, 1, 2):
+        out = lit_run(mutant, tmp_path, c, 1, yx, 0, 0.1, ph, amp, None, 2, order, 9)
+        try:
+            assert out is not None
+            compare(out[0], out[1], want, wimg, 0.1, 0, "mutant")
+        except AssertionError:
+            caught += 1
+    assert caught >= 1
