@@ -114,14 +114,11 @@ static uint32_t shuffle(uint32_t v, int src)
     return t->warp->slot[b][src & 31];
 }
 
-/* Runs body() once per thread of a grid x block launch with smem_bytes of dynamic shared memory per CTA (zero filled,
- * 1 KB aligned slack included).  Returns false if the threads dead-lock (a barrier not reached by everybody). */
-static bool launch(int grid, int block, size_t smem_bytes, Order order, unsigned seed, const std::function<void()> &body,
-                   size_t stack_bytes = 256 * 1024)
+/* Runs body() once per thread of the CTAs `bids` (all resident at once) with smem_bytes of dynamic shared memory per
+ * CTA (zero filled).  Returns false if the threads dead-lock (a barrier not reached by everybody). */
+static bool run_ctas(const std::vector<Dim> &bids, int block, size_t smem_bytes, Order order, unsigned seed, size_t stack_bytes)
 {
-    g_block = {(unsigned)block, 1, 1};
-    g_grid = {(unsigned)grid, 1, 1};
-    g_body = body;
+    const int grid = (int)bids.size();
     const int wpc = (block + 31) / 32;
     std::vector<Cta> ctas(grid);
     std::vector<Thread> th((size_t)grid * block);
@@ -132,7 +129,7 @@ static bool launch(int grid, int block, size_t smem_bytes, Order order, unsigned
         for (int t = 0; t < block; ++t) {
             Thread &T = th[(size_t)c * block + t];
             T.tid = {(unsigned)t, 0, 0};
-            T.bid = {(unsigned)c, 0, 0};
+            T.bid = bids[c];
             T.cta = &ctas[c];
             T.warp = &ctas[c].warps[t / 32];
             T.lane = t % 32;
@@ -170,6 +167,37 @@ static bool launch(int grid, int block, size_t smem_bytes, Order order, unsigned
         else idle_rounds = 0;
     }
     for (Thread &T : th) std::free(T.stack);
+    return true;
+}
+
+/* a 1-D launch, every CTA resident from the start (what the persistent kernels' grids are sized for) */
+static bool launch(int grid, int block, size_t smem_bytes, Order order, unsigned seed, const std::function<void()> &body,
+                   size_t stack_bytes = 256 * 1024)
+{
+    g_block = {(unsigned)block, 1, 1};
+    g_grid = {(unsigned)grid, 1, 1};
+    g_body = body;
+    std::vector<Dim> bids(grid);
+    for (int c = 0; c < grid; ++c) bids[c] = {(unsigned)c, 0, 0};
+    return run_ctas(bids, block, smem_bytes, order, seed, stack_bytes);
+}
+
+/* a 2-D launch in waves of `wave` CTAs (CTAs of these kernels never wait for one another) */
+static bool launch2d(int gx, int gy, int block, size_t smem_bytes, Order order, unsigned seed, const std::function<void()> &body,
+                     int wave = 16, size_t stack_bytes = 256 * 1024)
+{
+    g_block = {(unsigned)block, 1, 1};
+    g_grid = {(unsigned)gx, (unsigned)gy, 1};
+    g_body = body;
+    std::vector<Dim> bids;
+    for (int y = 0; y < gy; ++y)
+        for (int x = 0; x < gx; ++x) {
+            bids.push_back({(unsigned)x, (unsigned)y, 0});
+            if ((int)bids.size() == wave || (y == gy - 1 && x == gx - 1)) {
+                if (!run_ctas(bids, block, smem_bytes, order, seed + (unsigned)(y * gx + x), stack_bytes)) return false;
+                bids.clear();
+            }
+        }
     return true;
 }
 

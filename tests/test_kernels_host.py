@@ -451,3 +451,91 @@ def test_literal_chain_kernels_whole_on_the_host(tmp_path):
         except AssertionError:
             caught += 1
     assert caught >= 1
+
+
+# ---------------------------------------------------------------- pyramid.cu: the five kernels of a pyramid call
+
+def pyr_extract(tmp_path: Path, mutate=None) -> None:
+    src = (CSRC / "pyramid.cu").read_text()
+    block = cut(src, "constexpr int PY_LINES = 8;", "template <int R>\ncudaError_t run_chunk")
+    block, k1 = re.subn(r"extern __shared__ __align__\(16\) float2 py_smem\[\];",
+                        "float2 *py_smem = reinterpret_cast<float2 *>(simt::smem());", block)
+    block, k2 = re.subn(r"__shared__ float red\[256\];", "float *red = reinterpret_cast<float *>(simt::smem());", block)
+    assert (k1, k2) == (3, 1) and "pyr_cols_kernel(const PyArgs A)" in block
+    if mutate is not None:
+        assert block.count(mutate[0]) == 1, mutate[0]
+        block = block.replace(mutate[0], mutate[1])
+    (tmp_path / "pyr_kernel_extract.inc").write_text(block)
+
+
+def pyr_run(exe, tmp_path, ph, amp, yx, Np, s, bp, r_mod, K, D_pix, c_phi, order, seed):
+    T, N, _ = ph.shape
+    Sp = N // bp
+    fin, fout = tmp_path / "in.bin", tmp_path / "out.bin"
+    with open(fin, "wb") as f:
+        f.write(struct.pack("10i", N, Np, s, bp, K, T, len(yx), order, seed, 0))
+        f.write(struct.pack("3f", r_mod, D_pix, c_phi))
+        f.write(np.ascontiguousarray(ph, np.float32).tobytes())
+        f.write(np.ascontiguousarray(amp, np.float32).tobytes())
+        f.write(np.ascontiguousarray(yx, np.int32).tobytes())
+    r = subprocess.run([str(exe), str(fin), str(fout)], capture_output=True, text=True, timeout=900)
+    if r.returncode != 0 or not r.stdout.startswith("ok "):
+        assert r.stdout.startswith("FAIL"), r.stdout[-500:] + r.stderr[-500:]
+        return None
+    raw = np.fromfile(fout, np.float32)
+    ns = T * len(yx) * 2
+    return raw[:ns].reshape(T, len(yx), 2).astype(np.float64), raw[ns:].reshape(T, 2, 2, Sp, Sp).astype(np.float64)
+
+
+@needs_toolchain
+def test_pyramid_kernels_whole_on_the_host(tmp_path):
+    from oracle import pyramid as OP
+    pyr_extract(tmp_path)
+    exe = build_harness(tmp_path, "pyr_kernel_harness")
+    rng = np.random.default_rng(92)
+    cases = []
+    p = W.PYRAMIDS["tiny"]                                  # N = 48, Np = 256 (16 x 16 four-step), 8 modulation points
+    cases.append((W.pyramid_frames(p, range(2)), W.pyramid_mask(p), p.Np, p.s, p.bp, p.r_mod, p.K, p.D_pix, 1.0, 0.5, (0, 1, 2)))
+    # N not a multiple of the 8-line CTA, partially transmitting mask, phase_to_rad != 1, Np = 1024 (32 x 32 four-step)
+    N = 44
+    ax = np.arange(N) + 0.5 - N / 2
+    amp = ((np.hypot(ax[None, :], ax[:, None]) <= N / 2) * rng.uniform(0.4, 1.0, (N, N))).astype(np.float32)
+    cases.append((rng.normal(0, 2.0, (1, N, N)).astype(np.float32), amp, 1024, 200, 4, 1.5, 2, 0.9 * N, 0.6, 0.3, (2,)))
+    # unmodulated
+    N = 36
+    ax = np.arange(N) + 0.5 - N / 2
+    amp = (np.hypot(ax[None, :], ax[:, None]) <= N / 2).astype(np.float32)
+    cases.append((rng.normal(0, 1.0, (1, N, N)).astype(np.float32), amp, 256, 64, 2, 0.0, 0, float(N), 1.0, 0.5, (1,)))
+    runs = 0
+    for ph, amp, Np, s, bp, r_mod, K, D_pix, c_phi, min_illum, orders in cases:
+        yx = OP.valid_pixels(amp, bp, min_illum)
+        want, wq = OP.measure(ph, amp, yx, Np, s, bp, r_mod, K, D_pix, c_phi=np.float32(c_phi), return_quadrants=True)
+        first = None
+        for order in orders:
+            label = f"pyramid N={ph.shape[-1]} Np={Np} K={K} order={order}"
+            out = pyr_run(exe, tmp_path, ph, amp, yx, Np, s, bp, r_mod, K, D_pix, c_phi, order, 14 + runs)
+            assert out is not None, label
+            got, q = out
+            assert not np.isnan(q).any() and not np.isnan(got).any(), label
+            assert np.abs(q - wq).max() <= 1e-4 * wq.max(), (label, np.abs(q - wq).max() / wq.max())     # tests/test_pyramid_gpu.py
+            assert np.abs(got - want).max() <= 2e-4, (label, np.abs(got - want).max())
+            if first is None:
+                first = out
+            else:
+                assert np.array_equal(first[0], got) and np.array_equal(first[1], q), f"{label}: depends on the thread order"
+            runs += 1
+    assert runs == 5
+
+    # the exchange inside a line transform without its __syncwarp between the writes and the reads
+    pyr_extract(tmp_path, ("    __syncwarp();\n#pragma unroll\n    for (int jj = 0; jj < R; jj += 2) {",
+                           "#pragma unroll\n    for (int jj = 0; jj < R; jj += 2) {"))
+    mutant = build_harness(tmp_path, "pyr_kernel_harness")
+    ph, amp, Np, s, bp, r_mod, K, D_pix, c_phi, min_illum, _ = cases[2]
+    yx = OP.valid_pixels(amp, bp, min_illum)
+    want, wq = OP.measure(ph, amp, yx, Np, s, bp, r_mod, K, D_pix, c_phi=np.float32(c_phi), return_quadrants=True)
+    caught = 0
+    for order in (0, 1, 2):
+        out = pyr_run(mutant, tmp_path, ph, amp, yx, Np, s, bp, r_mod, K, D_pix, c_phi, order, 3)
+        if out is None or np.isnan(out[1]).any() or not np.abs(out[1] - wq).max() <= 1e-4 * wq.max():
+            caught += 1
+    assert caught >= 1
