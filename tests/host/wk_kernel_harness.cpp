@@ -16,9 +16,10 @@
  *   in.bin   int32[14] {N, n, P, b, T, nsub, mode, has_k, kernel, order, seed, L, grid, lazy_tma}, float[2] {tau, c_phi},
  *            kernel: 0 wk_measure_kernel, 1 wk_generic_kernel, 2 wkf_kernel (one tile per CTA), 3 wkf_kernel (TMA,
  *            persistent, `grid` CTAs)
- *            float sod_q[8], sod_sw[8], phase[T*(L>1 ? L : 1)*N*N] (L > 1: one wavefront per sub-layer), amp[N*N],
+ *            float sod_q[8], sod_sw[8], phase[T*(L > 0 && !shared ? L : 1)*N*N], amp[N*N],
  *            int32 valid[nsub*2] (sy, sx), float K[has_k ? nsub*P*P : 0], float sod_g[L*nsub*2]
- *   out.bin  slopes[T*nsub*2], binned[T*nsub*D*D]
+ *            after sod_sw: float[2] {flux, ron}, int32[4] {shared wavefront, photon_model, seed low, seed high}
+ *   out.bin  slopes[T*nsub*2], binned[T*nsub*D*D], noisy[flux > 0 ? T*nsub*D*D : 0]
  * What the harness supplies itself is what the launchers (host code of wk.cu) do: the WkArgs and the grids.
  * The comparison with the float64 oracle is the Python test's.  Test infrastructure only.
  */
@@ -49,6 +50,9 @@ struct Job {
     int N, n, P, b, T, nsub, mode, has_k, kernel, order, seed, L, grid, lazy;
     float tau, c_phi;
     float sod_q[8], sod_sw[8];
+    float flux, ron;
+    int shared, photon_model;
+    unsigned seed_lo, seed_hi;
 };
 
 template <int n, int MODE, int EXTK>
@@ -64,13 +68,22 @@ template <int n>
 bool special(const Job &J, const WkArgs &A)
 {
     if (A.L > 1) return A.mode == 0 ? run<n, 0, 2>(J, A) : run<n, 1, 2>(J, A);
-    if (A.L > 0) return A.mode == 0 ? run<n, 0, 1>(J, A) : run<n, 1, 1>(J, A);
+    if (A.L > 0 || A.flux > 0.f) return A.mode == 0 ? run<n, 0, 1>(J, A) : run<n, 1, 1>(J, A);
     return A.mode == 0 ? run<n, 0, 0>(J, A) : run<n, 1, 0>(J, A);
+}
+
+template <int n, int MODE, int EXTK>
+bool run_wkf_ext(const Job &J, const WkArgs &A, const CUtensorMap *map)
+{
+    return simt::launch((A.total + WF_SPOTS - 1) / WF_SPOTS, WF_THREADS, EXTK == 2 ? 2 * WF_SMEM : WF_SMEM, (simt::Order)J.order,
+                        (unsigned)J.seed, [&]() { wkf_kernel<n, MODE, EXTK, false>(A, *map); });
 }
 
 template <int n, int MODE>
 bool run_wkf(const Job &J, const WkArgs &A, const CUtensorMap *map)
 {
+    if (A.L > 1) return run_wkf_ext<n, MODE, 2>(J, A, map);
+    if (A.L > 0 || A.flux > 0.f) return run_wkf_ext<n, MODE, 1>(J, A, map);
     if constexpr (n == 16) {
         if (J.kernel == 3)
             return simt::launch(J.grid, WF_THREADS, WF_SMEM + WF_STAGE + 1024, (simt::Order)J.order, (unsigned)J.seed,
@@ -94,8 +107,8 @@ int main(int argc, char **argv)
     FILE *f = std::fopen(argv[1], "rb");
     if (!f) return 2;
     Job J;
-    if (std::fread(&J, 4, 14, f) != 14 || std::fread(&J.tau, 4, 18, f) != 18) return 2;
-    const int D = J.P / J.b, LX = 2 * J.n - 1, layers = J.L > 1 ? J.L : 1;
+    if (std::fread(&J, 4, 14, f) != 14 || std::fread(&J.tau, 4, 24, f) != 24) return 2;
+    const int D = J.P / J.b, LX = 2 * J.n - 1, layers = J.L > 0 && !J.shared ? J.L : 1;
     const size_t NN = (size_t)J.N * J.N, total = (size_t)J.T * J.nsub;
     std::vector<float> phase(NN * J.T * layers), amp(NN), K(J.has_k ? (size_t)J.nsub * J.P * J.P : 0);
     std::vector<int2> valid(J.nsub);
@@ -122,7 +135,12 @@ int main(int argc, char **argv)
     A.frame_stride = (long long)NN;
     A.sod_g = sod_g.data(); A.L = J.L;
     for (int l = 0; l < 8; ++l) { A.sod_q[l] = J.sod_q[l]; A.sod_sw[l] = J.sod_sw[l]; }
-    if (J.L > 1) { A.layer_stride = A.frame_stride; A.frame_stride *= J.L; }
+    if (J.L > 0 && !J.shared) { A.layer_stride = A.frame_stride; A.frame_stride *= J.L; }
+    std::vector<float> noisy(J.flux > 0.f ? total * D * D : 0, NAN);
+    A.flux = J.flux; A.ron2 = J.ron * J.ron; A.photon_model = J.photon_model;
+    A.key = make_uint2(J.seed_lo, J.seed_hi);
+    A.t0 = 0;
+    A.noisy = J.flux > 0.f ? noisy.data() : nullptr;
     A.T = J.T; A.N = J.N; A.nsub = J.nsub; A.mstride = J.has_k ? LX * J.n : 0;
     A.total = (int)total; A.mode = J.mode;
     A.tau = J.tau;
@@ -181,6 +199,7 @@ int main(int argc, char **argv)
     if (!f) return 2;
     std::fwrite(slopes.data(), 4, slopes.size(), f);
     std::fwrite(binned.data(), 4, binned.size(), f);
+    std::fwrite(noisy.data(), 4, noisy.size(), f);
     std::fclose(f);
     std::printf("ok switches %ld\n", simt::g_switches);
     return 0;

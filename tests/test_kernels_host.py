@@ -23,10 +23,6 @@ CSRC = ROOT / "paper_1408_0698_b200" / "csrc"
 CUDA_INC = Path("/usr/local/cuda/include")
 PATCH_LIT = 1 << 30
 
-needs_toolchain = pytest.mark.skipif(shutil.which("g++") is None or not (CUDA_INC / "cuda_runtime.h").exists(),
-                                     reason="needs g++ and the CUDA headers")
-
-
 def small_config(base: int, S: int, **kw) -> W.WfsConfig:
     """The geometry of config `base` on S x S subapertures: same n, P, b, pixel size and wavelength; the pupil radii
     scaled to the smaller grid so that fully lit, partially lit and dark subapertures all occur."""
@@ -44,13 +40,50 @@ def cut(src: str, begin: str, end: str) -> str:
     return block
 
 
-def build_harness(tmp_path: Path, name: str) -> Path:
-    exe = tmp_path / name
-    r = subprocess.run(["g++", "-std=c++17", "-O0", "-ffp-contract=off", f"-I{CUDA_INC}", f"-I{tmp_path}",
-                        "-Wno-attributes", "-Wno-psabi", "-o", str(exe), str(ROOT / "tests" / "host" / f"{name}.cpp")],
-                       capture_output=True, text=True, timeout=900)
-    assert r.returncode == 0, r.stderr[-3000:]
-    return exe
+MUTANTS = {
+    # the machine does see a missing barrier: each entry removes one the kernel needs
+    "pf_mut": ("pf", ("__syncwarp();                                      /* rows visible; the staging slot has been read */", "")),
+    "wk_mut": ("wk", ("if (pass == 1) __syncthreads();", "")),
+    "wkf_mut": ("wkf", ("    }   /* sub-layers */\n    __syncwarp();", "    }   /* sub-layers */\n")),
+    "lit_mut": ("lit", ("    for (int v = 0; v < P; ++v) Sh[(v ^ HP) * LD + (r ^ HP)] = re[v];\n    __syncthreads();",
+                        "    for (int v = 0; v < P; ++v) Sh[(v ^ HP) * LD + (r ^ HP)] = re[v];\n")),
+    "pyr_mut": ("pyr", ("    __syncwarp();\n#pragma unroll\n    for (int jj = 0; jj < R; jj += 2) {",
+                        "#pragma unroll\n    for (int jj = 0; jj < R; jj += 2) {")),
+}
+
+
+@pytest.fixture(scope="module")
+def harnesses(tmp_path_factory):
+    """Every harness and every mutant, each in a directory of its own with the kernel text cut out for it, compiled
+    side by side (g++ -O0 -ffp-contract=off: the fmaf calls of the shims are the only contractions)."""
+    if shutil.which("g++") is None or not (CUDA_INC / "cuda_runtime.h").exists():
+        pytest.skip("needs g++ and the CUDA headers")
+    jobs = {}
+    for key in ("pf", "wk", "lit", "pyr", *MUTANTS):
+        base, mutate = MUTANTS.get(key, (key, None))
+        d = tmp_path_factory.mktemp(key)
+        if base == "pf":
+            pf_extract(d, mutate)
+        elif base == "wk":
+            wk_extract(d, mutate)
+        elif base == "wkf":
+            wk_extract(d, None, mutate)
+        elif base == "lit":
+            lit_extract(d, mutate)
+        else:
+            pyr_extract(d, mutate)
+        name = {"pf": "pf", "wk": "wk", "wkf": "wk", "lit": "lit", "pyr": "pyr"}[base] + "_kernel_harness"
+        exe = d / name
+        proc = subprocess.Popen(["g++", "-std=c++17", "-O0", "-ffp-contract=off", f"-I{CUDA_INC}", f"-I{d}", "-Wno-attributes",
+                                 "-Wno-psabi", "-o", str(exe), str(ROOT / "tests" / "host" / f"{name}.cpp")],
+                                stdout=subprocess.DEVNULL, stderr=subprocess.PIPE, text=True)
+        jobs[key] = (proc, exe)
+    out = {}
+    for key, (proc, exe) in jobs.items():
+        _, err = proc.communicate(timeout=900)
+        assert proc.returncode == 0, key + ": " + err[-3000:]
+        out[key] = exe
+    return out
 
 
 def patch_table(amp: np.ndarray, yx: np.ndarray, n: int) -> np.ndarray:
@@ -122,10 +155,8 @@ def pf_run(exe, tmp_path, c, T, nsub, mode, tau, ph, amp, table, tma, chunk, laz
     return got, img, r.stdout
 
 
-@needs_toolchain
-def test_pruned_fft_kernel_whole_on_the_host(tmp_path):
-    pf_extract(tmp_path)
-    exe = build_harness(tmp_path, "pf_kernel_harness")
+def test_pruned_fft_kernel_whole_on_the_host(tmp_path, harnesses):
+    exe = harnesses["pf"]
 
     runs = 0
     for base, S, T, mode, tau, instances in PF_CASES:
@@ -164,8 +195,7 @@ def test_pruned_fft_kernel_whole_on_the_host(tmp_path):
     # the machine does see a missing barrier: without the __syncwarp between the row pass and the column pass the
     # register-gather instance reads rows nobody has written yet (wrong images), and the TMA instance re-arms a
     # staging slot other lanes still wait for (the launch hangs)
-    pf_extract(tmp_path, ("__syncwarp();                                      /* rows visible; the staging slot has been read */", ""))
-    mutant = build_harness(tmp_path, "pf_kernel_harness")
+    mutant = harnesses["pf_mut"]
     c = small_config(2, 6)
     amp = W.pupil_mask(c)
     yx = O.valid_list(amp, c.n, c.min_illum)
@@ -195,7 +225,7 @@ def wkf_extract(tmp_path: Path, mutate=None) -> None:
     (tmp_path / "wkf_kernel_extract.inc").write_text(block)
 
 
-def wk_extract(tmp_path: Path, mutate=None) -> None:
+def wk_extract(tmp_path: Path, mutate=None, mutate_fft=None) -> None:
     src = (CSRC / "wk.cu").read_text()
     block = cut(src, "__global__ void wk_table_kernel(", "template <int n, int MODE, int EXTK>\ncudaError_t launch_special_mode")
     block, k1 = re.subn(r"extern __shared__ double2 tmp\[\];", "double2 *tmp = reinterpret_cast<double2 *>(simt::smem());", block)
@@ -206,11 +236,11 @@ def wk_extract(tmp_path: Path, mutate=None) -> None:
         assert block.count(mutate[0]) == 1, mutate[0]
         block = block.replace(mutate[0], mutate[1])
     (tmp_path / "wk_kernel_extract.inc").write_text(block)
-    wkf_extract(tmp_path)
+    wkf_extract(tmp_path, mutate_fft)
 
 
 def wk_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, kernel, order, seed, L=0, sod_q=(), sod_sw=(), sod_g=None,
-           grid=0, lazy=0):
+           grid=0, lazy=0, shared=1, flux=0.0, ron=0.0, noise_seed=0, photon_model=0):
     """kernel: 0 wk_measure_kernel, 1 wk_generic_kernel, 2 wkf_kernel one tile per CTA, 3 wkf_kernel persistent (TMA)."""
     nsub = len(yx)
     fin, fout = tmp_path / "in.bin", tmp_path / "out.bin"
@@ -219,6 +249,7 @@ def wk_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, kernel, order, seed, 
         f.write(struct.pack("2f", tau, 1.0))
         f.write(np.resize(np.asarray(list(sod_q) + [0.0] * 8, np.float32), 8).tobytes())
         f.write(np.resize(np.asarray(list(sod_sw) + [0.0] * 8, np.float32), 8).tobytes())
+        f.write(struct.pack("2f2i2I", flux, ron, shared, photon_model, noise_seed & 0xffffffff, noise_seed >> 32))
         f.write(np.ascontiguousarray(ph, np.float32).tobytes())
         f.write(np.ascontiguousarray(amp, np.float32).tobytes())
         f.write(np.ascontiguousarray(yx, np.int32).tobytes())
@@ -232,8 +263,11 @@ def wk_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, kernel, order, seed, 
         return None
     raw = np.fromfile(fout, np.float32)
     D = c.P // c.b
-    ns = T * nsub * 2
-    return raw[:ns].reshape(T, nsub, 2).astype(np.float64), raw[ns:].reshape(T, nsub, D, D).astype(np.float64)
+    ns, ni = T * nsub * 2, T * nsub * D * D
+    out = (raw[:ns].reshape(T, nsub, 2).astype(np.float64), raw[ns:ns + ni].reshape(T, nsub, D, D).astype(np.float64))
+    if flux > 0:
+        out += (raw[ns + ni:].reshape(T, nsub, D, D).astype(np.float64),)
+    return out
 
 
 WK_CASES = [
@@ -245,10 +279,8 @@ WK_CASES = [
 ]
 
 
-@needs_toolchain
-def test_lag_domain_kernels_whole_on_the_host(tmp_path):
-    wk_extract(tmp_path)
-    exe = build_harness(tmp_path, "wk_kernel_harness")
+def test_lag_domain_kernels_whole_on_the_host(tmp_path, harnesses):
+    exe = harnesses["wk"]
     runs = 0
     for base, S, T, mode, tau, with_k, generic_too in WK_CASES:
         c = W.CONFIGS[1] if (base, S) == (1, 10) else small_config(base, S)
@@ -280,8 +312,7 @@ def test_lag_domain_kernels_whole_on_the_host(tmp_path):
     # the barrier the round-1 review worried about: the second-pass rows of H overwrite the field buffer "behind one
     # __syncthreads()" -- without it a warp that finishes its lag row early destroys field rows other warps still
     # read, and the machine shows it (wrong images under at least one thread order)
-    wk_extract(tmp_path, ("if (pass == 1) __syncthreads();", ""))
-    mutant = build_harness(tmp_path, "wk_kernel_harness")
+    mutant = harnesses["wk_mut"]
     c = small_config(3, 8)
     amp = W.pupil_mask(c)
     yx = O.valid_list(amp, c.n, c.min_illum)
@@ -310,10 +341,8 @@ WKF_CASES = [
 ]
 
 
-@needs_toolchain
-def test_fft_autocorrelation_kernel_whole_on_the_host(tmp_path):
-    wk_extract(tmp_path)
-    exe = build_harness(tmp_path, "wk_kernel_harness")
+def test_fft_autocorrelation_kernel_whole_on_the_host(tmp_path, harnesses):
+    exe = harnesses["wk"]
     runs = 0
     for base, S, T, mode, tau, with_k, n_over, instances in WKF_CASES:
         c = W.CONFIGS[1] if (base, S) == (1, 10) else small_config(base, S)
@@ -340,8 +369,7 @@ def test_fft_autocorrelation_kernel_whole_on_the_host(tmp_path):
     assert runs == 21
 
     # a missing __syncwarp between step C (every thread writes its two columns of g) and step D (a thread reads a row)
-    wkf_extract(tmp_path, ("    }   /* sub-layers */\n    __syncwarp();", "    }   /* sub-layers */\n"))
-    mutant = build_harness(tmp_path, "wk_kernel_harness")
+    mutant = harnesses["wkf_mut"]
     c = small_config(5, 6)
     amp = W.pupil_mask(c)
     yx = O.valid_list(amp, c.n, c.min_illum)
@@ -403,10 +431,8 @@ LIT_CASES = [
 ]
 
 
-@needs_toolchain
-def test_literal_chain_kernels_whole_on_the_host(tmp_path):
-    lit_extract(tmp_path)
-    exe = build_harness(tmp_path, "lit_kernel_harness")
+def test_literal_chain_kernels_whole_on_the_host(tmp_path, harnesses):
+    exe = harnesses["lit"]
     runs = 0
     for base, S, T, mode, tau, with_k, stages in LIT_CASES:
         c = W.CONFIGS[1] if (base, S) == (1, 10) else small_config(base, S)
@@ -434,9 +460,7 @@ def test_literal_chain_kernels_whole_on_the_host(tmp_path):
     assert runs == 18
 
     # without the barrier between the centred image written to shared memory and the binning that reads it
-    lit_extract(tmp_path, ("    for (int v = 0; v < P; ++v) Sh[(v ^ HP) * LD + (r ^ HP)] = re[v];\n    __syncthreads();",
-                           "    for (int v = 0; v < P; ++v) Sh[(v ^ HP) * LD + (r ^ HP)] = re[v];\n"))
-    mutant = build_harness(tmp_path, "lit_kernel_harness")
+    mutant = harnesses["lit_mut"]
     c = small_config(3, 8)
     amp = W.pupil_mask(c)
     yx = O.valid_list(amp, c.n, c.min_illum)
@@ -487,11 +511,9 @@ def pyr_run(exe, tmp_path, ph, amp, yx, Np, s, bp, r_mod, K, D_pix, c_phi, order
     return raw[:ns].reshape(T, len(yx), 2).astype(np.float64), raw[ns:].reshape(T, 2, 2, Sp, Sp).astype(np.float64)
 
 
-@needs_toolchain
-def test_pyramid_kernels_whole_on_the_host(tmp_path):
+def test_pyramid_kernels_whole_on_the_host(tmp_path, harnesses):
     from oracle import pyramid as OP
-    pyr_extract(tmp_path)
-    exe = build_harness(tmp_path, "pyr_kernel_harness")
+    exe = harnesses["pyr"]
     rng = np.random.default_rng(92)
     cases = []
     p = W.PYRAMIDS["tiny"]                                  # N = 48, Np = 256 (16 x 16 four-step), 8 modulation points
@@ -527,9 +549,7 @@ def test_pyramid_kernels_whole_on_the_host(tmp_path):
     assert runs == 5
 
     # the exchange inside a line transform without its __syncwarp between the writes and the reads
-    pyr_extract(tmp_path, ("    __syncwarp();\n#pragma unroll\n    for (int jj = 0; jj < R; jj += 2) {",
-                           "#pragma unroll\n    for (int jj = 0; jj < R; jj += 2) {"))
-    mutant = build_harness(tmp_path, "pyr_kernel_harness")
+    mutant = harnesses["pyr_mut"]
     ph, amp, Np, s, bp, r_mod, K, D_pix, c_phi, min_illum, _ = cases[2]
     yx = OP.valid_pixels(amp, bp, min_illum)
     want, wq = OP.measure(ph, amp, yx, Np, s, bp, r_mod, K, D_pix, c_phi=np.float32(c_phi), return_quadrants=True)
@@ -539,3 +559,77 @@ def test_pyramid_kernels_whole_on_the_host(tmp_path):
         if out is None or np.isnan(out[1]).any() or not np.abs(out[1] - wq).max() <= 1e-4 * wq.max():
             caught += 1
     assert caught >= 1
+
+
+# ---------------------------------------------------------------- the paper's full LGS model on the EXT instances
+
+def sodium_tables(c, yx, sod):
+    """What shwfs_set_sodium (api.cu, host code, float64) puts into the handle: curvature per pixel^2, sqrt of the
+    weights, and the local gradient of each sub-layer's analytic phase per subaperture, whole turns dropped."""
+    two_pi = 2.0 * np.pi
+    a = np.asarray(sod["defocus"], np.float64)
+    yc = ((yx[:, 0] + 0.5) * c.n - 0.5 * c.N) * c.dx
+    xc = ((yx[:, 1] + 0.5) * c.n - 0.5 * c.N) * c.dx
+    gx = (2.0 * a[:, None] * (xc[None, :] - sod["cx"]) + np.asarray(sod["tilt_x"])[:, None]) * c.dx / two_pi
+    gy = (2.0 * a[:, None] * (yc[None, :] - sod["cy"]) + np.asarray(sod["tilt_y"])[:, None]) * c.dx / two_pi
+    g = np.stack([gx - np.rint(gx), gy - np.rint(gy)], axis=2).astype(np.float32)          # [L][nsub][2]
+    return (a * c.dx * c.dx / two_pi).astype(np.float32), np.sqrt(np.asarray(sod["weight"])).astype(np.float32), g
+
+
+def test_sodium_layers_and_noise_instances_whole_on_the_host(tmp_path, harnesses):
+    """wk_measure_kernel<10,0,2> / <10,0,1> and wkf_kernel<10,0,2,ldg> / <10,0,1,ldg>: several sodium sub-layers with
+    their own or a shared wavefront, and Gaussian-limit detector noise before the centroid (f2),
+    against oracle/shwfs_oracle_lgs.c -- the MAORY geometry of config 3 at the real distance from the launch point."""
+    exe = harnesses["wk"]
+    c = small_config(3, 8)
+    amp = W.pupil_mask(c)
+    yx = O.valid_list(amp, c.n, c.min_illum)
+    K = W.spot_size_kernels(c, yx)
+    runs = 0
+    for L, shared, T in ((3, False, 2), (5, True, 1)):
+        sod = W.sodium_layers(W.CONFIGS[3], 0, L)              # launch point 19.5 m away: the elongation of the pupil edge
+        ph = W.phase_frames(c, 0, range(T)) if shared else \
+            np.stack([W.phase_frames(c, 0, range(10 * l, 10 * l + T)) for l in range(L)], axis=1)
+        kw = dict(weight=sod["weight"], defocus=sod["defocus"], tilt_x=sod["tilt_x"], tilt_y=sod["tilt_y"],
+                  cx=sod["cx"], cy=sod["cy"], tau=c.tau, kernels=K)
+        want, wimg = O.measure_lgs(ph, amp, yx, c.n, c.P, c.b, c.dx, stage=2, **kw)
+        plain = O.measure(ph if shared else ph[:, 0], amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K)
+        assert np.abs(want - plain).max() > 0.05                # the sub-layers do change the spots
+        q, sw, g = sodium_tables(c, yx, sod)
+        for kernel in (0, 2):
+            first = None
+            for order in (0, 2):
+                label = f"L={L} shared={shared} kernel={kernel} order={order}"
+                out = wk_run(exe, tmp_path, c, T, yx, 0, c.tau, ph, amp, K, kernel, order, 31 + runs, L=L, sod_q=q, sod_sw=sw,
+                             sod_g=g, shared=int(shared))
+                assert out is not None, label
+                compare(out[0], out[1], want, wimg, c.tau, 0, label)
+                if first is None:
+                    first = out
+                else:
+                    assert np.array_equal(first[0], out[0]) and np.array_equal(first[1], out[1]), label
+                runs += 1
+    # detector noise (Gaussian limit of the photon noise + read noise, Philox per (seed, t, i, pixel)) on 3 shared sub-layers
+    L, T = 3, 2
+    sod = W.sodium_layers(W.CONFIGS[3], 0, L)
+    ph = W.phase_frames(c, 0, range(T))
+    F, ron, seed = 500.0 / c.n ** 2, 3.0, 0x1408069800000091
+    kw = dict(weight=sod["weight"], defocus=sod["defocus"], tilt_x=sod["tilt_x"], tilt_y=sod["tilt_y"],
+              cx=sod["cx"], cy=sod["cy"], tau=c.tau, kernels=K)
+    want, wimg = O.measure_lgs(ph, amp, yx, c.n, c.P, c.b, c.dx, flux=F, ron=ron, seed=seed, stage=3, **kw)
+    clean = O.measure_lgs(ph, amp, yx, c.n, c.P, c.b, c.dx, **kw)
+    assert np.abs(want - clean).max() > 0.05
+    q, sw, g = sodium_tables(c, yx, sod)
+    for kernel, Lk in ((0, L), (2, L), (0, 0)):
+        if Lk == 0:                                             # noise on the plain single-layer sensor: instance <n,0,1>
+            want, wimg = O.measure_lgs(ph, amp, yx, c.n, c.P, c.b, c.dx, weight=[1.0], defocus=[0.0], tau=c.tau, kernels=K,
+                                       flux=F, ron=ron, seed=seed, stage=3)
+        out = wk_run(exe, tmp_path, c, T, yx, 0, c.tau, ph, amp, K, kernel, 2, 77, L=Lk, sod_q=q, sod_sw=sw,
+                     sod_g=g if Lk else None, shared=1, flux=F, ron=ron, noise_seed=seed)
+        assert out is not None
+        label = f"noise kernel={kernel} L={Lk}"
+        peak = wimg.max(axis=(2, 3), keepdims=True)
+        assert float((np.abs(out[2] - wimg) / peak).max()) <= 1e-4, label
+        assert float(np.abs(out[0] - want).max()) <= 1e-3, label
+        runs += 1
+    assert runs == 11
