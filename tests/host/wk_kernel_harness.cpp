@@ -18,7 +18,8 @@
  *            persistent, `grid` CTAs)
  *            float sod_q[8], sod_sw[8], phase[T*(L > 0 && !shared ? L : 1)*N*N], amp[N*N],
  *            int32 valid[nsub*2] (sy, sx), float K[has_k ? nsub*P*P : 0], float sod_g[L*nsub*2]
- *            after sod_sw: float[2] {flux, ron}, int32[4] {shared wavefront, photon_model, seed low, seed high}
+ *            after sod_sw: float[2] {flux, ron}, int32[5] {shared wavefront, photon_model, seed low, seed high, has_dm};
+ *            after sod_g: float dm_patch[has_dm ? T*nsub*n*n : 0] (subtracted from the wavefront in H1)
  *   out.bin  slopes[T*nsub*2], binned[T*nsub*D*D], noisy[flux > 0 ? T*nsub*D*D : 0]
  * What the harness supplies itself is what the launchers (host code of wk.cu) do: the WkArgs and the grids.
  * The comparison with the float64 oracle is the Python test's.  Test infrastructure only.
@@ -53,6 +54,7 @@ struct Job {
     float flux, ron;
     int shared, photon_model;
     unsigned seed_lo, seed_hi;
+    int has_dm;
 };
 
 template <int n, int MODE, int EXTK>
@@ -68,7 +70,7 @@ template <int n>
 bool special(const Job &J, const WkArgs &A)
 {
     if (A.L > 1) return A.mode == 0 ? run<n, 0, 2>(J, A) : run<n, 1, 2>(J, A);
-    if (A.L > 0 || A.flux > 0.f) return A.mode == 0 ? run<n, 0, 1>(J, A) : run<n, 1, 1>(J, A);
+    if (A.L > 0 || A.flux > 0.f || A.dm_patch != nullptr) return A.mode == 0 ? run<n, 0, 1>(J, A) : run<n, 1, 1>(J, A);
     return A.mode == 0 ? run<n, 0, 0>(J, A) : run<n, 1, 0>(J, A);
 }
 
@@ -83,7 +85,7 @@ template <int n, int MODE>
 bool run_wkf(const Job &J, const WkArgs &A, const CUtensorMap *map)
 {
     if (A.L > 1) return run_wkf_ext<n, MODE, 2>(J, A, map);
-    if (A.L > 0 || A.flux > 0.f) return run_wkf_ext<n, MODE, 1>(J, A, map);
+    if (A.L > 0 || A.flux > 0.f || A.dm_patch != nullptr) return run_wkf_ext<n, MODE, 1>(J, A, map);
     if constexpr (n == 16) {
         if (J.kernel == 3)
             return simt::launch(J.grid, WF_THREADS, WF_SMEM + WF_STAGE + 1024, (simt::Order)J.order, (unsigned)J.seed,
@@ -107,7 +109,7 @@ int main(int argc, char **argv)
     FILE *f = std::fopen(argv[1], "rb");
     if (!f) return 2;
     Job J;
-    if (std::fread(&J, 4, 14, f) != 14 || std::fread(&J.tau, 4, 24, f) != 24) return 2;
+    if (std::fread(&J, 4, 14, f) != 14 || std::fread(&J.tau, 4, 25, f) != 25) return 2;
     const int D = J.P / J.b, LX = 2 * J.n - 1, layers = J.L > 0 && !J.shared ? J.L : 1;
     const size_t NN = (size_t)J.N * J.N, total = (size_t)J.T * J.nsub;
     std::vector<float> phase(NN * J.T * layers), amp(NN), K(J.has_k ? (size_t)J.nsub * J.P * J.P : 0);
@@ -116,6 +118,8 @@ int main(int argc, char **argv)
     if (std::fread(phase.data(), 4, phase.size(), f) != phase.size() || std::fread(amp.data(), 4, NN, f) != NN ||
         std::fread(valid.data(), 8, valid.size(), f) != valid.size() || std::fread(K.data(), 4, K.size(), f) != K.size() ||
         std::fread(sod_g.data(), 8, sod_g.size(), f) != sod_g.size()) return 2;
+    std::vector<float> dm_patch(J.has_dm ? total * J.n * J.n : 0);      /* [T][nsub][n*n], as dm_phase_kernel leaves it */
+    if (std::fread(dm_patch.data(), 4, dm_patch.size(), f) != dm_patch.size()) return 2;
     std::fclose(f);
 
     /* H0: as shwfs_wk_build_table launches it */
@@ -141,6 +145,7 @@ int main(int argc, char **argv)
     A.key = make_uint2(J.seed_lo, J.seed_hi);
     A.t0 = 0;
     A.noisy = J.flux > 0.f ? noisy.data() : nullptr;
+    A.dm_patch = J.has_dm ? dm_patch.data() : nullptr;
     A.T = J.T; A.N = J.N; A.nsub = J.nsub; A.mstride = J.has_k ? LX * J.n : 0;
     A.total = (int)total; A.mode = J.mode;
     A.tau = J.tau;

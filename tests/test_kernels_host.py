@@ -47,6 +47,7 @@ MUTANTS = {
     "wkf_mut": ("wkf", ("    }   /* sub-layers */\n    __syncwarp();", "    }   /* sub-layers */\n")),
     "lit_mut": ("lit", ("    for (int v = 0; v < P; ++v) Sh[(v ^ HP) * LD + (r ^ HP)] = re[v];\n    __syncthreads();",
                         "    for (int v = 0; v < P; ++v) Sh[(v ^ HP) * LD + (r ^ HP)] = re[v];\n")),
+    "loop_mut": ("loop", ("        __syncthreads();                                    /* stage (ch & 1) is refilled two chunks later */", "")),
     "pyr_mut": ("pyr", ("    __syncwarp();\n#pragma unroll\n    for (int jj = 0; jj < R; jj += 2) {",
                         "#pragma unroll\n    for (int jj = 0; jj < R; jj += 2) {")),
 }
@@ -59,7 +60,7 @@ def harnesses(tmp_path_factory):
     if shutil.which("g++") is None or not (CUDA_INC / "cuda_runtime.h").exists():
         pytest.skip("needs g++ and the CUDA headers")
     jobs = {}
-    for key in ("pf", "wk", "lit", "pyr", *MUTANTS):
+    for key in ("pf", "wk", "lit", "pyr", "loop", *MUTANTS):
         base, mutate = MUTANTS.get(key, (key, None))
         d = tmp_path_factory.mktemp(key)
         if base == "pf":
@@ -70,9 +71,11 @@ def harnesses(tmp_path_factory):
             wk_extract(d, None, mutate)
         elif base == "lit":
             lit_extract(d, mutate)
+        elif base == "loop":
+            loop_extract(d, mutate)
         else:
             pyr_extract(d, mutate)
-        name = {"pf": "pf", "wk": "wk", "wkf": "wk", "lit": "lit", "pyr": "pyr"}[base] + "_kernel_harness"
+        name = {"pf": "pf", "wk": "wk", "wkf": "wk", "lit": "lit", "pyr": "pyr", "loop": "loop"}[base] + "_kernel_harness"
         exe = d / name
         proc = subprocess.Popen(["g++", "-std=c++17", "-O0", "-ffp-contract=off", f"-I{CUDA_INC}", f"-I{d}", "-Wno-attributes",
                                  "-Wno-psabi", "-o", str(exe), str(ROOT / "tests" / "host" / f"{name}.cpp")],
@@ -240,7 +243,7 @@ def wk_extract(tmp_path: Path, mutate=None, mutate_fft=None) -> None:
 
 
 def wk_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, kernel, order, seed, L=0, sod_q=(), sod_sw=(), sod_g=None,
-           grid=0, lazy=0, shared=1, flux=0.0, ron=0.0, noise_seed=0, photon_model=0):
+           grid=0, lazy=0, shared=1, flux=0.0, ron=0.0, noise_seed=0, photon_model=0, dm_patch=None):
     """kernel: 0 wk_measure_kernel, 1 wk_generic_kernel, 2 wkf_kernel one tile per CTA, 3 wkf_kernel persistent (TMA)."""
     nsub = len(yx)
     fin, fout = tmp_path / "in.bin", tmp_path / "out.bin"
@@ -249,7 +252,8 @@ def wk_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, kernel, order, seed, 
         f.write(struct.pack("2f", tau, 1.0))
         f.write(np.resize(np.asarray(list(sod_q) + [0.0] * 8, np.float32), 8).tobytes())
         f.write(np.resize(np.asarray(list(sod_sw) + [0.0] * 8, np.float32), 8).tobytes())
-        f.write(struct.pack("2f2i2I", flux, ron, shared, photon_model, noise_seed & 0xffffffff, noise_seed >> 32))
+        f.write(struct.pack("2f2i2Ii", flux, ron, shared, photon_model, noise_seed & 0xffffffff, noise_seed >> 32,
+                            int(dm_patch is not None)))
         f.write(np.ascontiguousarray(ph, np.float32).tobytes())
         f.write(np.ascontiguousarray(amp, np.float32).tobytes())
         f.write(np.ascontiguousarray(yx, np.int32).tobytes())
@@ -257,6 +261,8 @@ def wk_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, kernel, order, seed, 
             f.write(np.ascontiguousarray(K, np.float32).tobytes())
         if sod_g is not None:
             f.write(np.ascontiguousarray(sod_g, np.float32).tobytes())
+        if dm_patch is not None:
+            f.write(np.ascontiguousarray(dm_patch, np.float32).tobytes())
     r = subprocess.run([str(exe), str(fin), str(fout)], capture_output=True, text=True, timeout=900)
     if r.returncode != 0 or not r.stdout.startswith("ok "):
         assert r.stdout.startswith("FAIL"), r.stdout[-500:] + r.stderr[-500:]
@@ -633,3 +639,108 @@ def test_sodium_layers_and_noise_instances_whole_on_the_host(tmp_path, harnesses
         assert float(np.abs(out[0] - want).max()) <= 1e-3, label
         runs += 1
     assert runs == 11
+
+
+# ---------------------------------------------------------------- loop.cu: the closed-loop neighbours (FP32 kernels)
+
+def loop_extract(tmp_path: Path, mutate=None) -> None:
+    src = (CSRC / "loop.cu").read_text()
+    block = src[src.index("/* modes[M][N][N] -> out[nsub][M][n*n]: block = (subaperture, mode) */"):
+                src.index("}  // namespace\n\ncudaError_t shwfs_loop_relayout_modes")]
+    block, k = re.subn(r"template <[^>]*>\nvoid launch_dm_\w+\(.*?\n}\n", "", block, flags=re.S)     # the launchers between the kernels
+    assert k == 3 and "<<<" not in block
+    block, k1 = re.subn(r"extern __shared__ __align__\(16\) float dm_smem\[\];", "float *dm_smem = reinterpret_cast<float *>(simt::smem());", block)
+    block, k2 = re.subn(r"extern __shared__ float gv_coef\[\];", "float *gv_coef = reinterpret_cast<float *>(simt::smem());", block)
+    block, k3 = re.subn(r"__shared__ float part\[RC_THREADS / 32\]\[RC_TT\];",
+                        "float (*part)[RC_TT] = reinterpret_cast<float (*)[RC_TT]>(simt::smem());", block)
+    assert (k1, k2, k3) == (1, 1, 1) and "recon_kernel(" in block and "dm_phase_kernel(" in block
+    if mutate is not None:
+        assert block.count(mutate[0]) == 1, mutate[0]
+        block = block.replace(mutate[0], mutate[1])
+    (tmp_path / "loop_kernel_extract.inc").write_text(block)
+
+
+def loop_run(exe, tmp_path, c, yx, modes, coef, R, slopes, gain, variant, order, seed, lazy):
+    T, M = coef.shape
+    nsub = len(yx)
+    fin, fout = tmp_path / "in.bin", tmp_path / "out.bin"
+    with open(fin, "wb") as f:
+        f.write(struct.pack("10i", c.N, c.n, nsub, M, T, variant, order, seed, lazy, M))
+        f.write(struct.pack("f", gain))
+        for a, dt in ((modes, np.float32), (yx, np.int32), (coef, np.float32), (R, np.float32), (slopes, np.float32)):
+            f.write(np.ascontiguousarray(a, dt).tobytes())
+    r = subprocess.run([str(exe), str(fin), str(fout)], capture_output=True, text=True, timeout=900)
+    if r.returncode != 0 or not r.stdout.startswith("ok "):
+        assert r.stdout.startswith("FAIL"), r.stdout[-500:] + r.stderr[-500:]
+        return None
+    raw = np.fromfile(fout, np.float32)
+    npatch = T * nsub * c.n * c.n
+    return (raw[:npatch].reshape(T, nsub, c.n, c.n).astype(np.float64), raw[npatch:npatch + T * M].reshape(T, M).astype(np.float64),
+            raw[npatch + T * M:].reshape(T, M).astype(np.float64))
+
+
+def test_closed_loop_kernels_whole_on_the_host(tmp_path, harnesses):
+    """relayout_modes_kernel + dm_phase_kernel / dm_phase_gemv_kernel / dm_phase_simple_kernel against the definition
+    C1 (oracle/closed_loop.py: the DM phase sum_m c[t,m] mode[m], here on the patches), recon_kernel against C2 and the
+    integrator update, and the residual measured by wk_measure_kernel<10,0,1> / wkf_kernel<10,0,1,ldg> with that DM
+    phase subtracted in the gather against oracle measure_residual."""
+    from oracle import closed_loop as OL
+    exe = harnesses["loop"]
+    c = small_config(3, 8)
+    amp = W.pupil_mask(c)
+    yx = O.valid_list(amp, c.n, c.min_illum)
+    nsub, M = len(yx), 37                                    # M neither a multiple of the 16-mode chunk nor of 8
+    rng = np.random.default_rng(76)
+    modes = W.dm_modes(c, M)
+    R = rng.normal(0, 0.05, (M, 2 * nsub)).astype(np.float32)
+    runs = 0
+    for T, variant, lazy, orders in ((1, 0, 0, (0, 2)), (3, 0, 0, (1,)), (7, 1, 1, (0, 2)), (19, 0, 1, (0, 1, 2)), (37, 1, 0, (2,)), (2, 2, 0, (2,))):
+        coef = rng.normal(0, 0.5, (T, M)).astype(np.float32)
+        slopes = rng.normal(0, 0.3, (T, 2 * nsub)).astype(np.float32)
+        # C1 on the patches, float64
+        full = np.einsum("tm,myx->tyx", coef.astype(np.float64), modes.astype(np.float64))
+        want_patch = np.stack([full[:, sy * c.n:(sy + 1) * c.n, sx * c.n:(sx + 1) * c.n] for sy, sx in yx], axis=1)
+        d = OL.reconstruct(R, slopes.reshape(T, nsub, 2))
+        want_coef = coef.astype(np.float64) + 0.4 * d
+        first = None
+        for order in orders:
+            label = f"T={T} variant={variant} lazy={lazy} order={order}"
+            out = loop_run(exe, tmp_path, c, yx, modes, coef, R, slopes, 0.4, variant, order, 5 + runs, lazy)
+            assert out is not None, label
+            patch, coef_after, hist = out
+            assert not np.isnan(patch).any(), label
+            assert np.abs(patch - want_patch).max() <= 2e-5 * np.abs(want_patch).max(), (label, np.abs(patch - want_patch).max())
+            assert np.array_equal(hist, coef.astype(np.float64)), label            # reading C4: the coefficients before the update
+            assert np.abs(coef_after - want_coef).max() <= 1e-5, (label, np.abs(coef_after - want_coef).max())
+            if first is None:
+                first = out
+            else:
+                assert all(np.array_equal(a, b) for a, b in zip(first, out)), f"{label}: depends on the thread order"
+            runs += 1
+    assert runs == 10
+
+    # the residual through the sensor: the DM phase of dm_phase_kernel subtracted in the gather (EXT instance)
+    T = 2
+    ph = W.phase_frames(c, 0, range(T))
+    coef = rng.normal(0, 0.5, (T, M)).astype(np.float32)
+    K = W.elongation_kernels(c, 0, yx)
+    patch = loop_run(exe, tmp_path, c, yx, modes, coef, R, np.zeros((T, 2 * nsub), np.float32), 0.0, 1, 2, 3, 1)[0]
+    want, wimg = OL.measure_residual(ph, modes, coef, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K, stage=2)
+    for kernel in (0, 2):
+        out = wk_run(harnesses["wk"], tmp_path, c, T, yx, 0, c.tau, ph, amp, K, kernel, 2, 8, dm_patch=patch)
+        assert out is not None
+        compare(out[0], out[1], want, wimg, c.tau, 0, f"residual kernel={kernel}")
+
+    # the double buffer of dm_phase_kernel without the barrier in front of its refill: with the copies completing as
+    # late as the hardware may (lazy) and as early (eager), some thread order reads a stage another thread refills
+    mutant = harnesses["loop_mut"]
+    T = 19
+    coef = rng.normal(0, 0.5, (T, M)).astype(np.float32)
+    full = np.einsum("tm,myx->tyx", coef.astype(np.float64), modes.astype(np.float64))
+    want_patch = np.stack([full[:, sy * c.n:(sy + 1) * c.n, sx * c.n:(sx + 1) * c.n] for sy, sx in yx], axis=1)
+    caught = 0
+    for order, lazy in ((0, 0), (1, 0), (2, 0), (2, 1)):
+        out = loop_run(mutant, tmp_path, c, yx, modes, coef, R, np.zeros((T, 2 * nsub), np.float32), 0.0, 1, order, 3, lazy)
+        if out is None or not np.abs(out[0] - want_patch).max() <= 2e-5 * np.abs(want_patch).max():
+            caught += 1
+    assert caught >= 1
