@@ -744,3 +744,46 @@ def test_closed_loop_kernels_whole_on_the_host(tmp_path, harnesses):
         if out is None or not np.abs(out[0] - want_patch).max() <= 2e-5 * np.abs(want_patch).max():
             caught += 1
     assert caught >= 1
+
+
+@pytest.mark.parametrize("flux_total,ron", [(300.0, 0.0), (40000.0, 2.0)])
+def test_poisson_noise_instance_whole_on_the_host(tmp_path, harnesses, flux_total, ron):
+    """photon_model = 1 inside the kernels (add_noise_col16 of noise.cuh as wk_measure_kernel<10,0,1> and
+    wkf_kernel<10,0,1,ldg> call it: pixel pairs, Philox counters and lanes as on the device), the statement of
+    tests/test_lgs_gpu.py::test_config3_poisson_noise_matches_oracle: on every pixel whose draw the oracle reports as
+    decided by more than rounding the count is the oracle's (exactly without read noise), the others differ by at most
+    one count (inversion) or stay within 8 sigma (rejection), and spots whose image agrees have the oracle's slopes."""
+    c = small_config(3, 8)
+    amp = W.pupil_mask(c)
+    yx = O.valid_list(amp, c.n, c.min_illum)
+    K = W.elongation_kernels(c, 0, yx)
+    T = 2
+    ph = W.phase_frames(c, 0, range(T))
+    F, seed = flux_total / c.n ** 2, 0x14080698000000A7
+    kw = dict(weight=[1.0], defocus=[0.0], tau=c.tau, kernels=K, flux=F, ron=ron, seed=seed, photon_model=1)
+    want, wimg, margin = O.measure_lgs(ph, amp, yx, c.n, c.P, c.b, c.dx, stage=3, want_margins=True, **kw)
+    _, clean_img = O.measure_lgs(ph, amp, yx, c.n, c.P, c.b, c.dx, weight=[1.0], defocus=[0.0], tau=c.tau, kernels=K, stage=2)
+    rate = np.maximum(F * clean_img, 0.0)
+    assert (rate >= 30).any() == (flux_total > 1000)                  # which branch the case exercises
+    clear = margin > 1e-4 + 1e-5 * rate                               # _poisson_clear of tests/test_lgs_gpu.py
+    assert clear.mean() > 0.95
+    for kernel in (0, 2):
+        out = wk_run(harnesses["wk"], tmp_path, c, T, yx, 0, c.tau, ph, amp, K, kernel, 2, 21, flux=F, ron=ron,
+                     noise_seed=seed, photon_model=1)
+        assert out is not None
+        got, _, img = out
+        d = np.abs(img - wimg)
+        if ron == 0.0:
+            assert np.all(img == np.round(img)) and img.min() >= 0
+            assert np.all(d[clear] == 0.0), (kernel, d[clear].max(), int((d[clear] > 0).sum()))
+        else:
+            pk = wimg.max(axis=(2, 3), keepdims=True)
+            assert (d / pk)[clear].max() <= 1e-4, (kernel, (d / pk)[clear].max())
+        low = ~clear & (rate < 29.9)
+        assert d[low].max(initial=0.0) <= 1.0 + 1e-3
+        high = ~clear & (rate >= 29.9)
+        assert np.all(d[high] <= 8.0 * np.sqrt(rate[high]) + 2.0)
+        same = (d <= (1e-6 if ron == 0.0 else 1e-4 * wimg.max(axis=(2, 3), keepdims=True))).all(axis=(2, 3))
+        assert same.mean() > 0.05
+        assert np.abs(got - want)[same].max() <= 1e-3, (kernel, np.abs(got - want)[same].max())
+        assert (d > 0.5).mean() <= 2.0 * (~clear).mean() + 1e-4
