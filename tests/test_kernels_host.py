@@ -787,3 +787,20 @@ def test_poisson_noise_instance_whole_on_the_host(tmp_path, harnesses, flux_tota
         assert same.mean() > 0.05
         assert np.abs(got - want)[same].max() <= 1e-3, (kernel, np.abs(got - want)[same].max())
         assert (d > 0.5).mean() <= 2.0 * (~clear).mean() + 1e-4
+
+
+def test_config3_whole_frame_headline_kernel_on_the_host(tmp_path, harnesses):
+    """One whole frame of config 3 (BASELINE.json:configs[2], one WFS of the headline config 4): the real 800 x 800 pupil,
+    its 4632 valid subapertures with their radially elongated kernels, in the launch shape the library uses (145 CTAs of
+    32 spots, the last one ragged), through wk_table_kernel + wk_measure_kernel<10,0,0>: EVERY spot against the oracle."""
+    c = W.CONFIGS[3]
+    amp = W.pupil_mask(c)
+    yx = O.valid_list(amp, c.n, c.min_illum)
+    assert len(yx) == 4632
+    ph = W.phase_frames(c, 0, range(1))
+    K = W.elongation_kernels(c, 0, yx)
+    want, wimg = O.measure(ph, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K, stage=2)
+    out = wk_run(harnesses["wk"], tmp_path, c, 1, yx, 0, c.tau, ph, amp, K, 0, 2, 4)
+    assert out is not None
+    ierr, serr = compare(out[0], out[1], want, wimg, c.tau, 0, "config 3, whole frame")
+    assert ierr <= 2e-6 and serr <= 2e-5            # measured 3.4e-7 of the peak and 1.3e-6 px: two orders inside the tolerances
