@@ -31,6 +31,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <functional>
+#include <map>
 #include <random>
 #include <vector>
 
@@ -71,6 +72,7 @@ static ucontext_t g_main;
 static std::function<void()> g_body;
 static long g_switches = 0;
 static long g_progress = 0;             /* barriers released + threads finished */
+static std::map<size_t, std::vector<unsigned char *>> g_stack_pool;
 
 static void yield() { ++g_switches; swapcontext(&cur->ctx, &g_main); }
 
@@ -134,7 +136,12 @@ static bool run_ctas(const std::vector<Dim> &bids, int block, size_t smem_bytes,
             T.warp = &ctas[c].warps[t / 32];
             T.lane = t % 32;
             T.warp->live++;
-            T.stack = static_cast<unsigned char *>(std::malloc(stack_bytes));
+            if (!g_stack_pool[stack_bytes].empty()) {      /* stacks are reused from wave to wave and launch to launch */
+                T.stack = g_stack_pool[stack_bytes].back();
+                g_stack_pool[stack_bytes].pop_back();
+            } else {
+                T.stack = static_cast<unsigned char *>(std::malloc(stack_bytes));
+            }
             getcontext(&T.ctx);
             T.ctx.uc_stack.ss_sp = T.stack;
             T.ctx.uc_stack.ss_size = stack_bytes;
@@ -166,7 +173,7 @@ static bool run_ctas(const std::vector<Dim> &bids, int block, size_t smem_bytes,
         if (g_progress == before) { if (++idle_rounds > 2) return false; }     /* (stacks left to the exit) */
         else idle_rounds = 0;
     }
-    for (Thread &T : th) std::free(T.stack);
+    for (Thread &T : th) g_stack_pool[stack_bytes].push_back(T.stack);
     return true;
 }
 
