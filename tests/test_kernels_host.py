@@ -804,3 +804,23 @@ def test_config3_whole_frame_headline_kernel_on_the_host(tmp_path, harnesses):
     assert out is not None
     ierr, serr = compare(out[0], out[1], want, wimg, c.tau, 0, "config 3, whole frame")
     assert ierr <= 2e-6 and serr <= 2e-5            # measured 3.4e-7 of the peak and 1.3e-6 px: two orders inside the tolerances
+
+
+def test_config2_whole_frame_pruned_fft_kernel_on_the_host(tmp_path, harnesses):
+    """One whole frame of config 2 (BASELINE.json:configs[1]): the real 640 x 640 pupil with its 20 % obstruction, every
+    valid subaperture, through pruned_fft_kernel<32,16,0,tma> as a persistent launch of 8 CTAs with the dynamic deal
+    (chunks of four spots from the counter, boxes completed as late as the hardware may): EVERY spot against the oracle."""
+    c = W.CONFIGS[2]
+    amp = W.pupil_mask(c)
+    yx = O.valid_list(amp, c.n, c.min_illum)
+    ph = W.phase_frames(c, 0, range(1))
+    table = patch_table(amp, yx, c.n)
+    lit = (table[:, 0] & PATCH_LIT) != 0
+    assert 0.85 < lit.mean() < 0.98                                   # "93 % of config 2" read no amplitude (pruned_fft.cu)
+    want, wimg = O.measure(ph, amp, yx, c.n, c.P, c.b, tau=c.tau, stage=2)
+    out = pf_run(harnesses["pf"], tmp_path, c, 1, len(yx), 0, c.tau, ph, amp, table, 1, 4, 1, 8, 2, 11)
+    assert out is not None
+    words = out[2].split()
+    assert int(words[words.index("boxes") + 1]) == len(yx)
+    ierr, serr = compare(out[0], out[1], want, wimg, c.tau, 0, "config 2, whole frame")
+    assert ierr <= 5e-6 and serr <= 5e-5
