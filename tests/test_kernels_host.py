@@ -824,3 +824,19 @@ def test_config2_whole_frame_pruned_fft_kernel_on_the_host(tmp_path, harnesses):
     assert int(words[words.index("boxes") + 1]) == len(yx)
     ierr, serr = compare(out[0], out[1], want, wimg, c.tau, 0, "config 2, whole frame")
     assert ierr <= 5e-6 and serr <= 5e-5
+
+
+def test_config5_frame_subset_fft_kernel_on_the_host(tmp_path, harnesses):
+    """Config 5 (BASELINE.json:configs[4]: 1280 x 1280 pupil, n = 16, P = 64, 4 x 4 binning, kernels up to 6 arcsec) at its
+    real geometry, every seventh valid subaperture of one frame (pupil edge, obstruction edge and interior alike) with its
+    own elongation kernel, through wkf_kernel<16,0,0,tma> as a persistent launch of 3 CTAs with the dynamic deal."""
+    c = W.CONFIGS[5]
+    amp = W.pupil_mask(c)
+    yx = O.valid_list(amp, c.n, c.min_illum)[::7].copy()
+    ph = W.phase_frames(c, 0, range(1))
+    K = W.elongation_kernels(c, 0, yx)
+    want, wimg = O.measure(ph, amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K, stage=2)
+    out = wk_run(harnesses["wk"], tmp_path, c, 1, yx, 0, c.tau, ph, amp, K, 3, 2, 12, grid=3, lazy=1)
+    assert out is not None
+    ierr, serr = compare(out[0], out[1], want, wimg, c.tau, 0, "config 5, one frame, every 7th subaperture")
+    assert ierr <= 5e-6 and serr <= 5e-5
