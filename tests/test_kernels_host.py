@@ -307,6 +307,11 @@ def test_lag_domain_kernels_whole_on_the_host(tmp_path, harnesses):
             else:
                 assert np.array_equal(first[0], out[0]) and np.array_equal(first[1], out[1]), f"{label}: depends on the thread order"
             runs += 1
+        if with_k and c.n == 10:
+            # the headline instance under five more random interleavings of its 160-thread CTAs
+            for seed in range(5):
+                out = wk_run(exe, tmp_path, c, T, yx, mode, tau, ph, amp, K, 0, 2, 9000 + seed)
+                assert out is not None and np.array_equal(first[0], out[0]) and np.array_equal(first[1], out[1]), seed
         if generic_too and mode == 0:
             # the size-generic kernel: one frame, an independently written cross-check of the same table
             out = wk_run(exe, tmp_path, c, 1, yx, mode, tau, ph[:1], amp, K, 1, 2, 5)
