@@ -72,6 +72,8 @@ static ucontext_t g_main;
 static std::function<void()> g_body;
 static long g_switches = 0;
 static long g_progress = 0;             /* barriers released + threads finished */
+static int g_order = 0;
+static std::minstd_rand g_yield_rng(1408u);
 static std::map<size_t, std::vector<unsigned char *>> g_stack_pool;
 
 static void yield() { ++g_switches; swapcontext(&cur->ctx, &g_main); }
@@ -122,6 +124,8 @@ static bool run_ctas(const std::vector<Dim> &bids, int block, size_t smem_bytes,
 {
     const int grid = (int)bids.size();
     const int wpc = (block + 31) / 32;
+    g_order = (int)order;
+    g_yield_rng.seed(seed + 17u);
     std::vector<Cta> ctas(grid);
     std::vector<Thread> th((size_t)grid * block);
     for (int c = 0; c < grid; ++c) {
@@ -277,7 +281,16 @@ template <class T> static inline T __shfl_down_sync(unsigned, T v, int d)
 }
 
 template <class T> static inline T __ldg(const T *p) { return *p; }
-static inline int atomicAdd(int *p, int v) { const int o = *p; *p += v; return o; }
+/* under the random order a thread may also be switched out right before an atomic: the warps of the dynamic deal then
+ * reach the chunk counter (and its re-arming by the last warp out) in every interleaving, not only at barriers */
+static inline int atomicAdd(int *p, int v)
+{
+    if (simt::g_order == simt::RANDOM && (simt::g_yield_rng() & 1u)) simt::yield();
+    ++simt::g_progress;              /* an atomic performed is progress (dead-lock detection) */
+    const int o = *p;
+    *p += v;
+    return o;
+}
 using std::max;
 using std::min;
 
