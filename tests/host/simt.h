@@ -15,6 +15,9 @@
  * row r at chunk q ^ ((r >> 1) & 3)), performed either at once or -- `lazy_tma` -- only when a thread waits on its
  * mbarrier: the earliest and the latest moment the hardware may complete it.
  *
+ * Under the random order a thread may also be switched out right before an atomicAdd.  CTAs of a 1-D launch are all
+ * resident from the start (launch); 2-D launches run in waves of CTAs (launch2d).  Coroutine stacks are pooled.
+ *
  * Test infrastructure only (tests/test_kernels_host.py); nothing of the product uses it.
  */
 #ifndef SHWFS_TEST_SIMT_H_
