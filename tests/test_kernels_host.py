@@ -607,9 +607,9 @@ def test_sodium_layers_and_noise_instances_whole_on_the_host(tmp_path, harnesses
         plain = O.measure(ph if shared else ph[:, 0], amp, yx, c.n, c.P, c.b, tau=c.tau, kernels=K)
         assert np.abs(want - plain).max() > 0.05                # the sub-layers do change the spots
         q, sw, g = sodium_tables(c, yx, sod)
-        for kernel in (0, 2):
+        for kernel in ((0, 1, 2) if L == 3 else (0, 2)):      # 1: the size-generic kernel carries the sub-layers too
             first = None
-            for order in (0, 2):
+            for order in ((2,) if kernel == 1 else (0, 2)):
                 label = f"L={L} shared={shared} kernel={kernel} order={order}"
                 out = wk_run(exe, tmp_path, c, T, yx, 0, c.tau, ph, amp, K, kernel, order, 31 + runs, L=L, sod_q=q, sod_sw=sw,
                              sod_g=g, shared=int(shared))
@@ -643,7 +643,7 @@ def test_sodium_layers_and_noise_instances_whole_on_the_host(tmp_path, harnesses
         assert float((np.abs(out[2] - wimg) / peak).max()) <= 1e-4, label
         assert float(np.abs(out[0] - want).max()) <= 1e-3, label
         runs += 1
-    assert runs == 11
+    assert runs == 12
 
 
 # ---------------------------------------------------------------- loop.cu: the closed-loop neighbours (FP32 kernels)
