@@ -534,6 +534,10 @@ def test_pyramid_kernels_whole_on_the_host(tmp_path, harnesses):
     ax = np.arange(N) + 0.5 - N / 2
     amp = ((np.hypot(ax[None, :], ax[:, None]) <= N / 2) * rng.uniform(0.4, 1.0, (N, N))).astype(np.float32)
     cases.append((rng.normal(0, 2.0, (1, N, N)).astype(np.float32), amp, 1024, 200, 4, 1.5, 2, 0.9 * N, 0.6, 0.3, (2,)))
+    # the LBT-like workload (240 x 240 pupil, Np = 1024, separation 256, 8 x 8 binning) with 4 of its 16
+    # modulation points, one frame of its residual-like phase
+    p = W.PYRAMIDS["lbt"]
+    cases.append((W.pyramid_frames(p, range(1), 0.3), W.pyramid_mask(p), p.Np, p.s, p.bp, p.r_mod, 4, p.D_pix, 1.0, 0.5, (2,)))
     # unmodulated
     N = 36
     ax = np.arange(N) + 0.5 - N / 2
@@ -557,11 +561,11 @@ def test_pyramid_kernels_whole_on_the_host(tmp_path, harnesses):
             else:
                 assert np.array_equal(first[0], got) and np.array_equal(first[1], q), f"{label}: depends on the thread order"
             runs += 1
-    assert runs == 5
+    assert runs == 6
 
     # the exchange inside a line transform without its __syncwarp between the writes and the reads
     mutant = harnesses["pyr_mut"]
-    ph, amp, Np, s, bp, r_mod, K, D_pix, c_phi, min_illum, _ = cases[2]
+    ph, amp, Np, s, bp, r_mod, K, D_pix, c_phi, min_illum, _ = cases[3]
     yx = OP.valid_pixels(amp, bp, min_illum)
     want, wq = OP.measure(ph, amp, yx, Np, s, bp, r_mod, K, D_pix, c_phi=np.float32(c_phi), return_quadrants=True)
     caught = 0
