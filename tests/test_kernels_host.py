@@ -470,6 +470,17 @@ def test_literal_chain_kernels_whole_on_the_host(tmp_path, harnesses):
                 runs += 1
     assert runs == 18
 
+    # P = 8 (the smallest size the literal chain accepts): 16 spots per CTA, four per warp, reductions inside 8 lanes
+    c8 = dataclasses.replace(W.CONFIGS[1], n=4, P=8, S=10, N=40, dx=0.2, screen_M=256)
+    amp = W.pupil_mask(c8)
+    yx = O.valid_list(amp, c8.n, c8.min_illum)
+    ph = W.phase_frames(c8, 0, range(3))
+    want, wimg = O.measure(ph, amp, yx, c8.n, c8.P, c8.b, tau=0.05, stage=2)
+    for order in (0, 2):
+        out = lit_run(exe, tmp_path, c8, 3, yx, 0, 0.05, ph, amp, None, 2, order, 8)
+        assert out is not None
+        compare(out[0], out[1], want, wimg, 0.05, 0, f"P = 8 order={order}")
+
     # without the barrier between the centred image written to shared memory and the binning that reads it
     mutant = harnesses["lit_mut"]
     c = small_config(3, 8)
