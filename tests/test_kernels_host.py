@@ -860,3 +860,28 @@ def test_config5_frame_subset_fft_kernel_on_the_host(tmp_path, harnesses):
     assert out is not None
     ierr, serr = compare(out[0], out[1], want, wimg, c.tau, 0, "config 5, one frame, every 7th subaperture")
     assert ierr <= 5e-6 and serr <= 5e-5
+
+
+def test_tensor_core_operand_preparation_on_the_host(tmp_path):
+    """dm_umma.cu's operand kernels (TF32 hi/lo split into canonical K-major tiles) on the host SIMT machine
+    (tests/host/umma_prep_harness.cpp): layout, padding, TF32-ness, and the 3-term product summed exactly from the
+    tiles against the plain GEMM -- DESIGN.md 6.5's figures for the split (1.7e-7 of peak) and a single pass (4.9e-4)."""
+    if shutil.which("g++") is None or not (CUDA_INC / "cuda_runtime.h").exists():
+        pytest.skip("needs g++ and the CUDA headers")
+    src = (CSRC / "dm_umma.cu").read_text()
+    block = cut(src, "constexpr int UM_KB = 8;", "__device__ __forceinline__ uint64_t umma_desc(")
+    block, k = re.subn(r"    uint32_t r;\n    asm\(\"cvt\.rna\.tf32\.f32 %0, %1;\" : \"=r\"\(r\) : \"f\"\(x\)\);\n    return __uint_as_float\(r\);\n",
+                       "    return host_tf32_rna(x);\n", block)
+    assert k == 1 and "umma_split_modes_kernel(" in block and "umma_split_coef_kernel(" in block and "asm" not in block
+    (tmp_path / "umma_prep_extract.inc").write_text(block)
+    exe = tmp_path / "umma_prep_harness"
+    r = subprocess.run(["g++", "-std=c++17", "-O1", "-ffp-contract=off", f"-I{CUDA_INC}", f"-I{tmp_path}", "-Wno-attributes", "-Wno-psabi",
+                        "-o", str(exe), str(ROOT / "tests" / "host" / "umma_prep_harness.cpp")], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-3000:]
+    # (nsub, M, n*n, padded n*n, frames): the three sizes with an instance; M and T ragged against the 8-mode stage / 128-frame tile
+    for args in ((5, 37, 100, 112, 150), (3, 16, 64, 64, 128), (2, 21, 256, 256, 9)):
+        run = subprocess.run([str(exe), *map(str, args)], capture_output=True, text=True, timeout=600)
+        assert run.returncode == 0 and run.stdout.startswith("ok "), (args, run.stdout[-500:] + run.stderr[-500:])
+        split, single = (float(w) for w in run.stdout.split()[1:3])
+        assert split <= 5e-7, (args, split)                  # fp32-class: the dropped lo x lo term and the lo roundings
+        assert 5e-5 <= single <= 2e-3, (args, single)        # what one TF32 pass would have given
