@@ -1,10 +1,15 @@
-"""Whole kernels of csrc/ on the host: the kernel is cut out of its .cu file as text, compiled by g++ with the headers
+"""Whole kernels of csrc/ on the host: each kernel is cut out of its .cu file as text, compiled by g++ with the headers
 it includes as they are, and run thread by thread on the coroutine SIMT machine of tests/host/simt.h (shared memory,
 shuffles, __syncwarp / __syncthreads, the chunk counter of the dynamic deal, TMA boxes with their swizzle and
-mbarriers) on the same seeded inputs as the float64 oracle: binned images within 1e-4 of the spot peak, slopes within
-1e-3 px (north_star), for every spot.  Each case runs under three thread orders (ascending, descending, seeded
-random between synchronisation points) and must give bit-identical results: a barrier the code needs and does not
-have shows up as a difference.  CPU-side parity of device code, thread mapping included: no GPU."""
+mbarriers, cp.async batches) on the same seeded inputs as the float64 oracles: Shack-Hartmann kernels (pruned_fft.cu,
+wk.cu, wk_fft.cu, literal.cu; the sodium / noise / DM-residual instances) binned images within 1e-4 of the spot peak
+and slopes within 1e-3 px (north_star) for every spot; pyramid.cu quadrants 1e-4 of peak, signals 2e-4; loop.cu
+against the definitions C1 / C2 of oracle/closed_loop.py; the operand kernels of dm_umma.cu against the plain GEMM.
+Each case runs under up to three thread orders (ascending, descending, seeded random between synchronisation points)
+and must give bit-identical results: a barrier the code needs and does not have shows up as a difference -- and one
+mutant per kernel family, built from the same text with such a barrier removed, must fail (MUTANTS).  Whole frames at
+BASELINE.json's geometry: config 3 (every spot), config 2 (every spot), config 5 (every 7th subaperture), the LBT-like
+pyramid.  CPU-side parity of device code, thread mapping included: no GPU."""
 import dataclasses
 import re
 import shutil
